@@ -1,0 +1,163 @@
+/* starkv.h -- C ABI of libstarkv.so: decode attention read directly from a low-rank,
+ * mixed-precision-quantised KV cache (STAR-KV, arxiv/paper_2606_08382), hand-written CUDA for
+ * sm_100a.  Citations are PAPER.md:L<line> (+ section / equation); "DESIGN.md" is the repo's
+ * design file (cache page format v1, readings of the paper).
+ *
+ * Conventions
+ *   - Every `const void*` / `void*` data argument is a DEVICE pointer unless the name ends in
+ *     `_host` or the comment says HOST.  The descriptor and its rank tables are HOST memory and
+ *     are copied at starkv_create.
+ *   - The caller owns every buffer.  The library allocates nothing on the device after
+ *     starkv_create, keeps no reference to caller buffers between calls, never mutates
+ *     `seq_lens` or `block_table`.
+ *   - Every call only enqueues work on the context's CUDA stream and returns (no host sync);
+ *     all entry points are CUDA-graph capturable.  The `_host` variants are the exception: they
+ *     copy host buffers in, run, copy the result out and synchronise the stream.
+ *   - Return value: 0 = STARKV_OK, negative = error (see enum).  No exception or abort crosses
+ *     the ABI.  Inputs must be finite; NaN/Inf in the data are not detected.
+ *   - Device pointers must be 16-byte aligned; the page pool 128-byte aligned.
+ */
+#ifndef STARKV_H
+#define STARKV_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+enum {
+  STARKV_OK = 0,
+  STARKV_ERR_INVALID_ARG = -1, /* null / misaligned pointer, bad rank table, bad sizes          */
+  STARKV_ERR_UNSUPPORTED = -2, /* bit pair, layout_id, page_tokens or head count not built      */
+  STARKV_ERR_WORKSPACE = -3,   /* workspace_bytes smaller than starkv_workspace_bytes()         */
+  STARKV_ERR_CUDA = -4         /* a CUDA runtime call failed; text via starkv_last_error()      */
+};
+
+/* Cache / attention descriptor (POD, HOST memory).
+ *   Keys: head-wise decomposition, one latent cache L_k^h [l, r_h] and one reconstruction
+ *   B_k^h [r_h, d_h] per KV head, rank adaptive per head (§4.3.1, §4.3.3).
+ *   Values: joint decomposition, one latent L_v [l, r_v] per token shared by all heads,
+ *   reconstruction B_v [r_v, H_kv*d_h] (same passages).
+ *   Precision split: the leading rank_*_hi channels (highest singular values) are stored at
+ *   bits_hi, the rest at bits_lo, quantised per token (§4.4, Eq.12). */
+typedef struct {
+  int32_t n_q_heads;        /* H_q                                                             */
+  int32_t n_kv_heads;       /* H_kv, divides H_q; query head i reads KV head i / (H_q/H_kv)     */
+  int32_t head_dim;         /* d_h, multiple of 16, <= 256                                      */
+  const int32_t* rank_k;    /* HOST [n_kv_heads] r_h: multiple of 8, 8 <= r_h <= head_dim       */
+  const int32_t* rank_k_hi; /* HOST [n_kv_heads] leading high-precision channels: multiple of 8,
+                               0 < r_hi <= r_h (ignored when bits_hi == 16)                     */
+  int32_t rank_v;           /* r_v: multiple of 8, <= n_kv_heads*head_dim                       */
+  int32_t rank_v_hi;        /* multiple of 8, 0 < rank_v_hi <= rank_v                           */
+  int32_t bits_hi, bits_lo; /* {16,16} fp16 latents; {8,4}; {8,8}; {4,4}                        */
+  int32_t page_tokens;      /* tokens per cache page, multiple of 16 (fast path: 64)            */
+  int32_t layout_id;        /* 1 = DESIGN.md "Cache page format v1"                             */
+  float sm_scale;           /* softmax scale; <= 0 selects 1/sqrt(head_dim)      */
+} starkv_desc;
+
+typedef struct starkv_ctx starkv_ctx; /* opaque: descriptor copy, page byte map, stream */
+
+/* Create a context.  `cuda_stream` is a cudaStream_t (NULL = default stream) on the current
+ * device; all later calls enqueue on it.  Errors: INVALID_ARG, UNSUPPORTED, CUDA. */
+int starkv_create(starkv_ctx** out, const starkv_desc* desc, void* cuda_stream);
+void starkv_destroy(starkv_ctx* ctx);
+
+/* Bytes of one cache page (DESIGN.md format v1: every block padded to 16 B, the page to 128 B). */
+size_t starkv_page_bytes(const starkv_ctx* ctx);
+
+/* Bytes of scratch starkv_decode_attn needs for `batch` sequences of at most `max_pages` pages
+ * (latent-space queries + split-K partials).  Deterministic in (ctx, batch, max_pages). */
+size_t starkv_workspace_bytes(const starkv_ctx* ctx, int batch, int max_pages);
+
+/* Bytes of scratch starkv_append needs for n_new tokens (fp16 latents of the new tokens). */
+size_t starkv_append_workspace_bytes(const starkv_ctx* ctx, int n_new);
+
+/* starkv_pack: quantise + pack caller latents into consecutive pages (rows A2-A4 of the hot
+ * path on caller-supplied latents).  PAPER.md Eq.12: Z^ = [Q_hi(Z_out) Q_lo(Z_in)], per
+ * token; reading of Q in DESIGN.md (symmetric absmax, s = RN_fp16(max|z|/qmax),
+ * c = clamp(RNE(z/s), +-qmax), stored offset-binary).
+ *   latents_k  fp16 [n_tokens, sum r_h] row-major (head h = columns koff[h] .. koff[h]+r_h)
+ *   latents_v  fp16 [n_tokens, r_v]
+ *   pages_out  ceil(n_tokens/page_tokens) pages, fully written: slots >= n_tokens and all
+ *              padding bytes are zero, so whole pages are bit-comparable. */
+int starkv_pack(starkv_ctx* ctx, const void* latents_k, const void* latents_v, int n_tokens,
+                void* pages_out);
+
+/* starkv_unpack: inverse of starkv_pack on the first n_tokens slots of consecutive pages.
+ * Any output may be NULL.
+ *   codes_out    int8  [n_tokens, sum r_h + r_v] signed codes c (quantised modes only)
+ *   scales_out   fp16 bits [n_tokens, 2*H_kv + 2]: K (h, blk) then V (blk) (quantised only)
+ *   dequant_out  fp32  [n_tokens, sum r_h + r_v] = c*s exactly (or the fp16 latent) */
+int starkv_unpack(starkv_ctx* ctx, const void* pages_in, int n_tokens, int8_t* codes_out,
+                  uint16_t* scales_out, float* dequant_out);
+
+/* starkv_append: compress-on-append.  PAPER.md §3.2: K' = x (Sigma V)_K per head,
+ * V' = x (Sigma V)_V joint; then Eq.12 quantisation and a paged write.  Token j of the n_new
+ * new tokens goes to sequence seq_ids[j] at position positions[j]: page
+ * block_table[seq_ids[j]*max_pages + positions[j]/page_tokens], slot positions[j]%page_tokens.
+ * Other slots of the page are left untouched.  KV head h reads row j of its input at
+ * k_new + j*k_row_stride + h*k_head_stride (strides in ELEMENTS), width d_in_k, and multiplies
+ * by columns [koff[h], koff[h]+r_h) of A_k:
+ *   dense-KV mode   k_head_stride = head_dim, d_in_k = head_dim, d_in_v = H_kv*head_dim
+ *   hidden mode     k_head_stride = 0, k_new = v_new = x, d_in_k = d_in_v = d_model
+ *   A_k fp16 [d_in_k, sum r_h] row-major, A_v fp16 [d_in_v, r_v] row-major; fp32 accumulation,
+ *   one rounding to fp16, then quantise.  seq_ids / positions / block_table: device int32.
+ * Two new tokens must not target the same (sequence, position). */
+int starkv_append(starkv_ctx* ctx, void* page_pool, const int32_t* block_table, int max_pages,
+                  const int32_t* seq_ids, const int32_t* positions, int n_new,
+                  const void* k_new, int64_t k_row_stride, int64_t k_head_stride, int d_in_k,
+                  const void* v_new, int64_t v_row_stride, int d_in_v, const void* A_k,
+                  const void* A_v, void* workspace, size_t workspace_bytes);
+
+/* starkv_decode_attn: one decode step of attention read directly from the latent cache
+ * (rows D1-D9).  For sequence b with l = seq_lens[b], query head i, KV head g = i/(H_q/H_kv):
+ *   q~_i = sm_scale * q_i B_k^gT            (latent-space query; §3.3 L62-68 reordering)
+ *   s_t  = q~_i . L_k^g[t]   t in [0, l)     (== sm_scale * q_i . (L_k^g B_k^g)[t], L58)
+ *   p    = softmax(s)                        (§3.1)
+ *   out_i = ((p L_v)) B_v[:, g*d_h:(g+1)*d_h]   ("(p V') U_V")
+ * with L = code*scale dequantised in registers.  l = 0 gives a zero row.  No RoPE (A1).
+ *   q fp16 [batch, H_q, d_h]; B_k fp16 [sum r_h, d_h]; B_v fp16 [r_v, H_kv*d_h];
+ *   block_table int32 [batch, max_pages]; seq_lens int32 [batch], seq_lens[b] <= max_pages*P;
+ *   out fp16 [batch, H_q, d_h]. */
+int starkv_decode_attn(starkv_ctx* ctx, const void* q, const void* page_pool,
+                       const int32_t* block_table, int max_pages, const int32_t* seq_lens,
+                       int batch, const void* B_k, const void* B_v, void* workspace,
+                       size_t workspace_bytes, void* out);
+
+/* Same operation through the plain scalar kernel (any page_tokens / head count; fp32 math,
+ * exact dequantisation).  Slow; used as a second implementation in tests and for shapes the
+ * tensor-core kernel does not cover. */
+int starkv_decode_attn_generic(starkv_ctx* ctx, const void* q, const void* page_pool,
+                               const int32_t* block_table, int max_pages,
+                               const int32_t* seq_lens, int batch, const void* B_k,
+                               const void* B_v, void* workspace, size_t workspace_bytes,
+                               void* out);
+
+/* HOST-buffer variant (bench.py "e2e"): q_host / seq_lens_host / out_host are HOST pointers
+ * (pinned for best speed); the call copies q and seq_lens to device scratch inside `workspace`
+ * (sized by starkv_workspace_bytes, which reserves room for them), runs the decode step,
+ * copies `out` back and synchronises the stream.  The cache, block table and factors stay on
+ * the device (they are the resident state of a serving process). */
+int starkv_decode_attn_host(starkv_ctx* ctx, const void* q_host, const void* page_pool,
+                            const int32_t* block_table, int max_pages,
+                            const int32_t* seq_lens_host, int batch, const void* B_k,
+                            const void* B_v, void* workspace, size_t workspace_bytes,
+                            void* out_host);
+
+/* Tuning knob (0 = automatic): number of split-K ranges per sequence for the next decode calls. */
+int starkv_set_splits(starkv_ctx* ctx, int n_splits);
+
+/* Number of kernel launches the last decode/append/pack/unpack call enqueued (for bench.py's
+ * gpu_launches claim). */
+int starkv_last_launches(const starkv_ctx* ctx);
+
+const char* starkv_strerror(int code);
+/* Text of the last CUDA error seen by this context ("" if none). */
+const char* starkv_last_error(const starkv_ctx* ctx);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* STARKV_H */

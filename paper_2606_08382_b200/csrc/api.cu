@@ -1,0 +1,151 @@
+// C ABI of libstarkv.so (include/starkv.h): argument checks, context, dispatch.  No compute here.
+#include <stdio.h>
+#include <stdlib.h>
+#include <string.h>
+
+#include "ctx.h"
+
+int sk_cuda_fail(starkv_ctx* ctx, cudaError_t e, const char* what) {
+  if (ctx) snprintf(ctx->err, sizeof(ctx->err), "%s: %s (%s)", cudaGetErrorName(e), cudaGetErrorString(e), what);
+  (void)cudaGetLastError();   // clear the non-sticky error state
+  return STARKV_ERR_CUDA;
+}
+
+static bool aligned16(const void* p) { return ((uintptr_t)p & 15) == 0; }
+
+extern "C" {
+
+int starkv_create(starkv_ctx** out, const starkv_desc* d, void* cuda_stream) {
+  if (!out) return STARKV_ERR_INVALID_ARG;
+  *out = nullptr;
+  if (!d || !d->rank_k) return STARKV_ERR_INVALID_ARG;
+  if (d->layout_id != 1) return STARKV_ERR_UNSUPPORTED;
+  if (d->bits_hi != 16 && !d->rank_k_hi) return STARKV_ERR_INVALID_ARG;
+  if (d->n_kv_heads <= 0 || d->n_kv_heads > STARKV_MAX_KV_HEADS) return STARKV_ERR_INVALID_ARG;
+  starkv_ctx* ctx = (starkv_ctx*)calloc(1, sizeof(starkv_ctx));
+  if (!ctx) return STARKV_ERR_INVALID_ARG;
+  const float sm = d->sm_scale > 0.f ? d->sm_scale : 1.0f / sqrtf((float)(d->head_dim > 0 ? d->head_dim : 1));
+  const int rc = starkv_build_layout(&ctx->L, d->n_q_heads, d->n_kv_heads, d->head_dim, d->rank_k, d->rank_k_hi, d->rank_v,
+                                     d->rank_v_hi, d->bits_hi, d->bits_lo, d->page_tokens, sm);
+  if (rc != 0) {
+    free(ctx);
+    return rc == -2 ? STARKV_ERR_UNSUPPORTED : STARKV_ERR_INVALID_ARG;
+  }
+  ctx->stream = (cudaStream_t)cuda_stream;
+  cudaError_t e = cudaGetDevice(&ctx->device);
+  if (e == cudaSuccess) e = cudaDeviceGetAttribute(&ctx->n_sm, cudaDevAttrMultiProcessorCount, ctx->device);
+  if (e == cudaSuccess) e = cudaDeviceGetAttribute(&ctx->smem_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, ctx->device);
+  if (e != cudaSuccess) {   // no usable device: fail loudly, there is no CPU path
+    (void)cudaGetLastError();
+    free(ctx);
+    return STARKV_ERR_CUDA;
+  }
+  sk_fast_plan(ctx);
+  *out = ctx;
+  return STARKV_OK;
+}
+
+void starkv_destroy(starkv_ctx* ctx) { free(ctx); }
+
+size_t starkv_page_bytes(const starkv_ctx* ctx) { return ctx ? (size_t)ctx->L.page_bytes : 0; }
+
+size_t starkv_workspace_bytes(const starkv_ctx* ctx, int batch, int max_pages) {
+  if (!ctx || batch <= 0 || max_pages <= 0) return 0;
+  SkWorkspace w;
+  sk_plan_workspace(ctx, batch, max_pages, &w);
+  return w.total;
+}
+
+size_t starkv_append_workspace_bytes(const starkv_ctx* ctx, int n_new) { return ctx ? sk_append_ws_bytes(ctx, n_new) : 0; }
+
+int starkv_pack(starkv_ctx* ctx, const void* lk, const void* lv, int n_tokens, void* pages) {
+  if (!ctx) return STARKV_ERR_INVALID_ARG;
+  if (n_tokens > 0 && (!aligned16(lk) || !aligned16(lv) || !aligned16(pages))) return STARKV_ERR_INVALID_ARG;
+  return sk_pack(ctx, lk, lv, n_tokens, pages);
+}
+
+int starkv_unpack(starkv_ctx* ctx, const void* pages, int n_tokens, int8_t* codes, uint16_t* scales, float* deq) {
+  if (!ctx) return STARKV_ERR_INVALID_ARG;
+  if (n_tokens > 0 && !aligned16(pages)) return STARKV_ERR_INVALID_ARG;
+  return sk_unpack(ctx, pages, n_tokens, codes, scales, deq);
+}
+
+int starkv_append(starkv_ctx* ctx, void* pool, const int32_t* table, int max_pages, const int32_t* seq_ids,
+                  const int32_t* positions, int n_new, const void* k_new, int64_t k_row_stride, int64_t k_head_stride,
+                  int d_in_k, const void* v_new, int64_t v_row_stride, int d_in_v, const void* A_k, const void* A_v,
+                  void* ws, size_t ws_bytes) {
+  if (!ctx) return STARKV_ERR_INVALID_ARG;
+  if (n_new > 0 && (!aligned16(pool) || !aligned16(ws))) return STARKV_ERR_INVALID_ARG;
+  return sk_append(ctx, pool, table, max_pages, seq_ids, positions, n_new, k_new, k_row_stride, k_head_stride, d_in_k,
+                   v_new, v_row_stride, d_in_v, A_k, A_v, ws, ws_bytes);
+}
+
+static int check_decode_args(starkv_ctx* ctx, const void* q, const void* pool, const int32_t* table, int max_pages,
+                             const int32_t* seq_lens, int batch, const void* B_k, const void* B_v, void* ws, void* out) {
+  if (!ctx || batch <= 0 || max_pages <= 0) return STARKV_ERR_INVALID_ARG;
+  if (!q || !pool || !table || !seq_lens || !B_k || !B_v || !ws || !out) return STARKV_ERR_INVALID_ARG;
+  if (!aligned16(q) || !aligned16(B_k) || !aligned16(B_v) || !aligned16(ws) || !aligned16(out)) return STARKV_ERR_INVALID_ARG;
+  if (((uintptr_t)pool & 127) != 0) return STARKV_ERR_INVALID_ARG;
+  return STARKV_OK;
+}
+
+int starkv_decode_attn(starkv_ctx* ctx, const void* q, const void* pool, const int32_t* table, int max_pages,
+                       const int32_t* seq_lens, int batch, const void* B_k, const void* B_v, void* ws, size_t ws_bytes,
+                       void* out) {
+  const int rc = check_decode_args(ctx, q, pool, table, max_pages, seq_lens, batch, B_k, B_v, ws, out);
+  if (rc) return rc;
+  if (ctx->fast_ok) return sk_decode_fast(ctx, q, pool, table, max_pages, seq_lens, batch, B_k, B_v, ws, ws_bytes, out);
+  return sk_decode_generic(ctx, q, pool, table, max_pages, seq_lens, batch, B_k, B_v, ws, ws_bytes, out);
+}
+
+int starkv_decode_attn_generic(starkv_ctx* ctx, const void* q, const void* pool, const int32_t* table, int max_pages,
+                               const int32_t* seq_lens, int batch, const void* B_k, const void* B_v, void* ws,
+                               size_t ws_bytes, void* out) {
+  const int rc = check_decode_args(ctx, q, pool, table, max_pages, seq_lens, batch, B_k, B_v, ws, out);
+  if (rc) return rc;
+  return sk_decode_generic(ctx, q, pool, table, max_pages, seq_lens, batch, B_k, B_v, ws, ws_bytes, out);
+}
+
+int starkv_decode_attn_host(starkv_ctx* ctx, const void* q_host, const void* pool, const int32_t* table, int max_pages,
+                            const int32_t* seq_lens_host, int batch, const void* B_k, const void* B_v, void* ws,
+                            size_t ws_bytes, void* out_host) {
+  if (!ctx || batch <= 0 || max_pages <= 0 || !q_host || !seq_lens_host || !out_host || !ws) return STARKV_ERR_INVALID_ARG;
+  SkWorkspace w;
+  sk_plan_workspace(ctx, batch, max_pages, &w);
+  if (ws_bytes < w.total) return STARKV_ERR_WORKSPACE;
+  const size_t qbytes = (size_t)batch * ctx->L.n_q_heads * ctx->L.head_dim * 2;
+  const size_t qb = (qbytes + 255) / 256 * 256;
+  uint8_t* dq = (uint8_t*)ws + w.host_off;
+  uint8_t* dout = dq + qb;
+  int32_t* dlen = (int32_t*)(dout + qb);
+  SK_CUDA_CHECK(ctx, cudaMemcpyAsync(dq, q_host, qbytes, cudaMemcpyHostToDevice, ctx->stream));
+  SK_CUDA_CHECK(ctx, cudaMemcpyAsync(dlen, seq_lens_host, (size_t)batch * 4, cudaMemcpyHostToDevice, ctx->stream));
+  const int rc = starkv_decode_attn(ctx, dq, pool, table, max_pages, dlen, batch, B_k, B_v, ws, ws_bytes, dout);
+  if (rc) return rc;
+  SK_CUDA_CHECK(ctx, cudaMemcpyAsync(out_host, dout, qbytes, cudaMemcpyDeviceToHost, ctx->stream));
+  SK_CUDA_CHECK(ctx, cudaStreamSynchronize(ctx->stream));
+  return STARKV_OK;
+}
+
+int starkv_set_splits(starkv_ctx* ctx, int n_splits) {
+  if (!ctx || n_splits < 0) return STARKV_ERR_INVALID_ARG;
+  ctx->n_splits_override = n_splits;
+  return STARKV_OK;
+}
+
+int starkv_last_launches(const starkv_ctx* ctx) { return ctx ? ctx->last_launches : 0; }
+
+const char* starkv_strerror(int code) {
+  switch (code) {
+    case STARKV_OK: return "ok";
+    case STARKV_ERR_INVALID_ARG: return "invalid argument";
+    case STARKV_ERR_UNSUPPORTED: return "unsupported configuration";
+    case STARKV_ERR_WORKSPACE: return "workspace too small";
+    case STARKV_ERR_CUDA: return "CUDA error";
+    default: return "unknown error";
+  }
+}
+
+const char* starkv_last_error(const starkv_ctx* ctx) { return ctx ? ctx->err : ""; }
+
+}  // extern "C"

@@ -1,0 +1,410 @@
+// Page codec and compress-on-append kernels (rows A1-A4 and U of the hot path).
+//   PAPER.md §3.2 L58 (K' = x (Sigma V)_K per head, V' = x (Sigma V)_V joint),
+//   PAPER.md §4.4 L204-210 / Eq.12 L208 (leading channels at bits_hi, trailing at bits_lo, per token),
+//   DESIGN.md "Cache page format v1" (token-major K blocks, channel-major V blocks, offset-binary fields).
+#include "common.cuh"
+#include "ctx.h"
+
+namespace {
+
+// ---------------------------------------------------------------------------------------------
+// pack: one CTA builds one whole page image in shared memory, then writes it out coalesced.
+// ---------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256) pack_kernel(const __grid_constant__ StarkvLayout L,
+                                                   const __half* __restrict__ lk,
+                                                   const __half* __restrict__ lv, int n_tokens,
+                                                   uint8_t* __restrict__ pages) {
+  extern __shared__ __align__(16) uint8_t img[];
+  float* vs = reinterpret_cast<float*>(img + L.page_bytes);  // [2][P] value scales as float
+  const int P = L.page_tokens;
+  const int page = blockIdx.x;
+  const int t0 = page * P;
+  const bool quant = L.bits_hi != 16;
+
+  for (int i = threadIdx.x; i < L.page_bytes / 16; i += blockDim.x) reinterpret_cast<uint4*>(img)[i] = make_uint4(0, 0, 0, 0);
+  __syncthreads();
+
+  // keys: one (slot, head, blk) unit per thread -> whole bytes of a token-major row
+  for (int u = threadIdx.x; u < L.n_kv_heads * 2 * P; u += blockDim.x) {
+    const int slot = u % P, hb = u / P, h = hb >> 1, blk = hb & 1;
+    const int tok = t0 + slot;
+    if (tok >= n_tokens) continue;
+    const int n = blk ? L.k_lo_n[h] : L.k_hi_n[h];
+    if (n == 0) continue;
+    const __half* z = lk + (size_t)tok * L.sum_rank_k + L.koff[h] + (blk ? L.k_hi_n[h] : 0);
+    const int bits = blk ? L.bits_lo : L.bits_hi;
+    uint8_t* row = img + (blk ? L.k_lo_off[h] : L.k_hi_off[h]) + (size_t)slot * (n * bits / 8);
+    if (!quant) {
+      for (int c = 0; c < n; ++c) reinterpret_cast<__half*>(row)[c] = z[c];
+      continue;
+    }
+    float amax = 0.f;
+    for (int c = 0; c < n; ++c) amax = fmaxf(amax, fabsf(__half2float(z[c])));
+    const int qmax = sk_qmax(bits);
+    const __half s16 = sk_scale_of(amax, qmax);
+    const float s = __half2float(s16);
+    reinterpret_cast<uint16_t*>(img + L.k_scale_off)[(h * 2 + blk) * P + slot] = sk_half_bits(s16);
+    if (bits == 8) {
+      for (int c = 0; c < n; ++c) row[c] = (uint8_t)(sk_code_of(__half2float(z[c]), s, qmax) + 128);
+    } else {
+      for (int c = 0; c < n; c += 2) {
+        const int u0 = sk_code_of(__half2float(z[c]), s, qmax) + 8;
+        const int u1 = sk_code_of(__half2float(z[c + 1]), s, qmax) + 8;
+        row[c >> 1] = (uint8_t)(u0 | (u1 << 4));
+      }
+    }
+  }
+
+  // value scales: one (slot, blk) unit per thread
+  if (quant) {
+    for (int u = threadIdx.x; u < 2 * P; u += blockDim.x) {
+      const int slot = u % P, blk = u / P;
+      const int tok = t0 + slot;
+      const int n = blk ? L.v_lo_n : L.v_hi_n;
+      float s = 0.f;
+      if (tok < n_tokens && n > 0) {
+        const __half* z = lv + (size_t)tok * L.rank_v + (blk ? L.v_hi_n : 0);
+        float amax = 0.f;
+        for (int c = 0; c < n; ++c) amax = fmaxf(amax, fabsf(__half2float(z[c])));
+        const __half s16 = sk_scale_of(amax, sk_qmax(blk ? L.bits_lo : L.bits_hi));
+        reinterpret_cast<uint16_t*>(img + L.v_scale_off)[blk * P + slot] = sk_half_bits(s16);
+        s = __half2float(s16);
+      }
+      vs[blk * P + slot] = s;
+    }
+  }
+  __syncthreads();
+
+  // value fields, channel-major: consecutive threads take consecutive channels (coalesced reads)
+  for (int blk = 0; blk < 2; ++blk) {
+    const int n = blk ? L.v_lo_n : L.v_hi_n;
+    if (n == 0) continue;
+    const int bits = blk ? L.bits_lo : L.bits_hi;
+    const int c0 = blk ? L.v_hi_n : 0;
+    uint8_t* base = img + (blk ? L.v_lo_off : L.v_hi_off);
+    if (bits == 16) {
+      for (int i = threadIdx.x; i < n * P; i += blockDim.x) {
+        const int ch = i % n, slot = i / n, tok = t0 + slot;
+        if (tok < n_tokens) reinterpret_cast<__half*>(base)[ch * P + slot] = lv[(size_t)tok * L.rank_v + c0 + ch];
+      }
+    } else if (bits == 8) {
+      for (int i = threadIdx.x; i < n * P; i += blockDim.x) {
+        const int ch = i % n, slot = i / n, tok = t0 + slot;
+        if (tok < n_tokens)
+          base[ch * P + slot] =
+              (uint8_t)(sk_code_of(__half2float(lv[(size_t)tok * L.rank_v + c0 + ch]), vs[blk * P + slot], 127) + 128);
+      }
+    } else {
+      for (int i = threadIdx.x; i < n * (P / 2); i += blockDim.x) {
+        const int ch = i % n, k = i / n;
+        int byte = 0;
+        for (int e = 0; e < 2; ++e) {
+          const int slot = 2 * k + e, tok = t0 + slot;
+          if (tok < n_tokens) {
+            const int u = sk_code_of(__half2float(lv[(size_t)tok * L.rank_v + c0 + ch]), vs[blk * P + slot], 7) + 8;
+            byte |= u << (4 * e);
+          }
+        }
+        base[ch * (P / 2) + k] = (uint8_t)byte;
+      }
+    }
+  }
+  __syncthreads();
+  uint4* dst = reinterpret_cast<uint4*>(pages + (size_t)page * L.page_bytes);
+  for (int i = threadIdx.x; i < L.page_bytes / 16; i += blockDim.x) dst[i] = reinterpret_cast<uint4*>(img)[i];
+}
+
+// ---------------------------------------------------------------------------------------------
+// unpack
+// ---------------------------------------------------------------------------------------------
+__device__ __forceinline__ void sk_locate(const StarkvLayout& L, int col, int slot, int& bits, int& field_byte,
+                                          int& nib, int& scale_idx) {
+  // field_byte: byte offset inside the page of the byte holding the field (fp16: first byte);
+  // nib: 0/1 nibble selector for 4-bit; scale_idx: index into the page's fp16 scale arrays
+  // (K: (h*2+blk)*P+slot relative to k_scale_off; V: encoded as -(1 + blk*P + slot)).
+  const int P = L.page_tokens;
+  const bool quant = L.bits_hi != 16;
+  if (col < L.sum_rank_k) {
+    const int h = sk_head_of_col(L, col);
+    const int cc = col - L.koff[h];
+    const int blk = (quant && cc >= L.k_hi_n[h]) ? 1 : 0;
+    const int idx = blk ? cc - L.k_hi_n[h] : cc;
+    const int n = blk ? L.k_lo_n[h] : L.k_hi_n[h];
+    bits = blk ? L.bits_lo : L.bits_hi;
+    const int base = (blk ? L.k_lo_off[h] : L.k_hi_off[h]) + slot * (n * bits / 8);
+    field_byte = base + idx * bits / 8;
+    nib = (bits == 4) ? (idx & 1) : 0;
+    scale_idx = (h * 2 + blk) * P + slot;
+  } else {
+    const int cc = col - L.sum_rank_k;
+    const int blk = (quant && cc >= L.v_hi_n) ? 1 : 0;
+    const int idx = blk ? cc - L.v_hi_n : cc;
+    bits = blk ? L.bits_lo : L.bits_hi;
+    const int base = (blk ? L.v_lo_off : L.v_hi_off) + idx * (P * bits / 8);
+    field_byte = base + slot * bits / 8;
+    nib = (bits == 4) ? (slot & 1) : 0;
+    scale_idx = -(1 + blk * P + slot);
+  }
+}
+
+__global__ void unpack_kernel(const __grid_constant__ StarkvLayout L, const uint8_t* __restrict__ pages,
+                              int n_tokens, int8_t* __restrict__ codes, uint16_t* __restrict__ scales,
+                              float* __restrict__ deq) {
+  const int P = L.page_tokens;
+  const int R = L.sum_rank_k + L.rank_v;
+  const bool quant = L.bits_hi != 16;
+  const long long total = (long long)n_tokens * R;
+  for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < total;
+       i += (long long)gridDim.x * blockDim.x) {
+    const int tok = (int)(i / R), col = (int)(i % R);
+    const uint8_t* pg = pages + (size_t)(tok / P) * L.page_bytes;
+    int bits, fb, nib, si;
+    sk_locate(L, col, tok % P, bits, fb, nib, si);
+    if (!quant) {
+      if (deq) deq[i] = __half2float(*reinterpret_cast<const __half*>(pg + fb));
+      continue;
+    }
+    int u = pg[fb];
+    if (bits == 4) u = (u >> (4 * nib)) & 0xF;
+    const int c = u - (1 << (bits - 1));
+    if (codes) codes[i] = (int8_t)c;
+    if (deq) {
+      const uint16_t sb = si >= 0 ? reinterpret_cast<const uint16_t*>(pg + L.k_scale_off)[si]
+                                  : reinterpret_cast<const uint16_t*>(pg + L.v_scale_off)[-si - 1];
+      deq[i] = (float)c * __half2float(__ushort_as_half(sb));
+    }
+  }
+  if (quant && scales) {
+    const long long ts = (long long)n_tokens * L.n_scales;
+    for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < ts;
+         i += (long long)gridDim.x * blockDim.x) {
+      const int tok = (int)(i / L.n_scales), k = (int)(i % L.n_scales);
+      const uint8_t* pg = pages + (size_t)(tok / P) * L.page_bytes;
+      const int slot = tok % P;
+      scales[i] = k < 2 * L.n_kv_heads ? reinterpret_cast<const uint16_t*>(pg + L.k_scale_off)[k * P + slot]
+                                       : reinterpret_cast<const uint16_t*>(pg + L.v_scale_off)[(k - 2 * L.n_kv_heads) * P + slot];
+    }
+  }
+}
+
+// ---------------------------------------------------------------------------------------------
+// append, step A1: latent projection  z = fp16( X . A )  (fp32 accumulation)
+//   blockIdx.x < H_kv : key head h (input row at k_new + j*row_stride + h*head_stride, d_in_k wide)
+//   blockIdx.x >= H_kv: 128-column chunk of the joint value projection
+//   blockIdx.y        : tile of APP_TOK new tokens
+// ---------------------------------------------------------------------------------------------
+constexpr int APP_TOK = 16;
+constexpr int APP_KC = 64;
+
+__global__ void __launch_bounds__(128) append_project_kernel(
+    const __grid_constant__ StarkvLayout L, int n_new, const __half* __restrict__ k_new, long long k_row_stride,
+    long long k_head_stride, int d_in_k, const __half* __restrict__ v_new, long long v_row_stride, int d_in_v,
+    const __half* __restrict__ A_k, const __half* __restrict__ A_v, __half* __restrict__ z) {
+  __shared__ float xs[APP_TOK][APP_KC + 1];
+  const int R = L.sum_rank_k + L.rank_v;
+  const int j0 = blockIdx.y * APP_TOK;
+  const bool is_k = (int)blockIdx.x < L.n_kv_heads;
+  const int h = blockIdx.x;
+  const __half* x0;
+  long long xstride;
+  int d_in, ncols, col_out0, lda;
+  const __half* A;
+  if (is_k) {
+    x0 = k_new + (long long)h * k_head_stride; xstride = k_row_stride; d_in = d_in_k;
+    ncols = L.rank_k[h]; col_out0 = L.koff[h]; A = A_k + L.koff[h]; lda = L.sum_rank_k;
+  } else {
+    const int c0 = (blockIdx.x - L.n_kv_heads) * 128;
+    x0 = v_new; xstride = v_row_stride; d_in = d_in_v;
+    ncols = min(128, L.rank_v - c0); col_out0 = L.sum_rank_k + c0; A = A_v + c0; lda = L.rank_v;
+  }
+  for (int cbase = 0; cbase < ncols; cbase += 128) {
+    const int c = cbase + threadIdx.x;
+    float acc[APP_TOK];
+#pragma unroll
+    for (int t = 0; t < APP_TOK; ++t) acc[t] = 0.f;
+    for (int k0 = 0; k0 < d_in; k0 += APP_KC) {
+      __syncthreads();
+      for (int i = threadIdx.x; i < APP_TOK * APP_KC; i += blockDim.x) {
+        const int t = i / APP_KC, k = i % APP_KC;
+        const int j = j0 + t;
+        xs[t][k] = (j < n_new && k0 + k < d_in) ? __half2float(x0[(long long)j * xstride + k0 + k]) : 0.f;
+      }
+      __syncthreads();
+      if (c < ncols) {
+        const int kmax = min(APP_KC, d_in - k0);
+        for (int k = 0; k < kmax; ++k) {
+          const float a = __half2float(A[(size_t)(k0 + k) * lda + c]);
+#pragma unroll
+          for (int t = 0; t < APP_TOK; ++t) acc[t] = fmaf(xs[t][k], a, acc[t]);
+        }
+      }
+    }
+    if (c < ncols) {
+#pragma unroll
+      for (int t = 0; t < APP_TOK; ++t)
+        if (j0 + t < n_new) z[(size_t)(j0 + t) * R + col_out0 + c] = __float2half_rn(acc[t]);
+    }
+  }
+}
+
+// ---------------------------------------------------------------------------------------------
+// append, steps A2-A4: per-token scales, codes, pack, paged write.  One CTA per new token.
+// 4-bit value fields share a byte between two slots: set with atomicAnd/atomicOr on the
+// containing word so that concurrent appends to neighbouring slots cannot lose an update.
+// ---------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(128) append_write_kernel(const __grid_constant__ StarkvLayout L,
+                                                           const __half* __restrict__ z, int n_new,
+                                                           const int32_t* __restrict__ seq_ids,
+                                                           const int32_t* __restrict__ positions,
+                                                           const int32_t* __restrict__ table, int max_pages,
+                                                           uint8_t* __restrict__ pool) {
+  extern __shared__ __align__(16) uint8_t sm[];
+  __half* zr = reinterpret_cast<__half*>(sm);
+  __shared__ float vsc[2];
+  const int j = blockIdx.x;
+  const int P = L.page_tokens;
+  const int R = L.sum_rank_k + L.rank_v;
+  const bool quant = L.bits_hi != 16;
+  const int pos = positions[j];
+  const int pidx = table[(size_t)seq_ids[j] * max_pages + pos / P];
+  if (pidx < 0) return;
+  uint8_t* pg = pool + (size_t)pidx * L.page_bytes;
+  const int slot = pos % P;
+  for (int i = threadIdx.x; i < R; i += blockDim.x) zr[i] = z[(size_t)j * R + i];
+  __syncthreads();
+
+  for (int u = threadIdx.x; u < L.n_kv_heads * 2; u += blockDim.x) {
+    const int h = u >> 1, blk = u & 1;
+    const int n = blk ? L.k_lo_n[h] : L.k_hi_n[h];
+    if (!quant) {
+      if (blk) continue;
+      __half* row = reinterpret_cast<__half*>(pg + L.k_hi_off[h]) + (size_t)slot * n;
+      for (int c = 0; c < n; ++c) row[c] = zr[L.koff[h] + c];
+      continue;
+    }
+    uint16_t* sc = reinterpret_cast<uint16_t*>(pg + L.k_scale_off) + (h * 2 + blk) * P + slot;
+    if (n == 0) { *sc = 0; continue; }
+    const __half* zz = zr + L.koff[h] + (blk ? L.k_hi_n[h] : 0);
+    const int bits = blk ? L.bits_lo : L.bits_hi;
+    const int qmax = sk_qmax(bits);
+    float amax = 0.f;
+    for (int c = 0; c < n; ++c) amax = fmaxf(amax, fabsf(__half2float(zz[c])));
+    const __half s16 = sk_scale_of(amax, qmax);
+    const float s = __half2float(s16);
+    *sc = sk_half_bits(s16);
+    uint8_t* row = pg + (blk ? L.k_lo_off[h] : L.k_hi_off[h]) + (size_t)slot * (n * bits / 8);
+    if (bits == 8) {
+      for (int c = 0; c < n; ++c) row[c] = (uint8_t)(sk_code_of(__half2float(zz[c]), s, qmax) + 128);
+    } else {
+      for (int c = 0; c < n; c += 2) {
+        const int u0 = sk_code_of(__half2float(zz[c]), s, qmax) + 8;
+        const int u1 = sk_code_of(__half2float(zz[c + 1]), s, qmax) + 8;
+        row[c >> 1] = (uint8_t)(u0 | (u1 << 4));
+      }
+    }
+  }
+
+  const __half* zv = zr + L.sum_rank_k;
+  if (quant) {
+    // two warps: one per precision block, shuffle-reduce the absmax
+    const int w = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    if (w < 2) {
+      const int n = w ? L.v_lo_n : L.v_hi_n;
+      const int c0 = w ? L.v_hi_n : 0;
+      float amax = 0.f;
+      for (int c = lane; c < n; c += 32) amax = fmaxf(amax, fabsf(__half2float(zv[c0 + c])));
+#pragma unroll
+      for (int o = 16; o; o >>= 1) amax = fmaxf(amax, __shfl_xor_sync(0xffffffffu, amax, o));
+      if (lane == 0) {
+        const __half s16 = n ? sk_scale_of(amax, sk_qmax(w ? L.bits_lo : L.bits_hi)) : __float2half(0.f);
+        reinterpret_cast<uint16_t*>(pg + L.v_scale_off)[w * P + slot] = sk_half_bits(s16);
+        vsc[w] = __half2float(s16);
+      }
+    }
+    __syncthreads();
+  }
+  for (int c = threadIdx.x; c < L.rank_v; c += blockDim.x) {
+    const int blk = (quant && c >= L.v_hi_n) ? 1 : 0;
+    const int idx = blk ? c - L.v_hi_n : c;
+    const int bits = blk ? L.bits_lo : L.bits_hi;
+    uint8_t* base = pg + (blk ? L.v_lo_off : L.v_hi_off);
+    if (bits == 16) {
+      reinterpret_cast<__half*>(base)[(size_t)idx * P + slot] = zv[c];
+    } else if (bits == 8) {
+      base[(size_t)idx * P + slot] = (uint8_t)(sk_code_of(__half2float(zv[c]), vsc[blk], 127) + 128);
+    } else {
+      const unsigned u = (unsigned)(sk_code_of(__half2float(zv[c]), vsc[blk], 7) + 8);
+      const size_t byte = (size_t)idx * (P / 2) + (slot >> 1);
+      unsigned* word = reinterpret_cast<unsigned*>(base + (byte & ~(size_t)3));
+      const int sh = 8 * (int)(byte & 3) + 4 * (slot & 1);
+      atomicAnd(word, ~(0xFu << sh));
+      atomicOr(word, u << sh);
+    }
+  }
+}
+
+}  // namespace
+
+// ---------------------------------------------------------------------------------------------
+// host side
+// ---------------------------------------------------------------------------------------------
+int sk_pack(starkv_ctx* ctx, const void* lk, const void* lv, int n_tokens, void* pages) {
+  const StarkvLayout& L = ctx->L;
+  ctx->last_launches = 0;
+  if (n_tokens < 0) return STARKV_ERR_INVALID_ARG;
+  if (n_tokens == 0) return STARKV_OK;
+  if (!lk || !lv || !pages) return STARKV_ERR_INVALID_ARG;
+  const int n_pages = (n_tokens + L.page_tokens - 1) / L.page_tokens;
+  const size_t smem = (size_t)L.page_bytes + 2 * L.page_tokens * sizeof(float);
+  if ((int)smem > ctx->smem_optin) return STARKV_ERR_UNSUPPORTED;
+  SK_CUDA_CHECK(ctx, cudaFuncSetAttribute(pack_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+  pack_kernel<<<n_pages, 256, smem, ctx->stream>>>(L, (const __half*)lk, (const __half*)lv, n_tokens, (uint8_t*)pages);
+  ctx->last_launches = 1;
+  SK_CUDA_CHECK(ctx, cudaGetLastError());
+  return STARKV_OK;
+}
+
+int sk_unpack(starkv_ctx* ctx, const void* pages, int n_tokens, int8_t* codes, uint16_t* scales, float* deq) {
+  const StarkvLayout& L = ctx->L;
+  ctx->last_launches = 0;
+  if (n_tokens < 0) return STARKV_ERR_INVALID_ARG;
+  if (n_tokens == 0) return STARKV_OK;
+  if (!pages) return STARKV_ERR_INVALID_ARG;
+  const long long total = (long long)n_tokens * (L.sum_rank_k + L.rank_v);
+  const int blocks = (int)((total + 255) / 256 < 148 * 16 ? (total + 255) / 256 : 148 * 16);
+  unpack_kernel<<<blocks, 256, 0, ctx->stream>>>(L, (const uint8_t*)pages, n_tokens, codes, scales, deq);
+  ctx->last_launches = 1;
+  SK_CUDA_CHECK(ctx, cudaGetLastError());
+  return STARKV_OK;
+}
+
+size_t sk_append_ws_bytes(const starkv_ctx* ctx, int n_new) {
+  const size_t R = (size_t)ctx->L.sum_rank_k + ctx->L.rank_v;
+  return ((size_t)(n_new > 0 ? n_new : 0) * R * 2 + 255) / 256 * 256;
+}
+
+int sk_append(starkv_ctx* ctx, void* pool, const int32_t* table, int max_pages, const int32_t* seq_ids,
+              const int32_t* positions, int n_new, const void* k_new, int64_t k_row_stride, int64_t k_head_stride,
+              int d_in_k, const void* v_new, int64_t v_row_stride, int d_in_v, const void* A_k, const void* A_v,
+              void* ws, size_t ws_bytes) {
+  const StarkvLayout& L = ctx->L;
+  ctx->last_launches = 0;
+  if (n_new < 0 || max_pages <= 0 || d_in_k <= 0 || d_in_v <= 0) return STARKV_ERR_INVALID_ARG;
+  if (n_new == 0) return STARKV_OK;
+  if (!pool || !table || !seq_ids || !positions || !k_new || !v_new || !A_k || !A_v || !ws) return STARKV_ERR_INVALID_ARG;
+  if (ws_bytes < sk_append_ws_bytes(ctx, n_new)) return STARKV_ERR_WORKSPACE;
+  __half* z = (__half*)ws;
+  dim3 g1(L.n_kv_heads + (L.rank_v + 127) / 128, (n_new + APP_TOK - 1) / APP_TOK);
+  append_project_kernel<<<g1, 128, 0, ctx->stream>>>(L, n_new, (const __half*)k_new, k_row_stride, k_head_stride, d_in_k,
+                                                     (const __half*)v_new, v_row_stride, d_in_v, (const __half*)A_k,
+                                                     (const __half*)A_v, z);
+  SK_CUDA_CHECK(ctx, cudaGetLastError());
+  const size_t smem = ((size_t)(L.sum_rank_k + L.rank_v) * 2 + 15) / 16 * 16;
+  if ((int)smem > ctx->smem_optin) return STARKV_ERR_UNSUPPORTED;
+  if (smem > 48 * 1024)
+    SK_CUDA_CHECK(ctx, cudaFuncSetAttribute(append_write_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+  append_write_kernel<<<n_new, 128, smem, ctx->stream>>>(L, z, n_new, seq_ids, positions, table, max_pages, (uint8_t*)pool);
+  ctx->last_launches = 2;
+  SK_CUDA_CHECK(ctx, cudaGetLastError());
+  return STARKV_OK;
+}

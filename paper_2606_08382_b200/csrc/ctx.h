@@ -1,0 +1,57 @@
+// Internal context of libstarkv.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "../../include/starkv.h"
+#include "decode_fast.h"
+#include "starkv_layout.h"
+
+struct starkv_ctx {
+  StarkvLayout L;
+  cudaStream_t stream;
+  int device;
+  int n_sm;
+  int smem_optin;        // max dynamic shared memory per block (opt-in)
+  int n_splits_override; // 0 = automatic
+  int last_launches;
+  int fast_ok;           // tensor-core decode kernel covers this descriptor
+  FastPlan plan;
+  char err[512];
+};
+
+int sk_cuda_fail(starkv_ctx* ctx, cudaError_t e, const char* what);
+
+#define SK_CUDA_CHECK(ctx, expr)                    \
+  do {                                              \
+    cudaError_t _e = (expr);                        \
+    if (_e != cudaSuccess) return sk_cuda_fail((ctx), _e, #expr); \
+  } while (0)
+
+// codec.cu
+int sk_pack(starkv_ctx* ctx, const void* lk, const void* lv, int n_tokens, void* pages);
+int sk_unpack(starkv_ctx* ctx, const void* pages, int n_tokens, int8_t* codes, uint16_t* scales, float* deq);
+int sk_append(starkv_ctx* ctx, void* pool, const int32_t* table, int max_pages, const int32_t* seq_ids,
+              const int32_t* positions, int n_new, const void* k_new, int64_t k_row_stride,
+              int64_t k_head_stride, int d_in_k, const void* v_new, int64_t v_row_stride, int d_in_v,
+              const void* A_k, const void* A_v, void* ws, size_t ws_bytes);
+size_t sk_append_ws_bytes(const starkv_ctx* ctx, int n_new);
+
+// decode.cu / decode_generic.cu
+struct SkWorkspace {   // carve-up of the caller's decode workspace
+  size_t qimg_off;     // latent-space query images, per sequence
+  size_t qimg_stride;
+  size_t part_off;     // split-K partials
+  size_t host_off;     // staging for the _host variant (q, seq_lens, out)
+  size_t total;
+  int n_splits;
+};
+void sk_plan_workspace(const starkv_ctx* ctx, int batch, int max_pages, SkWorkspace* w);
+int sk_decode_generic(starkv_ctx* ctx, const void* q, const void* pool, const int32_t* table, int max_pages,
+                      const int32_t* seq_lens, int batch, const void* B_k, const void* B_v, void* ws,
+                      size_t ws_bytes, void* out);
+int sk_decode_fast(starkv_ctx* ctx, const void* q, const void* pool, const int32_t* table, int max_pages,
+                   const int32_t* seq_lens, int batch, const void* B_k, const void* B_v, void* ws,
+                   size_t ws_bytes, void* out);
+int sk_fast_supported(const starkv_ctx* ctx);
+int sk_fast_plan(starkv_ctx* ctx);   // fills ctx->plan, ctx->fast_ok

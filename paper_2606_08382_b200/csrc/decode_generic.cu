@@ -1,0 +1,196 @@
+// Plain scalar decode-attention kernel (any page_tokens / head count; fp32 math, exact dequantisation),
+// the split-K combine + B_v up-projection kernel (rows D8, D9), and the workspace carve-up.
+//   PAPER.md §3.1 L54 (softmax attention), §3.2 L58 (K = K' U_K^T, V = V' U_V^T),
+//   §3.3 L62-68 (reordering: score in latent space, (p V') U_V), Eq.12 L208 (dequantisation).
+#include "decode_common.cuh"
+
+namespace {
+
+constexpr float kLog2e = 1.4426950408889634f;
+
+__device__ __forceinline__ float block_reduce(float v, bool is_max, float* red) {
+  const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+#pragma unroll
+  for (int o = 16; o; o >>= 1) {
+    const float x = __shfl_xor_sync(0xffffffffu, v, o);
+    v = is_max ? fmaxf(v, x) : v + x;
+  }
+  __syncthreads();
+  if (lane == 0) red[w] = v;
+  __syncthreads();
+  float r = red[0];
+  for (int i = 1; i < (int)(blockDim.x >> 5); ++i) r = is_max ? fmaxf(r, red[i]) : r + red[i];
+  return r;
+}
+
+// field `idx` of a row of `bits`-wide fields starting at `row`
+__device__ __forceinline__ float field_value(const uint8_t* row, int idx, int bits) {
+  if (bits == 16) return __half2float(reinterpret_cast<const __half*>(row)[idx]);
+  if (bits == 8) return (float)((int)row[idx] - 128);
+  return (float)((int)((row[idx >> 1] >> (4 * (idx & 1))) & 0xF) - 8);
+}
+
+// grid (n_splits, H_q, batch), 128 threads
+__global__ void __launch_bounds__(128) decode_generic_kernel(
+    const __grid_constant__ StarkvLayout L, const __half* __restrict__ q, const uint8_t* __restrict__ pool,
+    const int32_t* __restrict__ table, int max_pages, const int32_t* __restrict__ seq_lens,
+    const __half* __restrict__ B_k, float* __restrict__ parts, int n_splits) {
+  __shared__ float qt[256];   // latent-space query of this head (r_g <= head_dim <= 256)
+  __shared__ float pbuf[128];
+  __shared__ float red[4];
+  const int split = blockIdx.x, head = blockIdx.y, b = blockIdx.z;
+  const int g = head / L.group;
+  const int P = L.page_tokens;
+  const bool quant = L.bits_hi != 16;
+  const int r = L.rank_k[g];
+  const int len = seq_lens[b];
+  const int n_pages = (len + P - 1) / P;
+  int p0, p1;
+  sk_split_range(n_pages, n_splits, 1, split, &p0, &p1);
+
+  // D1: q~ = sm_scale * log2e * q B_k^T
+  const __half* qrow = q + ((size_t)b * L.n_q_heads + head) * L.head_dim;
+  for (int c = threadIdx.x; c < r; c += blockDim.x) {
+    const __half* brow = B_k + (size_t)(L.koff[g] + c) * L.head_dim;
+    float a = 0.f;
+    for (int d = 0; d < L.head_dim; ++d) a = fmaf(__half2float(qrow[d]), __half2float(brow[d]), a);
+    qt[c] = a * L.sm_scale * kLog2e;
+  }
+  __syncthreads();
+
+  float m_run = -INFINITY, l_run = 0.f;
+  float acc[4] = {0.f, 0.f, 0.f, 0.f};   // channels threadIdx.x + 128*k  (rank_v <= 512)
+  const int n_hi = L.k_hi_n[g], n_lo = L.k_lo_n[g];
+  for (int pg = p0; pg < p1; ++pg) {
+    const uint8_t* page = pool + (size_t)table[(size_t)b * max_pages + pg] * L.page_bytes;
+    for (int s0 = 0; s0 < P; s0 += 128) {
+      const int slot = s0 + threadIdx.x;
+      const int tok = pg * P + slot;
+      const bool valid = slot < P && tok < len;
+      float s = -INFINITY;
+      if (valid) {
+        const uint8_t* row = page + L.k_hi_off[g] + (size_t)slot * (n_hi * L.bits_hi / 8);
+        float d = 0.f;
+        for (int c = 0; c < n_hi; ++c) d = fmaf(qt[c], field_value(row, c, L.bits_hi), d);
+        if (quant) {
+          const __half* ksc = reinterpret_cast<const __half*>(page + L.k_scale_off);
+          d *= __half2float(ksc[(g * 2 + 0) * P + slot]);
+          if (n_lo) {
+            const uint8_t* row2 = page + L.k_lo_off[g] + (size_t)slot * (n_lo * L.bits_lo / 8);
+            float d2 = 0.f;
+            for (int c = 0; c < n_lo; ++c) d2 = fmaf(qt[n_hi + c], field_value(row2, c, L.bits_lo), d2);
+            d = fmaf(d2, __half2float(ksc[(g * 2 + 1) * P + slot]), d);
+          }
+        }
+        s = d;
+      }
+      const float m_blk = block_reduce(s, true, red);
+      if (m_blk == -INFINITY) continue;   // uniform
+      const float m_new = fmaxf(m_run, m_blk);
+      const float alpha = exp2f(m_run - m_new);   // 0 on the first block
+      const float p = valid ? exp2f(s - m_new) : 0.f;
+      const float psum = block_reduce(p, false, red);
+      l_run = l_run * alpha + psum;
+      m_run = m_new;
+      __syncthreads();
+      pbuf[threadIdx.x] = p;
+      __syncthreads();
+      const int nt = min(128, P - s0);
+#pragma unroll
+      for (int k = 0; k < 4; ++k) {
+        const int c = threadIdx.x + 128 * k;
+        if (c >= L.rank_v) break;
+        const int blk = (quant && c >= L.v_hi_n) ? 1 : 0;
+        const int idx = blk ? c - L.v_hi_n : c;
+        const int bits = blk ? L.bits_lo : L.bits_hi;
+        const uint8_t* row = page + (blk ? L.v_lo_off : L.v_hi_off) + (size_t)idx * (P * bits / 8);
+        const __half* vsc = quant ? reinterpret_cast<const __half*>(page + L.v_scale_off) + blk * P : nullptr;
+        float a = 0.f;
+        for (int t = 0; t < nt; ++t) {
+          const float pv = pbuf[t];
+          if (pv == 0.f) continue;   // masked slots may hold arbitrary bits
+          float v = field_value(row, s0 + t, bits);
+          if (quant) v *= __half2float(vsc[s0 + t]);
+          a = fmaf(pv, v, a);
+        }
+        acc[k] = acc[k] * alpha + a;
+      }
+    }
+  }
+  float* out = parts + (((size_t)b * n_splits + split) * L.n_q_heads + head) * sk_part_stride(L.rank_v);
+  if (threadIdx.x == 0) { out[0] = m_run; out[1] = l_run; }
+#pragma unroll
+  for (int k = 0; k < 4; ++k) {
+    const int c = threadIdx.x + 128 * k;
+    if (c < L.rank_v) out[2 + c] = acc[k];
+  }
+}
+
+// grid (H_q, batch), 128 threads.  D8: LSE merge; D9: out_i = o_i . B_v[:, g d_h : (g+1) d_h]
+__global__ void __launch_bounds__(128) combine_kernel(const __grid_constant__ StarkvLayout L,
+                                                      const float* __restrict__ parts, int n_splits,
+                                                      const __half* __restrict__ B_v, __half* __restrict__ out) {
+  __shared__ float o_lat[512];
+  __shared__ float wsm[512];
+  const int head = blockIdx.x, b = blockIdx.y;
+  const int g = head / L.group;
+  const size_t ps = sk_part_stride(L.rank_v);
+  const float* base = parts + ((size_t)b * n_splits * L.n_q_heads + head) * ps;
+  const size_t sstride = (size_t)L.n_q_heads * ps;
+  float mstar = -INFINITY;
+  for (int s = 0; s < n_splits; ++s) mstar = fmaxf(mstar, base[s * sstride]);
+  float lstar = 0.f;
+  for (int s0 = 0; s0 < n_splits; s0 += 512) {   // weights staged in chunks of 512 splits
+    const int ns = min(512, n_splits - s0);
+    __syncthreads();
+    for (int s = threadIdx.x; s < ns; s += blockDim.x) {
+      const float m = base[(s0 + s) * sstride];
+      wsm[s] = (m == -INFINITY) ? 0.f : exp2f(m - mstar);
+    }
+    __syncthreads();
+    for (int s = 0; s < ns; ++s) lstar += wsm[s] * base[(s0 + s) * sstride + 1];
+    for (int c = threadIdx.x; c < L.rank_v; c += blockDim.x) {
+      float a = s0 ? o_lat[c] : 0.f;
+      for (int s = 0; s < ns; ++s)
+        if (wsm[s] != 0.f) a = fmaf(wsm[s], base[(s0 + s) * sstride + 2 + c], a);
+      o_lat[c] = a;
+    }
+  }
+  __syncthreads();
+  const float inv = (mstar == -INFINITY || lstar == 0.f) ? 0.f : 1.f / lstar;
+  const int dv = L.n_kv_heads * L.head_dim;
+  for (int d = threadIdx.x; d < L.head_dim; d += blockDim.x) {
+    const __half* col = B_v + g * L.head_dim + d;
+    float a = 0.f;
+    if (inv != 0.f)
+      for (int c = 0; c < L.rank_v; ++c) a = fmaf(o_lat[c], __half2float(col[(size_t)c * dv]), a);
+    out[((size_t)b * L.n_q_heads + head) * L.head_dim + d] = __float2half_rn(a * inv);
+  }
+}
+
+}  // namespace
+
+int sk_launch_combine(starkv_ctx* ctx, const float* parts, int n_splits, int batch, const void* B_v, void* out) {
+  combine_kernel<<<dim3(ctx->L.n_q_heads, batch), 128, 0, ctx->stream>>>(ctx->L, parts, n_splits, (const __half*)B_v,
+                                                                         (__half*)out);
+  SK_CUDA_CHECK(ctx, cudaGetLastError());
+  return STARKV_OK;
+}
+
+int sk_decode_generic(starkv_ctx* ctx, const void* q, const void* pool, const int32_t* table, int max_pages,
+                      const int32_t* seq_lens, int batch, const void* B_k, const void* B_v, void* ws,
+                      size_t ws_bytes, void* out) {
+  const StarkvLayout& L = ctx->L;
+  ctx->last_launches = 0;
+  if (L.rank_v > 512) return STARKV_ERR_UNSUPPORTED;
+  SkWorkspace w;
+  sk_plan_workspace(ctx, batch, max_pages, &w);
+  if (ws_bytes < w.total) return STARKV_ERR_WORKSPACE;
+  float* parts = reinterpret_cast<float*>((uint8_t*)ws + w.part_off);
+  decode_generic_kernel<<<dim3(w.n_splits, L.n_q_heads, batch), 128, 0, ctx->stream>>>(
+      L, (const __half*)q, (const uint8_t*)pool, table, max_pages, seq_lens, (const __half*)B_k, parts, w.n_splits);
+  SK_CUDA_CHECK(ctx, cudaGetLastError());
+  const int rc = sk_launch_combine(ctx, parts, w.n_splits, batch, B_v, out);
+  ctx->last_launches = 2;
+  return rc;
+}

@@ -1,0 +1,194 @@
+"""GPU parity, decode attention: starkv_decode_attn (tensor-core kernel) and starkv_decode_attn_generic
+(scalar kernel) through the C ABI against the CPU fp64 oracle on the same seeded inputs.
+
+Bar (BASELINE.json north_star): max relative error 2e-3, measured per (b, q-head) row as
+||out - ref||_inf / ||ref||_inf."""
+import numpy as np
+import pytest
+import torch
+
+import synth
+from oracle import attention as oattn
+from tests.gpu_util import run_decode
+from tests.util import build_cache, row_rel_err
+
+pytestmark = pytest.mark.gpu
+sk = pytest.importorskip("paper_2606_08382_b200")
+
+TOL = 2e-3
+
+
+def _check(cfg, seq_lens=None, regime="diffuse", generic=False, splits=0, heads=None, tol=TOL):
+    cache = build_cache(cfg, seq_lens=seq_lens, regime=regime)
+    bk, bv = synth.make_factors(cfg)
+    q = synth.make_q(cfg, batch=len(cache["seq_lens"]))
+    ref = oattn.decode_attn(cache["desc"], q, cache["pool"], cache["table"], cache["seq_lens"], bk, bv, heads=heads)
+    out = run_decode(cfg, cache, q, bk, bv, generic=generic, splits=splits)
+    assert np.isfinite(out).all()
+    if heads is not None:
+        out, ref = out[:, heads], ref[:, heads]
+    err = row_rel_err(out, ref)
+    assert err <= tol, f"{cfg.name} {regime} generic={generic} splits={splits}: row rel err {err:.3e}"
+    return err
+
+
+@pytest.mark.parametrize("generic", [True, False], ids=["generic", "fast"])
+def test_c1_full(generic):
+    cfg = synth.make_config("C1")
+    _check(cfg, generic=generic)
+    _check(cfg, generic=generic, regime="peaky")
+
+
+@pytest.mark.parametrize("generic", [True, False], ids=["generic", "fast"])
+@pytest.mark.parametrize("name,ctx,batch", [("C2", 2500, 2), ("C3", 5000, 2), ("C4", 1300, 2), ("C5", 3000, 3)])
+def test_reduced_configs_ragged(name, ctx, batch, generic):
+    cfg = synth.make_config(name, context=ctx, batch=batch)
+    lens = synth.make_seq_lens(cfg, ragged=True)
+    _check(cfg, seq_lens=lens, generic=generic)
+
+
+@pytest.mark.parametrize("name", ["C3", "C4"])
+def test_peaky_regime(name):
+    cfg = synth.make_config(name, context=3000, batch=1)
+    _check(cfg, regime="peaky")
+
+
+@pytest.mark.parametrize("bits", [(8, 8), (4, 4), (8, 4), (16, 16)], ids=str)
+@pytest.mark.parametrize("generic", [True, False], ids=["generic", "fast"])
+def test_bit_pairs_and_odd_shapes(bits, generic):
+    # MHA (G=1), G=2 and G=4; r_hi == r; value rank not a multiple of 16
+    for (hq, hkv, dh, rk, rv) in [(8, 8, 64, [8, 16, 24, 32, 40, 48, 56, 64], 72),
+                                  (8, 4, 128, [8, 96, 128, 32], 40),
+                                  (16, 4, 64, [16, 64, 8, 24], 136)]:
+        cfg = synth.custom_config(f"b{bits[0]}{bits[1]}", 2, hq, hkv, dh, 700, rk, rv, bits=bits, outlier_frac=0.1)
+        _check(cfg, seq_lens=[700, 333], generic=generic)
+
+
+@pytest.mark.parametrize("generic", [True, False], ids=["generic", "fast"])
+def test_sequence_length_edges(generic):
+    cfg = synth.make_config("C3", context=400, batch=8)
+    _check(cfg, seq_lens=[0, 1, 63, 64, 65, 127, 129, 400], generic=generic)
+    cfg = synth.make_config("C1", context=200, batch=4)
+    _check(cfg, seq_lens=[1, 0, 200, 64], generic=generic)
+
+
+def test_zero_length_gives_zero_rows():
+    cfg = synth.make_config("C3", context=128, batch=2)
+    cache = build_cache(cfg, seq_lens=[0, 100])
+    bk, bv = synth.make_factors(cfg)
+    q = synth.make_q(cfg, batch=2)
+    out = run_decode(cfg, cache, q, bk, bv)
+    assert np.all(out[0] == 0) and np.abs(out[1]).max() > 0
+
+
+def test_tail_slots_never_influence_the_output():
+    """Slots >= seq_len of the last page are unspecified (DESIGN.md format): poison them."""
+    cfg = synth.make_config("C3", context=100, batch=1)
+    cache = build_cache(cfg, seq_lens=[100])
+    bk, bv = synth.make_factors(cfg)
+    q = synth.make_q(cfg, batch=1)
+    clean = run_decode(cfg, cache, q, bk, bv)
+    lay = cache["layout"]
+    last = cache["table"][0, 1]
+    page = cache["pool"][last]
+    sc = page[lay.v_scale_off:lay.v_scale_off + 2 * 2 * 64].view(np.uint16).reshape(2, 64)
+    sc[:, 36:] = 0x7E00                                   # NaN scales in the dead slots (100 = 64 + 36)
+    ks = page[lay.k_scale_off:lay.k_scale_off + cfg.n_kv_heads * 2 * 64 * 2].view(np.uint16).reshape(-1, 64)
+    ks[:, 36:] = 0x7C00                                   # +inf key scales
+    poisoned = run_decode(cfg, cache, q, bk, bv)
+    assert np.array_equal(clean, poisoned)
+    cfg = synth.make_config("C2", context=100, batch=1)
+    cache = build_cache(cfg, seq_lens=[100])
+    bk, bv = synth.make_factors(cfg)
+    clean = run_decode(cfg, cache, q, bk, bv)
+    lay = cache["layout"]
+    page = cache["pool"][cache["table"][0, 1]]
+    v = page[lay.v_hi_off:lay.v_hi_off + cfg.rank_v * 64 * 2].view(np.uint16).reshape(cfg.rank_v, 64)
+    v[:, 36:] = 0x7E00
+    for h in range(cfg.n_kv_heads):
+        r = cfg.rank_k[h]
+        kk = page[lay.k_hi_off[h]:lay.k_hi_off[h] + 64 * r * 2].view(np.uint16).reshape(64, r)
+        kk[36:] = 0x7E00
+    poisoned = run_decode(cfg, cache, q, bk, bv)
+    assert np.array_equal(clean, poisoned)
+
+
+@pytest.mark.parametrize("splits", [1, 2, 7, 64])
+def test_split_count_does_not_change_the_result(splits):
+    cfg = synth.make_config("C3", context=2000, batch=2)
+    _check(cfg, seq_lens=[2000, 1111], splits=splits)
+
+
+def test_fast_matches_generic_on_a_larger_case():
+    """Second implementation as cross-check at a size the oracle is slow on (all heads)."""
+    cfg = synth.make_config("C5", context=20000, batch=2)
+    cache = build_cache(cfg)
+    bk, bv = synth.make_factors(cfg)
+    q = synth.make_q(cfg)
+    a = run_decode(cfg, cache, q, bk, bv, generic=True)
+    b = run_decode(cfg, cache, q, bk, bv, generic=False)
+    assert row_rel_err(b, a) <= TOL
+
+
+@pytest.mark.parametrize("D", [10, 12, 14, 16])
+def test_underflow_closed_form(D):
+    """Pin P16 on the GPU: one token at score +D (natural log units) over N equal tokens, constant value
+    codes: out = (v0 + N e^-D v) / (1 + N e^-D) -- exercises fp16 P underflow handling."""
+    cfg = synth.custom_config("uf", 1, 4, 1, 64, 32768, [16], 32, bits=(8, 4), rank_v_hi=16)
+    n = cfg.context
+    bk, bv = synth.make_factors(cfg)
+    q = synth.make_q(cfg, batch=1)
+    # latent-space query of head 0, then key latents along it: token 0 at +D, the others at 0
+    qt = (bk.astype(np.float64) @ q[0, 0].astype(np.float64)) * cfg.sm_scale
+    u = qt / np.dot(qt, qt)
+    lk = np.zeros((n, 16), np.float16)
+    lk[0] = (D * u).astype(np.float16)
+    lv = np.full((n, 32), np.float16(1e-3))
+    lv[0] = np.float16(0.5)
+    cache = build_cache(cfg, seq_lens=[n], latents=[(lk, lv)])
+    ref = oattn.decode_attn(cache["desc"], q, cache["pool"], cache["table"], cache["seq_lens"], bk, bv)
+    out = run_decode(cfg, cache, q, bk, bv)
+    assert row_rel_err(out[:, :1], ref[:, :1]) <= TOL
+
+
+def test_error_paths():
+    cfg = synth.make_config("C1")
+    cache = build_cache(cfg)
+    ctx = sk.create_from_config(cfg)
+    bk, bv = synth.make_factors(cfg)
+    from tests.gpu_util import dev, f16
+    pool, table, lens = dev(cache["pool"]), dev(cache["table"].astype(np.int32)), dev(cache["seq_lens"])
+    q, bkd, bvd = f16(synth.make_q(cfg)), f16(bk), f16(bv)
+    out = torch.empty((1, 4, 64), dtype=torch.float16, device="cuda")
+    need = sk.starkv_workspace_bytes(ctx, 1, table.shape[1])
+    ws = torch.empty(need, dtype=torch.uint8, device="cuda")
+    with pytest.raises(sk.StarkvError) as e:
+        sk.starkv_decode_attn(ctx, q, pool, table, table.shape[1], lens, 1, bkd, bvd, ws, need - 1, out)
+    assert e.value.code == sk.STARKV_ERR_WORKSPACE
+    with pytest.raises(sk.StarkvError) as e:
+        sk.starkv_decode_attn(ctx, q, pool, table, table.shape[1], lens, 1, bkd, bvd, None, need, out)
+    assert e.value.code == sk.STARKV_ERR_INVALID_ARG
+    with pytest.raises(sk.StarkvError) as e:
+        sk.starkv_decode_attn(ctx, q.data_ptr() + 2, pool, table, table.shape[1], lens, 1, bkd, bvd, ws, need, out)
+    assert e.value.code == sk.STARKV_ERR_INVALID_ARG
+    sk.starkv_decode_attn(ctx, q, pool, table, table.shape[1], lens, 1, bkd, bvd, ws, need, out)
+    torch.cuda.synchronize()
+    assert sk.starkv_last_launches(ctx) == 3
+
+
+def test_host_variant_matches_device_variant():
+    cfg = synth.make_config("C3", context=1000, batch=2)
+    cache = build_cache(cfg)
+    bk, bv = synth.make_factors(cfg)
+    q16 = synth.make_q(cfg)
+    want = run_decode(cfg, cache, q16, bk, bv)
+    from tests.gpu_util import dev, f16
+    ctx = sk.create_from_config(cfg)
+    pool, table = dev(cache["pool"]), dev(cache["table"].astype(np.int32))
+    wsb = sk.starkv_workspace_bytes(ctx, 2, table.shape[1])
+    ws = torch.empty(wsb, dtype=torch.uint8, device="cuda")
+    qh = torch.from_numpy(q16.view(np.uint16).astype(np.int16)).view(torch.float16).pin_memory()
+    lh = torch.from_numpy(np.asarray(cache["seq_lens"], np.int32)).pin_memory()
+    oh = torch.empty((2, cfg.n_q_heads, cfg.head_dim), dtype=torch.float16).pin_memory()
+    sk.starkv_decode_attn_host(ctx, qh, pool, table, table.shape[1], lh, 2, f16(bk), f16(bv), ws, wsb, oh)
+    assert np.array_equal(oh.double().numpy(), want)

@@ -146,6 +146,28 @@ int starkv_decode_attn_host(starkv_ctx* ctx, const void* q_host, const void* pag
                             const void* B_v, void* workspace, size_t workspace_bytes,
                             void* out_host);
 
+/* HOST-buffer variant of starkv_append (bench.py "e2e"): k_new_host [n_new, k_row_elems] and
+ * v_new_host [n_new, v_row_elems] fp16, seq_ids_host / positions_host int32 [n_new] are HOST
+ * pointers (pinned for best speed); strides are the row element counts (k_row_stride =
+ * k_row_elems, v_row_stride = v_row_elems).  In hidden mode pass v_new_host == k_new_host (copied
+ * once).  The call copies them into `workspace` (sized by starkv_append_host_workspace_bytes) and
+ * enqueues the append; it does NOT synchronise (copies and kernels are ordered on the stream;
+ * the host buffers must stay unchanged until the stream reaches the end of the call). */
+size_t starkv_append_host_workspace_bytes(const starkv_ctx* ctx, int n_new, int k_row_elems,
+                                          int v_row_elems);
+int starkv_append_host(starkv_ctx* ctx, void* page_pool, const int32_t* block_table, int max_pages,
+                       const int32_t* seq_ids_host, const int32_t* positions_host, int n_new,
+                       const void* k_new_host, int k_row_elems, int64_t k_head_stride, int d_in_k,
+                       const void* v_new_host, int v_row_elems, int d_in_v, const void* A_k,
+                       const void* A_v, void* workspace, size_t workspace_bytes);
+
+/* Kernel timing (bench.py "roofline"): when on, the decode calls record CUDA events on the
+ * context's stream directly before and after the main split-K kernel (rows D2-D7).
+ * starkv_last_decode_kernel_ms waits for the second event and returns the elapsed milliseconds of
+ * the last decode call's main kernel in *ms (STARKV_ERR_INVALID_ARG if timing was off). */
+int starkv_set_kernel_timing(starkv_ctx* ctx, int on);
+int starkv_last_decode_kernel_ms(starkv_ctx* ctx, float* ms);
+
 /* Tuning knob (0 = automatic): number of split-K ranges per sequence for the next decode calls. */
 int starkv_set_splits(starkv_ctx* ctx, int n_splits);
 

@@ -23,6 +23,8 @@ SYMBOLS = [
     "starkv_create", "starkv_destroy", "starkv_page_bytes", "starkv_workspace_bytes",
     "starkv_append_workspace_bytes", "starkv_pack", "starkv_unpack", "starkv_append",
     "starkv_decode_attn", "starkv_decode_attn_generic", "starkv_decode_attn_host",
+    "starkv_append_host_workspace_bytes", "starkv_append_host", "starkv_set_kernel_timing",
+    "starkv_last_decode_kernel_ms",
     "starkv_set_splits", "starkv_last_launches", "starkv_strerror", "starkv_last_error",
 ]
 
@@ -77,6 +79,15 @@ def _load() -> ctypes.CDLL:
     for name in ("starkv_decode_attn", "starkv_decode_attn_generic", "starkv_decode_attn_host"):
         getattr(lib, name).argtypes = dec
         getattr(lib, name).restype = c_int
+    lib.starkv_append_host_workspace_bytes.argtypes = [vp, c_int, c_int, c_int]
+    lib.starkv_append_host_workspace_bytes.restype = c_sz
+    lib.starkv_append_host.argtypes = [vp, vp, i32p, c_int, i32p, i32p, c_int, vp, c_int, c_i64, c_int, vp, c_int,
+                                       c_int, vp, vp, vp, c_sz]
+    lib.starkv_append_host.restype = c_int
+    lib.starkv_set_kernel_timing.argtypes = [vp, c_int]
+    lib.starkv_set_kernel_timing.restype = c_int
+    lib.starkv_last_decode_kernel_ms.argtypes = [vp, ctypes.POINTER(ctypes.c_float)]
+    lib.starkv_last_decode_kernel_ms.restype = c_int
     lib.starkv_set_splits.argtypes = [vp, c_int]
     lib.starkv_set_splits.restype = c_int
     lib.starkv_last_launches.argtypes = [vp]
@@ -198,6 +209,29 @@ def starkv_decode_attn_host(ctx, q_host, page_pool, block_table, max_pages, seq_
                             workspace, workspace_bytes, out_host) -> None:
     _decode(_lib.starkv_decode_attn_host, ctx, q_host, page_pool, block_table, max_pages, seq_lens_host, batch,
             B_k, B_v, workspace, workspace_bytes, out_host)
+
+
+def starkv_append_host_workspace_bytes(ctx: Context, n_new: int, k_row_elems: int, v_row_elems: int) -> int:
+    return int(_lib.starkv_append_host_workspace_bytes(ctx.handle, n_new, k_row_elems, v_row_elems))
+
+
+def starkv_append_host(ctx: Context, page_pool, block_table, max_pages: int, seq_ids_host, positions_host,
+                       n_new: int, k_new_host, k_row_elems: int, k_head_stride: int, d_in_k: int, v_new_host,
+                       v_row_elems: int, d_in_v: int, A_k, A_v, workspace, workspace_bytes: int) -> None:
+    ctx._check(_lib.starkv_append_host(ctx.handle, _ptr(page_pool), _ptr(block_table), max_pages,
+                                       _ptr(seq_ids_host), _ptr(positions_host), n_new, _ptr(k_new_host),
+                                       k_row_elems, k_head_stride, d_in_k, _ptr(v_new_host), v_row_elems, d_in_v,
+                                       _ptr(A_k), _ptr(A_v), _ptr(workspace), workspace_bytes))
+
+
+def starkv_set_kernel_timing(ctx: Context, on: bool) -> None:
+    ctx._check(_lib.starkv_set_kernel_timing(ctx.handle, 1 if on else 0))
+
+
+def starkv_last_decode_kernel_ms(ctx: Context) -> float:
+    ms = ctypes.c_float(0.0)
+    ctx._check(_lib.starkv_last_decode_kernel_ms(ctx.handle, ctypes.byref(ms)))
+    return float(ms.value)
 
 
 def starkv_set_splits(ctx: Context, n_splits: int) -> None:

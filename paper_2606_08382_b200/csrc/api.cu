@@ -45,7 +45,12 @@ int starkv_create(starkv_ctx** out, const starkv_desc* d, void* cuda_stream) {
   return STARKV_OK;
 }
 
-void starkv_destroy(starkv_ctx* ctx) { free(ctx); }
+void starkv_destroy(starkv_ctx* ctx) {
+  if (!ctx) return;
+  if (ctx->ev0) cudaEventDestroy(ctx->ev0);
+  if (ctx->ev1) cudaEventDestroy(ctx->ev1);
+  free(ctx);
+}
 
 size_t starkv_page_bytes(const starkv_ctx* ctx) { return ctx ? (size_t)ctx->L.page_bytes : 0; }
 
@@ -124,6 +129,58 @@ int starkv_decode_attn_host(starkv_ctx* ctx, const void* q_host, const void* poo
   if (rc) return rc;
   SK_CUDA_CHECK(ctx, cudaMemcpyAsync(out_host, dout, qbytes, cudaMemcpyDeviceToHost, ctx->stream));
   SK_CUDA_CHECK(ctx, cudaStreamSynchronize(ctx->stream));
+  return STARKV_OK;
+}
+
+size_t starkv_append_host_workspace_bytes(const starkv_ctx* ctx, int n_new, int k_row_elems, int v_row_elems) {
+  if (!ctx || n_new <= 0 || k_row_elems < 0 || v_row_elems < 0) return 0;
+  const size_t up = 255;
+  return sk_append_ws_bytes(ctx, n_new) + (((size_t)n_new * k_row_elems * 2 + up) & ~up) +
+         (((size_t)n_new * v_row_elems * 2 + up) & ~up) + 2 * (((size_t)n_new * 4 + up) & ~up);
+}
+
+int starkv_append_host(starkv_ctx* ctx, void* pool, const int32_t* table, int max_pages, const int32_t* seq_ids_host,
+                       const int32_t* positions_host, int n_new, const void* k_new_host, int k_row_elems,
+                       int64_t k_head_stride, int d_in_k, const void* v_new_host, int v_row_elems, int d_in_v,
+                       const void* A_k, const void* A_v, void* ws, size_t ws_bytes) {
+  if (!ctx || n_new < 0) return STARKV_ERR_INVALID_ARG;
+  if (n_new == 0) return STARKV_OK;
+  if (!seq_ids_host || !positions_host || !k_new_host || !v_new_host || !ws || !aligned16(ws)) return STARKV_ERR_INVALID_ARG;
+  if (ws_bytes < starkv_append_host_workspace_bytes(ctx, n_new, k_row_elems, v_row_elems)) return STARKV_ERR_WORKSPACE;
+  const size_t up = 255;
+  const size_t zb = sk_append_ws_bytes(ctx, n_new);
+  const size_t kb = (size_t)n_new * k_row_elems * 2, vb = (size_t)n_new * v_row_elems * 2, ib = (size_t)n_new * 4;
+  uint8_t* dk = (uint8_t*)ws + zb;
+  uint8_t* dv = dk + ((kb + up) & ~up);
+  int32_t* dseq = (int32_t*)(dv + ((vb + up) & ~up));
+  int32_t* dpos = (int32_t*)((uint8_t*)dseq + ((ib + up) & ~up));
+  SK_CUDA_CHECK(ctx, cudaMemcpyAsync(dk, k_new_host, kb, cudaMemcpyHostToDevice, ctx->stream));
+  const void* vdev = dk;
+  if (v_new_host != k_new_host) {
+    SK_CUDA_CHECK(ctx, cudaMemcpyAsync(dv, v_new_host, vb, cudaMemcpyHostToDevice, ctx->stream));
+    vdev = dv;
+  }
+  SK_CUDA_CHECK(ctx, cudaMemcpyAsync(dseq, seq_ids_host, ib, cudaMemcpyHostToDevice, ctx->stream));
+  SK_CUDA_CHECK(ctx, cudaMemcpyAsync(dpos, positions_host, ib, cudaMemcpyHostToDevice, ctx->stream));
+  return starkv_append(ctx, pool, table, max_pages, dseq, dpos, n_new, dk, k_row_elems, k_head_stride, d_in_k, vdev,
+                       v_row_elems, d_in_v, A_k, A_v, ws, zb);
+}
+
+int starkv_set_kernel_timing(starkv_ctx* ctx, int on) {
+  if (!ctx) return STARKV_ERR_INVALID_ARG;
+  if (on && !ctx->ev0) {
+    SK_CUDA_CHECK(ctx, cudaEventCreate(&ctx->ev0));
+    SK_CUDA_CHECK(ctx, cudaEventCreate(&ctx->ev1));
+  }
+  ctx->timing_on = on ? 1 : 0;
+  ctx->timing_valid = 0;
+  return STARKV_OK;
+}
+
+int starkv_last_decode_kernel_ms(starkv_ctx* ctx, float* ms) {
+  if (!ctx || !ms || !ctx->timing_valid) return STARKV_ERR_INVALID_ARG;
+  SK_CUDA_CHECK(ctx, cudaEventSynchronize(ctx->ev1));
+  SK_CUDA_CHECK(ctx, cudaEventElapsedTime(ms, ctx->ev0, ctx->ev1));
   return STARKV_OK;
 }
 

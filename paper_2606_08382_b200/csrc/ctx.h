@@ -17,6 +17,9 @@ struct starkv_ctx {
   int last_launches;
   int fast_ok;           // tensor-core decode kernel covers this descriptor
   FastPlan plan;
+  int timing_on;         // record events around the main decode kernel
+  int timing_valid;
+  cudaEvent_t ev0, ev1;
   char err[512];
 };
 

@@ -732,12 +732,17 @@ int sk_decode_fast(starkv_ctx* ctx, const void* q, const void* pool, const int32
   do { if (mt == 2) SK_PICK_ITP(Q, NTv, 2); else SK_PICK_ITP(Q, NTv, 4); } while (0)
 #define SK_PICK_NT(Q) \
   do { if (P.nt == 1) SK_PICK_MT(Q, 1); else SK_PICK_MT(Q, 4); } while (0)
+  if (ctx->timing_on) SK_CUDA_CHECK(ctx, cudaEventRecord(ctx->ev0, ctx->stream));
   if (quant) SK_PICK_NT(true); else SK_PICK_NT(false);
 #undef SK_PICK_NT
 #undef SK_PICK_MT
 #undef SK_PICK_ITP
 #undef SK_LAUNCH
   SK_CUDA_CHECK(ctx, e);
+  if (ctx->timing_on) {
+    SK_CUDA_CHECK(ctx, cudaEventRecord(ctx->ev1, ctx->stream));
+    ctx->timing_valid = 1;
+  }
   const int rc = sk_launch_combine(ctx, parts, w.n_splits, batch, B_v, out);
   ctx->last_launches = 3;
   return rc;

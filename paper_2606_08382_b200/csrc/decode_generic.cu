@@ -187,9 +187,14 @@ int sk_decode_generic(starkv_ctx* ctx, const void* q, const void* pool, const in
   sk_plan_workspace(ctx, batch, max_pages, &w);
   if (ws_bytes < w.total) return STARKV_ERR_WORKSPACE;
   float* parts = reinterpret_cast<float*>((uint8_t*)ws + w.part_off);
+  if (ctx->timing_on) SK_CUDA_CHECK(ctx, cudaEventRecord(ctx->ev0, ctx->stream));
   decode_generic_kernel<<<dim3(w.n_splits, L.n_q_heads, batch), 128, 0, ctx->stream>>>(
       L, (const __half*)q, (const uint8_t*)pool, table, max_pages, seq_lens, (const __half*)B_k, parts, w.n_splits);
   SK_CUDA_CHECK(ctx, cudaGetLastError());
+  if (ctx->timing_on) {
+    SK_CUDA_CHECK(ctx, cudaEventRecord(ctx->ev1, ctx->stream));
+    ctx->timing_valid = 1;
+  }
   const int rc = sk_launch_combine(ctx, parts, w.n_splits, batch, B_v, out);
   ctx->last_launches = 2;
   return rc;

@@ -35,6 +35,7 @@ int starkv_create(starkv_ctx** out, const starkv_desc* d, void* cuda_stream) {
   cudaError_t e = cudaGetDevice(&ctx->device);
   if (e == cudaSuccess) e = cudaDeviceGetAttribute(&ctx->n_sm, cudaDevAttrMultiProcessorCount, ctx->device);
   if (e == cudaSuccess) e = cudaDeviceGetAttribute(&ctx->smem_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, ctx->device);
+  if (e == cudaSuccess) e = cudaDeviceGetAttribute(&ctx->smem_per_sm, cudaDevAttrMaxSharedMemoryPerMultiprocessor, ctx->device);
   if (e != cudaSuccess) {   // no usable device: fail loudly, there is no CPU path
     (void)cudaGetLastError();
     free(ctx);

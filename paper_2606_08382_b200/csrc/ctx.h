@@ -4,7 +4,7 @@
 #include <stdint.h>
 
 #include "../../include/starkv.h"
-#include "decode_fast.h"
+#include "decode_v2.h"
 #include "starkv_layout.h"
 
 struct starkv_ctx {
@@ -13,10 +13,11 @@ struct starkv_ctx {
   int device;
   int n_sm;
   int smem_optin;        // max dynamic shared memory per block (opt-in)
+  int smem_per_sm;       // shared memory per SM
   int n_splits_override; // 0 = automatic
   int last_launches;
   int fast_ok;           // tensor-core decode kernel covers this descriptor
-  FastPlan plan;
+  V2Plan plan;
   int timing_on;         // record events around the main decode kernel
   int timing_valid;
   cudaEvent_t ev0, ev1;

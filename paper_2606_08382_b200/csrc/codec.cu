@@ -248,12 +248,89 @@ __global__ void __launch_bounds__(128) append_project_kernel(
 }
 
 // ---------------------------------------------------------------------------------------------
+// append, step A1 for a handful of new tokens (decode-time append, n_new <= 16): z = X . A is bound by reading
+// A once, so the K dimension is split over APS_KS blocks and 8 warps per block, 64 columns per block (one
+// half2 per lane and row); partial sums are reduced in a fixed order (deterministic) and written as fp32
+//   zp[ks][token][column];  the write kernel adds the APS_KS partials, rounds once to fp16 and quantises.
+// grid (column tiles of keys then values, APS_KS), 256 threads.
+// ---------------------------------------------------------------------------------------------
+constexpr int APS_COLS = 64, APS_KCH = 256, APS_TOK = 16, APS_KS = 4;
+
+__global__ void __launch_bounds__(256) append_project_small_kernel(
+    const __grid_constant__ StarkvLayout L, int n_new, int n_key_tiles, const __half* __restrict__ k_new,
+    long long k_row_stride, long long k_head_stride, int d_in_k, const __half* __restrict__ v_new, long long v_row_stride,
+    int d_in_v, const __half* __restrict__ A_k, const __half* __restrict__ A_v, float* __restrict__ zp) {
+  __shared__ __align__(16) float sm[8 * APS_TOK * APS_COLS];   // x chunk [16][256] during the loop, then the warp partials
+  const int R = L.sum_rank_k + L.rank_v;
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const __half* x0;
+  long long xstride;
+  int d_in, ncols, col_out0, lda;
+  const __half* A;
+  if ((int)blockIdx.x < n_key_tiles) {
+    int h = 0, t = blockIdx.x;
+    while (t >= (L.rank_k[h] + APS_COLS - 1) / APS_COLS) { t -= (L.rank_k[h] + APS_COLS - 1) / APS_COLS; ++h; }
+    const int c0 = t * APS_COLS;
+    x0 = k_new + (long long)h * k_head_stride; xstride = k_row_stride; d_in = d_in_k;
+    ncols = min(APS_COLS, L.rank_k[h] - c0); col_out0 = L.koff[h] + c0; A = A_k + L.koff[h] + c0; lda = L.sum_rank_k;
+  } else {
+    const int c0 = (blockIdx.x - n_key_tiles) * APS_COLS;
+    x0 = v_new; xstride = v_row_stride; d_in = d_in_v;
+    ncols = min(APS_COLS, L.rank_v - c0); col_out0 = L.sum_rank_k + c0; A = A_v + c0; lda = L.rank_v;
+  }
+  const int per = ((d_in + APS_KS - 1) / APS_KS + 31) / 32 * 32;
+  const int k_begin = blockIdx.y * per, k_end = min(d_in, k_begin + per);
+  float acc[APS_TOK][2];
+#pragma unroll
+  for (int t = 0; t < APS_TOK; ++t) acc[t][0] = acc[t][1] = 0.f;
+  const bool col_ok = 2 * lane < ncols;
+  for (int kc = k_begin; kc < k_end; kc += APS_KCH) {
+    __syncthreads();
+    for (int i = tid; i < APS_TOK * APS_KCH; i += 256) {
+      const int t = i / APS_KCH, k = i % APS_KCH;
+      sm[i] = (t < n_new && kc + k < k_end) ? __half2float(x0[(long long)t * xstride + kc + k]) : 0.f;
+    }
+    __syncthreads();
+    const int kw = kc + warp * 32;
+    if (col_ok && kw < k_end) {
+      const int kn = min(32, k_end - kw);
+      const __half* ap = A + (size_t)kw * lda + 2 * lane;
+      const float* xp = sm + warp * 32;
+#pragma unroll 4
+      for (int kk = 0; kk < kn; ++kk) {
+        const float2 a = __half22float2(*reinterpret_cast<const __half2*>(ap + (size_t)kk * lda));
+#pragma unroll
+        for (int t = 0; t < APS_TOK; ++t) {
+          const float x = xp[t * APS_KCH + kk];
+          acc[t][0] = fmaf(x, a.x, acc[t][0]);
+          acc[t][1] = fmaf(x, a.y, acc[t][1]);
+        }
+      }
+    }
+  }
+  __syncthreads();
+#pragma unroll
+  for (int t = 0; t < APS_TOK; ++t)
+    *reinterpret_cast<float2*>(sm + (warp * APS_TOK + t) * APS_COLS + 2 * lane) = make_float2(acc[t][0], acc[t][1]);
+  __syncthreads();
+  for (int i = tid; i < APS_TOK * APS_COLS; i += 256) {
+    const int t = i / APS_COLS, c = i % APS_COLS;
+    float s = 0.f;
+#pragma unroll
+    for (int w = 0; w < 8; ++w) s += sm[(w * APS_TOK + t) * APS_COLS + c];
+    if (t < n_new && c < ncols) zp[((size_t)blockIdx.y * n_new + t) * R + col_out0 + c] = s;
+  }
+}
+
+// ---------------------------------------------------------------------------------------------
 // append, steps A2-A4: per-token scales, codes, pack, paged write.  One CTA per new token.
 // 4-bit value fields share a byte between two slots: set with atomicAnd/atomicOr on the
 // containing word so that concurrent appends to neighbouring slots cannot lose an update.
 // ---------------------------------------------------------------------------------------------
+// z16 (fp16 latents) or, when zp != nullptr, n_part fp32 partial sums zp[part][token][column] added in order.
 __global__ void __launch_bounds__(128) append_write_kernel(const __grid_constant__ StarkvLayout L,
-                                                           const __half* __restrict__ z, int n_new,
+                                                           const __half* __restrict__ z, const float* __restrict__ zp,
+                                                           int n_part, int n_new,
                                                            const int32_t* __restrict__ seq_ids,
                                                            const int32_t* __restrict__ positions,
                                                            const int32_t* __restrict__ table, int max_pages,
@@ -270,7 +347,15 @@ __global__ void __launch_bounds__(128) append_write_kernel(const __grid_constant
   if (pidx < 0) return;
   uint8_t* pg = pool + (size_t)pidx * L.page_bytes;
   const int slot = pos % P;
-  for (int i = threadIdx.x; i < R; i += blockDim.x) zr[i] = z[(size_t)j * R + i];
+  if (zp) {
+    for (int i = threadIdx.x; i < R; i += blockDim.x) {
+      float a = 0.f;
+      for (int p = 0; p < n_part; ++p) a += zp[((size_t)p * n_new + j) * R + i];
+      zr[i] = __float2half_rn(a);
+    }
+  } else {
+    for (int i = threadIdx.x; i < R; i += blockDim.x) zr[i] = z[(size_t)j * R + i];
+  }
   __syncthreads();
 
   for (int u = threadIdx.x; u < L.n_kv_heads * 2; u += blockDim.x) {
@@ -380,7 +465,9 @@ int sk_unpack(starkv_ctx* ctx, const void* pages, int n_tokens, int8_t* codes, u
 
 size_t sk_append_ws_bytes(const starkv_ctx* ctx, int n_new) {
   const size_t R = (size_t)ctx->L.sum_rank_k + ctx->L.rank_v;
-  return ((size_t)(n_new > 0 ? n_new : 0) * R * 2 + 255) / 256 * 256;
+  const size_t n = (size_t)(n_new > 0 ? n_new : 0);
+  const size_t b = n <= (size_t)APS_TOK ? n * R * 4 * APS_KS : n * R * 2;
+  return (b + 255) / 256 * 256;
 }
 
 int sk_append(starkv_ctx* ctx, void* pool, const int32_t* table, int max_pages, const int32_t* seq_ids,
@@ -394,16 +481,27 @@ int sk_append(starkv_ctx* ctx, void* pool, const int32_t* table, int max_pages, 
   if (!pool || !table || !seq_ids || !positions || !k_new || !v_new || !A_k || !A_v || !ws) return STARKV_ERR_INVALID_ARG;
   if (ws_bytes < sk_append_ws_bytes(ctx, n_new)) return STARKV_ERR_WORKSPACE;
   __half* z = (__half*)ws;
+  const float* zp = nullptr;
+  if (n_new <= APS_TOK) {
+    int nkt = 0;
+    for (int h = 0; h < L.n_kv_heads; ++h) nkt += (L.rank_k[h] + APS_COLS - 1) / APS_COLS;
+    const int nvt = (L.rank_v + APS_COLS - 1) / APS_COLS;
+    append_project_small_kernel<<<dim3(nkt + nvt, APS_KS), 256, 0, ctx->stream>>>(
+        L, n_new, nkt, (const __half*)k_new, k_row_stride, k_head_stride, d_in_k, (const __half*)v_new, v_row_stride, d_in_v,
+        (const __half*)A_k, (const __half*)A_v, (float*)ws);
+    zp = (const float*)ws;
+  } else {
   dim3 g1(L.n_kv_heads + (L.rank_v + 127) / 128, (n_new + APP_TOK - 1) / APP_TOK);
   append_project_kernel<<<g1, 128, 0, ctx->stream>>>(L, n_new, (const __half*)k_new, k_row_stride, k_head_stride, d_in_k,
                                                      (const __half*)v_new, v_row_stride, d_in_v, (const __half*)A_k,
                                                      (const __half*)A_v, z);
+  }
   SK_CUDA_CHECK(ctx, cudaGetLastError());
   const size_t smem = ((size_t)(L.sum_rank_k + L.rank_v) * 2 + 15) / 16 * 16;
   if ((int)smem > ctx->smem_optin) return STARKV_ERR_UNSUPPORTED;
   if (smem > 48 * 1024)
     SK_CUDA_CHECK(ctx, cudaFuncSetAttribute(append_write_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-  append_write_kernel<<<n_new, 128, smem, ctx->stream>>>(L, z, n_new, seq_ids, positions, table, max_pages, (uint8_t*)pool);
+  append_write_kernel<<<n_new, 128, smem, ctx->stream>>>(L, z, zp, APS_KS, n_new, seq_ids, positions, table, max_pages, (uint8_t*)pool);
   ctx->last_launches = 2;
   SK_CUDA_CHECK(ctx, cudaGetLastError());
   return STARKV_OK;

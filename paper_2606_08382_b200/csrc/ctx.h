@@ -4,7 +4,7 @@
 #include <stdint.h>
 
 #include "../../include/starkv.h"
-#include "decode_v2.h"
+#include "decode_plan.h"
 #include "starkv_layout.h"
 
 struct starkv_ctx {
@@ -17,7 +17,7 @@ struct starkv_ctx {
   int n_splits_override; // 0 = automatic
   int last_launches;
   int fast_ok;           // tensor-core decode kernel covers this descriptor
-  V2Plan plan;
+  DecodePlan plan;
   int timing_on;         // record events around the main decode kernel
   int timing_valid;
   cudaEvent_t ev0, ev1;

@@ -126,52 +126,100 @@ __global__ void __launch_bounds__(128) decode_generic_kernel(
   }
 }
 
-// grid (H_q, batch), 128 threads.  D8: LSE merge; D9: out_i = o_i . B_v[:, g d_h : (g+1) d_h]
-__global__ void __launch_bounds__(128) combine_kernel(const __grid_constant__ StarkvLayout L,
+// grid (H_q, batch), 256 threads.  D8: LSE merge; D9: out_i = o_i . B_v[:, g d_h : (g+1) d_h]
+//   1. split weights w_s = 2^(m_s - m*) and l* by block reductions
+//   2. o[c] = sum_s w_s acc_s[c], one channel per thread (coalesced over c), loads independent over s
+//   3. up-projection with the channel range cut into slices: each thread takes 8 output columns (one 16-byte
+//      load of a B_v row) of one slice, slices reduced through shared memory
+__global__ void __launch_bounds__(256) combine_kernel(const __grid_constant__ StarkvLayout L,
                                                       const float* __restrict__ parts, int n_splits,
                                                       const __half* __restrict__ B_v, __half* __restrict__ out) {
   __shared__ float o_lat[512];
   __shared__ float wsm[512];
-  const int head = blockIdx.x, b = blockIdx.y;
+  __shared__ __align__(16) float red[32 * 64];   // [slice][d] partial outputs (slices * d_h <= 2048)
+  __shared__ float rsm[8];
+  const int head = blockIdx.x, b = blockIdx.y, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const int g = head / L.group;
   const size_t ps = sk_part_stride(L.rank_v);
   const float* base = parts + ((size_t)b * n_splits * L.n_q_heads + head) * ps;
   const size_t sstride = (size_t)L.n_q_heads * ps;
-  float mstar = -INFINITY;
-  for (int s = 0; s < n_splits; ++s) mstar = fmaxf(mstar, base[s * sstride]);
+  // m* = max_s m_s
+  float mx = -INFINITY;
+  for (int s = tid; s < n_splits; s += 256) mx = fmaxf(mx, base[s * sstride]);
+#pragma unroll
+  for (int o = 16; o; o >>= 1) mx = fmaxf(mx, __shfl_xor_sync(0xffffffffu, mx, o));
+  if (lane == 0) rsm[warp] = mx;
+  __syncthreads();
+  float mstar = rsm[0];
+#pragma unroll
+  for (int i = 1; i < 8; ++i) mstar = fmaxf(mstar, rsm[i]);
   float lstar = 0.f;
   for (int s0 = 0; s0 < n_splits; s0 += 512) {   // weights staged in chunks of 512 splits
     const int ns = min(512, n_splits - s0);
     __syncthreads();
-    for (int s = threadIdx.x; s < ns; s += blockDim.x) {
+    float lp = 0.f;
+    for (int s = tid; s < ns; s += 256) {
       const float m = base[(s0 + s) * sstride];
-      wsm[s] = (m == -INFINITY) ? 0.f : exp2f(m - mstar);
+      const float w = (m == -INFINITY) ? 0.f : exp2f(m - mstar);
+      wsm[s] = w;
+      lp = fmaf(w, base[(s0 + s) * sstride + 1], lp);
     }
+#pragma unroll
+    for (int o = 16; o; o >>= 1) lp += __shfl_xor_sync(0xffffffffu, lp, o);
+    if (lane == 0) rsm[warp] = lp;
     __syncthreads();
-    for (int s = 0; s < ns; ++s) lstar += wsm[s] * base[(s0 + s) * sstride + 1];
-    for (int c = threadIdx.x; c < L.rank_v; c += blockDim.x) {
-      float a = s0 ? o_lat[c] : 0.f;
-      for (int s = 0; s < ns; ++s)
-        if (wsm[s] != 0.f) a = fmaf(wsm[s], base[(s0 + s) * sstride + 2 + c], a);
-      o_lat[c] = a;
+#pragma unroll
+    for (int i = 0; i < 8; ++i) lstar += rsm[i];
+    for (int c = tid; c < L.rank_v; c += 256) {
+      const float* col = base + (size_t)s0 * sstride + 2 + c;
+      float a0 = 0.f, a1 = 0.f, a2 = 0.f, a3 = 0.f;
+      int s = 0;
+      for (; s + 4 <= ns; s += 4) {
+        const float v0 = col[(s + 0) * sstride], v1 = col[(s + 1) * sstride], v2 = col[(s + 2) * sstride],
+                    v3 = col[(s + 3) * sstride];
+        a0 = fmaf(wsm[s + 0], v0, a0); a1 = fmaf(wsm[s + 1], v1, a1);
+        a2 = fmaf(wsm[s + 2], v2, a2); a3 = fmaf(wsm[s + 3], v3, a3);
+      }
+      for (; s < ns; ++s) a0 = fmaf(wsm[s], col[s * sstride], a0);
+      o_lat[c] = (s0 ? o_lat[c] : 0.f) + ((a0 + a1) + (a2 + a3));
     }
   }
   __syncthreads();
   const float inv = (mstar == -INFINITY || lstar == 0.f) ? 0.f : 1.f / lstar;
-  const int dv = L.n_kv_heads * L.head_dim;
-  for (int d = threadIdx.x; d < L.head_dim; d += blockDim.x) {
-    const __half* col = B_v + g * L.head_dim + d;
-    float a = 0.f;
-    if (inv != 0.f)
-      for (int c = 0; c < L.rank_v; ++c) a = fmaf(o_lat[c], __half2float(col[(size_t)c * dv]), a);
-    out[((size_t)b * L.n_q_heads + head) * L.head_dim + d] = __float2half_rn(a * inv);
+  const int dh = L.head_dim, dv = L.n_kv_heads * dh;
+  const int nd8 = dh >> 3;            // 16-byte column groups (<= 32)
+  const int nsl = 256 / nd8;          // channel slices (>= 8)
+  const int d8 = tid % nd8, sl = tid / nd8;
+  float a[8] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
+  if (sl < nsl && inv != 0.f) {
+    const __half* bcol = B_v + (size_t)g * dh + 8 * d8;
+#pragma unroll 4
+    for (int c = sl; c < L.rank_v; c += nsl) {
+      const uint4 x = *reinterpret_cast<const uint4*>(bcol + (size_t)c * dv);
+      const float w = o_lat[c];
+      const float2 x0 = __half22float2(*reinterpret_cast<const __half2*>(&x.x)), x1 = __half22float2(*reinterpret_cast<const __half2*>(&x.y)),
+                   x2 = __half22float2(*reinterpret_cast<const __half2*>(&x.z)), x3 = __half22float2(*reinterpret_cast<const __half2*>(&x.w));
+      a[0] = fmaf(w, x0.x, a[0]); a[1] = fmaf(w, x0.y, a[1]); a[2] = fmaf(w, x1.x, a[2]); a[3] = fmaf(w, x1.y, a[3]);
+      a[4] = fmaf(w, x2.x, a[4]); a[5] = fmaf(w, x2.y, a[5]); a[6] = fmaf(w, x3.x, a[6]); a[7] = fmaf(w, x3.y, a[7]);
+    }
+  }
+  if (sl < nsl) {
+    float* r = red + sl * dh + 8 * d8;   // nsl * dh = 256 * 8 = 2048 floats
+    *reinterpret_cast<float4*>(r) = make_float4(a[0], a[1], a[2], a[3]);
+    *reinterpret_cast<float4*>(r + 4) = make_float4(a[4], a[5], a[6], a[7]);
+  }
+  __syncthreads();
+  for (int d = tid; d < dh; d += 256) {
+    float s = 0.f;
+    for (int k = 0; k < nsl; ++k) s += red[k * dh + d];
+    out[((size_t)b * L.n_q_heads + head) * dh + d] = __float2half_rn(s * inv);
   }
 }
 
 }  // namespace
 
 int sk_launch_combine(starkv_ctx* ctx, const float* parts, int n_splits, int batch, const void* B_v, void* out) {
-  combine_kernel<<<dim3(ctx->L.n_q_heads, batch), 128, 0, ctx->stream>>>(ctx->L, parts, n_splits, (const __half*)B_v,
+  combine_kernel<<<dim3(ctx->L.n_q_heads, batch), 256, 0, ctx->stream>>>(ctx->L, parts, n_splits, (const __half*)B_v,
                                                                          (__half*)out);
   SK_CUDA_CHECK(ctx, cudaGetLastError());
   return STARKV_OK;

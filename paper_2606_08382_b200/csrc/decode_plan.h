@@ -1,5 +1,4 @@
-// Host-built plan of the register-resident tensor-core decode kernel (decode_v2.cu); passed to the
-// kernels by value.
+// Host-built plan of the tensor-core decode kernel (decode_fast.cu); passed to the kernel by value.
 #pragma once
 #include <stdint.h>
 
@@ -10,8 +9,8 @@
 // One "q step" = one m16n8k16 MMA of the QK product of one KV head: 16 latent channels of one
 // precision block (a 32-channel int4 chunk makes two steps).  The latent-space query image holds, per
 // step, the B fragment (q~^T, zero outside the KV head's own columns) for all 32 lanes (uint2 per lane).
-struct V2Plan {
-  int32_t nq;                                     // quads = ceil(H_q / 4) <= 8; warp w scores quad w
+struct DecodePlan {
+  int32_t nq;                                     // quads = ceil(H_q / 4) <= 8; warp w of a group scores quad w
   int32_t kv_per_quad;                            // 4 / G
   int32_t qstep_begin[STARKV_MAX_KV_HEADS + 1];   // first q step of KV head g
   int32_t n_qsteps;
@@ -20,14 +19,23 @@ struct V2Plan {
   int32_t mt;                                     // PV m-tiles (16 value channels) per warp: 1..4
   int32_t v_tiles_hi, v_tiles;                    // m-tiles in the leading value block / in total
   int32_t nstage;                                 // page ring depth
-  int32_t ctas_per_sm;                            // 1 or 2 (shared memory and registers permitting)
-  int32_t off_stage, off_qimg, off_p, off_alpha, off_bar, smem_bytes;
+  // shared-memory carve-up (bytes from the 128-aligned base)
+  int32_t off_stage;                              // [nstage][page_bytes]; reused for the final group merge
+  int32_t off_qimg;                               // latent-space query image
+  int32_t off_p;                                  // [2 groups][2][P_BUF_BYTES]; P exchange buffers
+  int32_t off_alpha;                              // [2 groups][2][32] float
+  int32_t off_flag;                               // [2 groups][2][8] bytes: "some head of quad w rescaled"
+  int32_t off_bar;                                // full[nstage] + image mbarriers, done[nstage] tickets, issued[nstage]
+  int32_t off_tbl;                                // block-table entries of the CTA's page range
+  int32_t off_kcst;                               // = off_qimg + qimg_bytes: QK accumulator start values
+                                                  // [H_kv][2 blocks][4 quad columns] fp32 (same bulk copy as the image)
+  int32_t smem_bytes;
 };
 
 // channel (inside its precision block) that k index `k` (0..15) of q step `m` of a chunk refers to
 //   8/16-bit blocks: chunk = 16 channels, lane j loads channels 4j..4j+3:  k = 8*hi8 + 2j + e -> 4j + 2*hi8 + e
 //   4-bit blocks   : chunk = 32 channels, lane j loads channels 8j..8j+7:  -> 8j + 2m + hi8 + 4e
-static inline __host__ __device__ int v2_k_to_channel(int bits, int m, int k) {
+static inline __host__ __device__ int sk_k_to_channel(int bits, int m, int k) {
   const int hi8 = k >> 3, j = (k & 7) >> 1, e = k & 1;
   return bits == 4 ? 8 * j + 2 * m + hi8 + 4 * e : 4 * j + 2 * hi8 + e;
 }

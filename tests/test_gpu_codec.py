@@ -116,18 +116,21 @@ def _append_case(cfg, mode, n_new, dyadic):
     return d, lay, dpool.cpu().numpy(), ref, n
 
 
+@pytest.mark.parametrize("n_new", [37, 8, 1], ids=["n37-gemm", "n8-small", "n1-small"])
 @pytest.mark.parametrize("name,mode", [("C1", "dense"), ("C3", "dense"), ("C3", "hidden"), ("C4", "dense")])
-def test_append_bit_exact_on_dyadic_inputs(name, mode):
+def test_append_bit_exact_on_dyadic_inputs(name, mode, n_new):
+    """n_new 37 -> 62 tokens (tiled projection kernel); 8 -> 15 and 1 -> 2 tokens (split-K small-n kernel)."""
     cfg = synth.make_config(name, context=256, batch=3)
-    d, lay, got, ref, n = _append_case(cfg, mode, 37, dyadic=True)
+    d, lay, got, ref, n = _append_case(cfg, mode, n_new, dyadic=True)
     assert np.array_equal(got, ref), f"{int((got != ref).sum())} bytes differ of {got.size}"
 
 
-def test_append_gaussian_inputs_close():
+@pytest.mark.parametrize("n_new", [40, 8])
+def test_append_gaussian_inputs_close(n_new):
     """Gaussian activations: fp32 summation order differs from the oracle's exact sum, so the fp16
     latent may differ in the last bit on a few entries; scales within 1 ulp, codes within 1 step."""
     cfg = synth.make_config("C3", context=256, batch=3)
-    d, lay, got, ref, n = _append_case(cfg, "dense", 40, dyadic=False)
+    d, lay, got, ref, n = _append_case(cfg, "dense", n_new, dyadic=False)
     frac = float((got != ref).mean())
     assert frac < 2e-3, frac
     # compare decoded values of the touched pages

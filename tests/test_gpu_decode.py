@@ -119,6 +119,13 @@ def test_split_count_does_not_change_the_result(splits):
     _check(cfg, seq_lens=[2000, 1111], splits=splits)
 
 
+@pytest.mark.parametrize("name,ctx,splits", [("C2", 4000, 1), ("C2", 4000, 3), ("C4", 1300, 1), ("C1", 3000, 2)])
+def test_long_page_ranges_per_cta(name, ctx, splits):
+    """Many pages per CTA: exercises the shared-memory ring (odd and even depths) and both warp groups."""
+    cfg = synth.make_config(name, context=ctx, batch=1)
+    _check(cfg, seq_lens=[ctx - 17], splits=splits)
+
+
 def test_fast_matches_generic_on_a_larger_case():
     """Second implementation as cross-check at a size the oracle is slow on (all heads)."""
     cfg = synth.make_config("C5", context=20000, batch=2)

@@ -421,13 +421,13 @@ def run_ours(args, cfg):
 
     # ---- roofline: the split-K decode kernel alone (events recorded by the library around it) ----
     Kr = min(K, 200)
-    flush = torch.empty(2 * L2_BYTES, dtype=torch.uint8, device=device)
     sk.starkv_set_kernel_timing(wl.ctx, True)
     kms = []
     sampler.timed = True
     with torch.cuda.stream(wl.stream):
         for i in range(Kr + 3):
-            flush.zero_()          # L2 flush; also lets the host run ahead so the events sit back to back
+            torch.cuda._sleep(300000)   # ~150 us spin kernel: the host runs ahead, so the library's events sit
+                                        # directly around the kernel; L2 is defeated by the replica rotation
             wl.step(i % R)
             ms = sk.starkv_last_decode_kernel_ms(wl.ctx)
             if i >= 3:

@@ -285,20 +285,26 @@ __global__ void __launch_bounds__(256) append_project_small_kernel(
   for (int t = 0; t < APS_TOK; ++t) acc[t][0] = acc[t][1] = 0.f;
   const bool col_ok = 2 * lane < ncols;
   for (int kc = k_begin; kc < k_end; kc += APS_KCH) {
+    // this warp's 32 rows of A first (independent loads, all in flight), then the x chunk
+    const int kw = kc + warp * 32;
+    const int kn = col_ok ? max(0, min(32, k_end - kw)) : 0;
+    uint32_t av[32];
+    {
+      const __half* ap = A + (size_t)kw * lda + 2 * lane;
+#pragma unroll
+      for (int kk = 0; kk < 32; ++kk) av[kk] = kk < kn ? *reinterpret_cast<const uint32_t*>(ap + (size_t)kk * lda) : 0u;
+    }
     __syncthreads();
     for (int i = tid; i < APS_TOK * APS_KCH; i += 256) {
       const int t = i / APS_KCH, k = i % APS_KCH;
       sm[i] = (t < n_new && kc + k < k_end) ? __half2float(x0[(long long)t * xstride + kc + k]) : 0.f;
     }
     __syncthreads();
-    const int kw = kc + warp * 32;
-    if (col_ok && kw < k_end) {
-      const int kn = min(32, k_end - kw);
-      const __half* ap = A + (size_t)kw * lda + 2 * lane;
+    if (kn > 0) {
       const float* xp = sm + warp * 32;
-#pragma unroll 4
-      for (int kk = 0; kk < kn; ++kk) {
-        const float2 a = __half22float2(*reinterpret_cast<const __half2*>(ap + (size_t)kk * lda));
+#pragma unroll
+      for (int kk = 0; kk < 32; ++kk) {
+        const float2 a = __half22float2(*reinterpret_cast<const __half2*>(&av[kk]));
 #pragma unroll
         for (int t = 0; t < APS_TOK; ++t) {
           const float x = xp[t * APS_KCH + kk];
@@ -328,7 +334,7 @@ __global__ void __launch_bounds__(256) append_project_small_kernel(
 // containing word so that concurrent appends to neighbouring slots cannot lose an update.
 // ---------------------------------------------------------------------------------------------
 // z16 (fp16 latents) or, when zp != nullptr, n_part fp32 partial sums zp[part][token][column] added in order.
-__global__ void __launch_bounds__(128) append_write_kernel(const __grid_constant__ StarkvLayout L,
+__global__ void __launch_bounds__(256) append_write_kernel(const __grid_constant__ StarkvLayout L,
                                                            const __half* __restrict__ z, const float* __restrict__ zp,
                                                            int n_part, int n_new,
                                                            const int32_t* __restrict__ seq_ids,
@@ -358,33 +364,42 @@ __global__ void __launch_bounds__(128) append_write_kernel(const __grid_constant
   }
   __syncthreads();
 
-  for (int u = threadIdx.x; u < L.n_kv_heads * 2; u += blockDim.x) {
-    const int h = u >> 1, blk = u & 1;
-    const int n = blk ? L.k_lo_n[h] : L.k_hi_n[h];
-    if (!quant) {
-      if (blk) continue;
-      __half* row = reinterpret_cast<__half*>(pg + L.k_hi_off[h]) + (size_t)slot * n;
-      for (int c = 0; c < n; ++c) row[c] = zr[L.koff[h] + c];
-      continue;
-    }
-    uint16_t* sc = reinterpret_cast<uint16_t*>(pg + L.k_scale_off) + (h * 2 + blk) * P + slot;
-    if (n == 0) { *sc = 0; continue; }
-    const __half* zz = zr + L.koff[h] + (blk ? L.k_hi_n[h] : 0);
-    const int bits = blk ? L.bits_lo : L.bits_hi;
-    const int qmax = sk_qmax(bits);
-    float amax = 0.f;
-    for (int c = 0; c < n; ++c) amax = fmaxf(amax, fabsf(__half2float(zz[c])));
-    const __half s16 = sk_scale_of(amax, qmax);
-    const float s = __half2float(s16);
-    *sc = sk_half_bits(s16);
-    uint8_t* row = pg + (blk ? L.k_lo_off[h] : L.k_hi_off[h]) + (size_t)slot * (n * bits / 8);
-    if (bits == 8) {
-      for (int c = 0; c < n; ++c) row[c] = (uint8_t)(sk_code_of(__half2float(zz[c]), s, qmax) + 128);
-    } else {
-      for (int c = 0; c < n; c += 2) {
-        const int u0 = sk_code_of(__half2float(zz[c]), s, qmax) + 8;
-        const int u1 = sk_code_of(__half2float(zz[c + 1]), s, qmax) + 8;
-        row[c >> 1] = (uint8_t)(u0 | (u1 << 4));
+  // keys: one warp per (head, precision block), lanes over channels
+  {
+    const int lane = threadIdx.x & 31, nw = blockDim.x >> 5;
+    for (int u = threadIdx.x >> 5; u < L.n_kv_heads * 2; u += nw) {
+      const int h = u >> 1, blk = u & 1;
+      const int n = blk ? L.k_lo_n[h] : L.k_hi_n[h];
+      if (!quant) {
+        if (blk) continue;
+        __half* row = reinterpret_cast<__half*>(pg + L.k_hi_off[h]) + (size_t)slot * n;
+        for (int c = lane; c < n; c += 32) row[c] = zr[L.koff[h] + c];
+        continue;
+      }
+      uint16_t* sc = reinterpret_cast<uint16_t*>(pg + L.k_scale_off) + (h * 2 + blk) * P + slot;
+      if (n == 0) {
+        if (lane == 0) *sc = 0;
+        continue;
+      }
+      const __half* zz = zr + L.koff[h] + (blk ? L.k_hi_n[h] : 0);
+      const int bits = blk ? L.bits_lo : L.bits_hi;
+      const int qmax = sk_qmax(bits);
+      float amax = 0.f;
+      for (int c = lane; c < n; c += 32) amax = fmaxf(amax, fabsf(__half2float(zz[c])));
+#pragma unroll
+      for (int o = 16; o; o >>= 1) amax = fmaxf(amax, __shfl_xor_sync(0xffffffffu, amax, o));
+      const __half s16 = sk_scale_of(amax, qmax);
+      const float sf = __half2float(s16);
+      if (lane == 0) *sc = sk_half_bits(s16);
+      uint8_t* row = pg + (blk ? L.k_lo_off[h] : L.k_hi_off[h]) + (size_t)slot * (n * bits / 8);
+      if (bits == 8) {
+        for (int c = lane; c < n; c += 32) row[c] = (uint8_t)(sk_code_of(__half2float(zz[c]), sf, qmax) + 128);
+      } else {
+        for (int c = lane; c < n / 2; c += 32) {
+          const int u0 = sk_code_of(__half2float(zz[2 * c]), sf, qmax) + 8;
+          const int u1 = sk_code_of(__half2float(zz[2 * c + 1]), sf, qmax) + 8;
+          row[c] = (uint8_t)(u0 | (u1 << 4));
+        }
       }
     }
   }
@@ -486,6 +501,7 @@ int sk_append(starkv_ctx* ctx, void* pool, const int32_t* table, int max_pages, 
     int nkt = 0;
     for (int h = 0; h < L.n_kv_heads; ++h) nkt += (L.rank_k[h] + APS_COLS - 1) / APS_COLS;
     const int nvt = (L.rank_v + APS_COLS - 1) / APS_COLS;
+    SK_PREFER_SMEM(ctx, append_project_small_kernel);
     append_project_small_kernel<<<dim3(nkt + nvt, APS_KS), 256, 0, ctx->stream>>>(
         L, n_new, nkt, (const __half*)k_new, k_row_stride, k_head_stride, d_in_k, (const __half*)v_new, v_row_stride, d_in_v,
         (const __half*)A_k, (const __half*)A_v, (float*)ws);
@@ -501,7 +517,8 @@ int sk_append(starkv_ctx* ctx, void* pool, const int32_t* table, int max_pages, 
   if ((int)smem > ctx->smem_optin) return STARKV_ERR_UNSUPPORTED;
   if (smem > 48 * 1024)
     SK_CUDA_CHECK(ctx, cudaFuncSetAttribute(append_write_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-  append_write_kernel<<<n_new, 128, smem, ctx->stream>>>(L, z, zp, APS_KS, n_new, seq_ids, positions, table, max_pages, (uint8_t*)pool);
+  SK_PREFER_SMEM(ctx, append_write_kernel);
+  append_write_kernel<<<n_new, 256, smem, ctx->stream>>>(L, z, zp, APS_KS, n_new, seq_ids, positions, table, max_pages, (uint8_t*)pool);
   ctx->last_launches = 2;
   SK_CUDA_CHECK(ctx, cudaGetLastError());
   return STARKV_OK;

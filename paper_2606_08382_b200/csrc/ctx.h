@@ -32,6 +32,19 @@ int sk_cuda_fail(starkv_ctx* ctx, cudaError_t e, const char* what);
     if (_e != cudaSuccess) return sk_cuda_fail((ctx), _e, #expr); \
   } while (0)
 
+// The decode kernel runs with the maximum shared-memory carve-out.  Every other kernel of the step asks for the
+// same carve-out, so that no L1/shared reconfiguration (an SM drain of several microseconds) sits between
+// consecutive launches of a step.
+#define SK_PREFER_SMEM(ctx, kernel)                                                                       \
+  do {                                                                                                    \
+    static bool _done = false;                                                                            \
+    if (!_done) {                                                                                         \
+      SK_CUDA_CHECK((ctx), cudaFuncSetAttribute((kernel), cudaFuncAttributePreferredSharedMemoryCarveout, \
+                                                (int)cudaSharedmemCarveoutMaxShared));                    \
+      _done = true;                                                                                       \
+    }                                                                                                     \
+  } while (0)
+
 // codec.cu
 int sk_pack(starkv_ctx* ctx, const void* lk, const void* lv, int n_tokens, void* pages);
 int sk_unpack(starkv_ctx* ctx, const void* pages, int n_tokens, int8_t* codes, uint16_t* scales, float* deq);

@@ -3,11 +3,12 @@
 #include "common.cuh"
 #include "ctx.h"
 
-// Split-K partial of one (sequence, split, query head):  [m, l, acc[r_v]] fp32, where
+// Split-K partial of one (sequence, split, query head):  [m, l, 0, 0, acc[r_v]] fp32 (16-byte aligned rows), where
 //   m   = running maximum of the base-2 scores (s * log2 e), -inf for an empty range
 //   l   = sum_t 2^(s_t - m)          acc[c] = sum_t 2^(s_t - m) L_v[t, c]
 // (both may carry a common power-of-two factor: only acc / l is used).
-__host__ __device__ inline size_t sk_part_stride(int rank_v) { return (size_t)rank_v + 2; }
+constexpr int SK_PART_ACC = 4;   // offset of acc[] inside a partial row
+__host__ __device__ inline size_t sk_part_stride(int rank_v) { return (size_t)rank_v + SK_PART_ACC; }
 
 // page range [p0, p1) of split `s` of a sequence with n_pages pages, in units of `gran` pages
 __host__ __device__ inline void sk_split_range(int n_pages, int n_splits, int gran, int s, int* p0, int* p1) {

@@ -103,6 +103,14 @@ __device__ __forceinline__ void mma16816(float (&d)[4], uint32_t a0, uint32_t a1
       : "+f"(d[0]), "+f"(d[1]), "+f"(d[2]), "+f"(d[3])
       : "r"(a0), "r"(a1), "r"(a2), "r"(a3), "r"(b0), "r"(b1));
 }
+// same, D = A.B + (c0, c1, c0, c1): starts an accumulator from a per-column constant without register moves
+__device__ __forceinline__ void mma16816_init(float (&d)[4], uint32_t a0, uint32_t a1, uint32_t a2, uint32_t a3, uint32_t b0,
+                                              uint32_t b1, float c0, float c1) {
+  asm volatile(
+      "mma.sync.aligned.m16n8k16.row.col.f32.f16.f16.f32 {%0,%1,%2,%3}, {%4,%5,%6,%7}, {%8,%9}, {%10,%11,%10,%11};"
+      : "=f"(d[0]), "=f"(d[1]), "=f"(d[2]), "=f"(d[3])
+      : "r"(a0), "r"(a1), "r"(a2), "r"(a3), "r"(b0), "r"(b1), "f"(c0), "f"(c1));
+}
 // 8x8 b16 transpose across the warp: lane (R, j) holds M[R][2j..2j+1] and receives M[2j..2j+1][R]
 __device__ __forceinline__ uint32_t movmatrix_trans(uint32_t x) {
   uint32_t r;
@@ -185,10 +193,11 @@ __global__ void __launch_bounds__(256) qproj_kernel(const __grid_constant__ Star
     qv[i][4] = d.x; qv[i][5] = d.y; qv[i][6] = e.x; qv[i][7] = e.y;
   }
   const float qscale = L.sm_scale * kLog2e;
-  for (int ch0 = 0; ch0 < r; ch0 += 16) {   // two channels per warp in flight
-    float a[2][4];
+  constexpr int QU = 4;                        // channels per warp in flight
+  for (int ch0 = 0; ch0 < r; ch0 += 8 * QU) {
+    float a[QU][4];
 #pragma unroll
-    for (int u = 0; u < 2; ++u) {
+    for (int u = 0; u < QU; ++u) {
       const int ch = ch0 + warp + 8 * u;
       uint4 x = make_uint4(0, 0, 0, 0);
       if (ch < r && act) x = *reinterpret_cast<const uint4*>(B_k + (size_t)(L.koff[g] + ch) * dh + lane * 8);
@@ -204,12 +213,12 @@ __global__ void __launch_bounds__(256) qproj_kernel(const __grid_constant__ Star
 #pragma unroll
     for (int o = 16; o; o >>= 1)
 #pragma unroll
-      for (int u = 0; u < 2; ++u)
+      for (int u = 0; u < QU; ++u)
 #pragma unroll
         for (int i = 0; i < 4; ++i) a[u][i] += __shfl_xor_sync(0xffffffffu, a[u][i], o);
     if (lane == 0) {
 #pragma unroll
-      for (int u = 0; u < 2; ++u) {
+      for (int u = 0; u < QU; ++u) {
         const int ch = ch0 + warp + 8 * u;
         if (ch < r) *reinterpret_cast<float4*>(qt[ch]) = make_float4(a[u][0] * qscale, a[u][1] * qscale, a[u][2] * qscale, a[u][3] * qscale);
       }
@@ -289,10 +298,22 @@ __global__ void __launch_bounds__(256) qproj_kernel(const __grid_constant__ Star
 template <bool QUANT>
 __device__ __forceinline__ int tok_base(int R) { return QUANT ? 16 * (R >> 1) + 4 * (R & 1) : 16 * (R >> 1) + (R & 1); }
 
+// Each function OVERWRITES acc: the first chunk's MMAs start from the per-column constant (cinit, 0).
 __device__ __forceinline__ void qk_f16(float (&acc)[4][4], const uint8_t* __restrict__ p0, int rowbytes, int nch,
-                                       const uint2* __restrict__ qi) {
+                                       const uint2* __restrict__ qi, float cinit) {
   const int rb2 = 2 * rowbytes, rb8 = 8 * rowbytes;
-  for (int c = 0; c < nch; ++c, p0 += 32, qi += 32) {
+  {
+    const uint2 bf = *qi;
+#pragma unroll
+    for (int s = 0; s < 4; ++s) {
+      const uint8_t* p = p0 + s * rb2;
+      const uint2 x0 = *reinterpret_cast<const uint2*>(p);
+      const uint2 x1 = *reinterpret_cast<const uint2*>(p + rb8);
+      mma16816_init(acc[s], x0.x, x1.x, x0.y, x1.y, bf.x, bf.y, cinit, 0.f);
+    }
+  }
+  for (int c = 1; c < nch; ++c) {
+    p0 += 32; qi += 32;
     const uint2 bf = *qi;
 #pragma unroll
     for (int s = 0; s < 4; ++s) {
@@ -305,9 +326,21 @@ __device__ __forceinline__ void qk_f16(float (&acc)[4][4], const uint8_t* __rest
 }
 
 __device__ __forceinline__ void qk_i8(float (&acc)[4][4], const uint8_t* __restrict__ p0, int rowbytes, int nch,
-                                      const uint2* __restrict__ qi) {
+                                      const uint2* __restrict__ qi, float cinit) {
   const int rb8 = 8 * rowbytes;
-  for (int c = 0; c < nch; ++c, p0 += 16, qi += 32) {
+  {
+    const uint2 bf = *qi;
+#pragma unroll
+    for (int s = 0; s < 4; ++s) {
+      const uint8_t* p = p0 + s * rowbytes;
+      const uint32_t w0 = *reinterpret_cast<const uint32_t*>(p);
+      const uint32_t w1 = *reinterpret_cast<const uint32_t*>(p + rb8);
+      mma16816_init(acc[s], prmt(w0, 0u, 0x4140u), prmt(w1, 0u, 0x4140u), prmt(w0, 0u, 0x4342u), prmt(w1, 0u, 0x4342u),
+                    bf.x, bf.y, cinit, 0.f);
+    }
+  }
+  for (int c = 1; c < nch; ++c) {
+    p0 += 16; qi += 32;
     const uint2 bf = *qi;
 #pragma unroll
     for (int s = 0; s < 4; ++s) {
@@ -321,9 +354,22 @@ __device__ __forceinline__ void qk_i8(float (&acc)[4][4], const uint8_t* __restr
 }
 
 __device__ __forceinline__ void qk_i4(float (&acc)[4][4], const uint8_t* __restrict__ p0, int rowbytes, int nch,
-                                      const uint2* __restrict__ qi) {
+                                      const uint2* __restrict__ qi, float cinit) {
   const int rb8 = 8 * rowbytes;
-  for (int c = 0; c < nch; ++c, p0 += 16, qi += 64) {
+  {
+    const uint2 bf0 = qi[0], bf1 = qi[32];
+#pragma unroll
+    for (int s = 0; s < 4; ++s) {
+      const uint8_t* p = p0 + s * rowbytes;
+      const uint32_t w0 = *reinterpret_cast<const uint32_t*>(p);
+      const uint32_t w1 = *reinterpret_cast<const uint32_t*>(p + rb8);
+      const uint32_t v0 = w0 >> 8, v1 = w1 >> 8;
+      mma16816_init(acc[s], w0 & 0x000f000fu, w1 & 0x000f000fu, w0 & 0x00f000f0u, w1 & 0x00f000f0u, bf0.x, bf0.y, cinit, 0.f);
+      mma16816(acc[s], v0 & 0x000f000fu, v1 & 0x000f000fu, v0 & 0x00f000f0u, v1 & 0x00f000f0u, bf1.x, bf1.y);
+    }
+  }
+  for (int c = 1; c < nch; ++c) {
+    p0 += 16; qi += 64;
     const uint2 bf0 = qi[0], bf1 = qi[32];
 #pragma unroll
     for (int s = 0; s < 4; ++s) {
@@ -339,13 +385,13 @@ __device__ __forceinline__ void qk_i4(float (&acc)[4][4], const uint8_t* __restr
 
 template <int BITS>
 __device__ __forceinline__ void qk_block(float (&acc)[4][4], const uint8_t* __restrict__ blk, int n, int tb, int j,
-                                         const uint2* __restrict__ qi) {
+                                         const uint2* __restrict__ qi, float cinit) {
   if (BITS == 16) {
-    qk_f16(acc, blk + tb * (2 * n) + 8 * j, 2 * n, (n + 15) >> 4, qi);
+    qk_f16(acc, blk + tb * (2 * n) + 8 * j, 2 * n, (n + 15) >> 4, qi, cinit);
   } else if (BITS == 8) {
-    qk_i8(acc, blk + tb * n + 4 * j, n, (n + 15) >> 4, qi);
+    qk_i8(acc, blk + tb * n + 4 * j, n, (n + 15) >> 4, qi, cinit);
   } else {
-    qk_i4(acc, blk + tb * (n >> 1) + 4 * j, n >> 1, (n + 31) >> 5, qi);
+    qk_i4(acc, blk + tb * (n >> 1) + 4 * j, n >> 1, (n + 31) >> 5, qi, cinit);
   }
 }
 
@@ -456,11 +502,7 @@ __device__ __forceinline__ void score_page(const StarkvLayout& L, const DecodePl
     const int n_hi = L.k_hi_n[g];
     float chi[4][4];
     if (!QUANT) {
-#pragma unroll
-      for (int s = 0; s < 4; ++s)
-#pragma unroll
-        for (int e = 0; e < 4; ++e) chi[s][e] = 0.f;
-      qk_block<16>(chi, pg + L.k_hi_off[g], n_hi, tb, j, qi);
+      qk_block<16>(chi, pg + L.k_hi_off[g], n_hi, tb, j, qi, 0.f);
 #pragma unroll
       for (int s = 0; s < 4; ++s) {
         sc[s][0] += chi[s][0] + chi[s][1];
@@ -468,18 +510,12 @@ __device__ __forceinline__ void score_page(const StarkvLayout& L, const DecodePl
       }
     } else {
       const __half* ksc = reinterpret_cast<const __half*>(pg + L.k_scale_off) + (g * 2) * PTOK + tb;
-      const float c_hi = kcst[g * 8 + j];
-#pragma unroll
-      for (int s = 0; s < 4; ++s) { chi[s][0] = c_hi; chi[s][1] = 0.f; chi[s][2] = c_hi; chi[s][3] = 0.f; }
-      qk_block<BH>(chi, pg + L.k_hi_off[g], n_hi, tb, j, qi);
+      qk_block<BH>(chi, pg + L.k_hi_off[g], n_hi, tb, j, qi, kcst[g * 8 + j]);
       apply_k_scales(sc, chi, ksc);
       const int n_lo = L.k_lo_n[g];
       if (n_lo > 0) {
-        const float c_lo = kcst[g * 8 + 4 + j];
-#pragma unroll
-        for (int s = 0; s < 4; ++s) { chi[s][0] = c_lo; chi[s][1] = 0.f; chi[s][2] = c_lo; chi[s][3] = 0.f; }
         qi += 32 * (BH == 4 ? 2 * ((n_hi + 31) >> 5) : (n_hi + 15) >> 4);
-        qk_block<BL>(chi, pg + L.k_lo_off[g], n_lo, tb, j, qi);
+        qk_block<BL>(chi, pg + L.k_lo_off[g], n_lo, tb, j, qi, kcst[g * 8 + 4 + j]);
         apply_k_scales(sc, chi, ksc + PTOK);
       }
     }
@@ -732,12 +768,15 @@ __global__ void __launch_bounds__(NTHREADS, 1) decode_fast_kernel(
     if (st >= nstage) { st -= nstage; ++use; }   // nstage >= 3 > 2: at most one wrap
   }
 
-  // ================= merge the two groups (stage memory is free: every issued page was consumed) =================
+  // ================= merge the two groups and write the split-K partial (D7) =================
+  // Stage memory is free (every issued page was consumed): it holds m[2][32], l[2][32] and the partial in its
+  // global layout [head][4 + r_v], which is then streamed out with coalesced 16-byte stores.
   if (grp == 0) SK_STAMP(3);
   bar_sync(3, NCONS_THREADS);
   SK_STAMP(4);
-  float* mg = reinterpret_cast<float*>(smem + PL.off_stage);   // m[2][32], l[2][32], then group B's accumulators
-  float* accB = mg + 128;                                      // [((gw*MT + a)*NT + c)*4 + e][lane]
+  float* mg = reinterpret_cast<float*>(smem + PL.off_stage);
+  float* ost = mg + 128;
+  const int ST = (int)pstride;
   if (has_quad) {
     float lsum = l_run;
     lsum += __shfl_xor_sync(0xffffffffu, lsum, 4);
@@ -748,55 +787,54 @@ __global__ void __launch_bounds__(NTHREADS, 1) decode_fast_kernel(
       mg[64 + grp * 32 + 4 * gw + j] = lsum;
     }
   }
-  if (grp == 1) {
-#pragma unroll
-    for (int a = 0; a < MT; ++a)
-#pragma unroll
-      for (int c = 0; c < NT; ++c)
-#pragma unroll
-        for (int e = 0; e < 4; ++e) accB[((((gw * MT + a) * NT + c) * 4 + e) << 5) + lane] = acc[a][c][e];
-  }
   bar_sync(3, NCONS_THREADS);
-  if (grp == 1) return;
-
-  // ================= D7: write the split-K partial =================
-  if (tid < L.n_q_heads) {
-    const float mA = mg[tid], mB = mg[32 + tid];
-    const float ms = fmaxf(mA, mB);   // finite: group A always has a page
-    const float fA = exp2f(mA - ms), fB = mB == -INFINITY ? 0.f : exp2f(mB - ms);
-    my_parts[tid * pstride + 0] = ms;
-    my_parts[tid * pstride + 1] = mg[64 + tid] * fA + mg[96 + tid] * fB;
-  }
-  float fA[NT][2], fB[NT][2];
+  float fme[NT][2];   // this group's weight per head column: 2^(m_own - max(m_A, m_B)); group A always has a page
 #pragma unroll
   for (int c = 0; c < NT; ++c)
 #pragma unroll
     for (int e = 0; e < 2; ++e) {
       const int head = 8 * c + 2 * j + e;
       const float mA = mg[head], mB = mg[32 + head];
-      const float ms = fmaxf(mA, mB);
-      fA[c][e] = exp2f(mA - ms);
-      fB[c][e] = mB == -INFINITY ? 0.f : exp2f(mB - ms);
+      const float mo = grp ? mB : mA;
+      fme[c][e] = mo == -INFINITY ? 0.f : ex2(mo - fmaxf(mA, mB));
     }
+  if (tid < L.n_q_heads) {
+    const float mA = mg[tid], mB = mg[32 + tid];
+    const float ms = fmaxf(mA, mB);
+    const float wA = ex2(mA - ms), wB = mB == -INFINITY ? 0.f : ex2(mB - ms);
+    *reinterpret_cast<float4*>(ost + tid * ST) = make_float4(ms, mg[64 + tid] * wA + mg[96 + tid] * wB, 0.f, 0.f);
+  }
 #pragma unroll
-  for (int a = 0; a < MT; ++a) {
-    const int tile = gw + GW * a;
-    if (tile >= PL.v_tiles) break;
-    const int blk = tile >= PL.v_tiles_hi ? 1 : 0;
-    const int ch0 = 16 * (tile - (blk ? PL.v_tiles_hi : 0));
-    const int n = blk ? L.v_lo_n : L.v_hi_n;
-    const int cg = blk ? L.v_hi_n : 0;
+  for (int pass = 1; pass >= 0; --pass) {   // group B stores, then group A adds
+    if (grp == pass) {
 #pragma unroll
-    for (int c = 0; c < NT; ++c) {
-      const int h0 = 8 * c + 2 * j;
+      for (int a = 0; a < MT; ++a) {
+        const int tile = gw + GW * a;
+        if (tile < PL.v_tiles) {
+          const int blk = tile >= PL.v_tiles_hi ? 1 : 0;
+          const int ch0 = 16 * (tile - (blk ? PL.v_tiles_hi : 0));
+          const int n = blk ? L.v_lo_n : L.v_hi_n;
+          float* o0 = ost + 4 + (blk ? L.v_hi_n : 0) + ch0 + R;
 #pragma unroll
-      for (int e = 0; e < 4; ++e) {
-        const int head = h0 + (e & 1), ch = ch0 + R + 8 * (e >> 1);
-        const float vB = accB[((((gw * MT + a) * NT + c) * 4 + e) << 5) + lane];
-        if (head < L.n_q_heads && ch < n)
-          my_parts[head * pstride + 2 + cg + ch] = acc[a][c][e] * fA[c][e & 1] + vB * fB[c][e & 1];
+          for (int c = 0; c < NT; ++c)
+#pragma unroll
+            for (int e = 0; e < 4; ++e) {
+              const int head = 8 * c + 2 * j + (e & 1), dch = 8 * (e >> 1);
+              if (head < L.n_q_heads && ch0 + R + dch < n) {
+                float* o = o0 + head * ST + dch;
+                const float v = acc[a][c][e] * fme[c][e & 1];
+                *o = pass ? v : *o + v;
+              }
+            }
+        }
       }
     }
+    bar_sync(3, NCONS_THREADS);
+  }
+  {
+    const float4* src = reinterpret_cast<const float4*>(ost);
+    float4* dst = reinterpret_cast<float4*>(my_parts);
+    for (int i = tid; i < L.n_q_heads * ST / 4; i += NCONS_THREADS) dst[i] = src[i];
   }
   SK_STAMP(5);
 }
@@ -805,8 +843,12 @@ template <int BH, int BL, int NT, int MT>
 cudaError_t launch_fast(const starkv_ctx* ctx, dim3 grid, const uint8_t* qimg, size_t qimg_stride, const uint8_t* pool,
                         const int32_t* table, int max_pages, const int32_t* seq_lens, float* parts, int n_splits) {
   auto kern = decode_fast_kernel<BH, BL, NT, MT>;
-  cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, ctx->plan.smem_bytes);
-  if (e != cudaSuccess) return e;
+  static int smem_set = 0;   // largest dynamic shared-memory size already granted to this instantiation
+  if (ctx->plan.smem_bytes > smem_set) {
+    const cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, ctx->plan.smem_bytes);
+    if (e != cudaSuccess) return e;
+    smem_set = ctx->plan.smem_bytes;
+  }
   kern<<<grid, NTHREADS, ctx->plan.smem_bytes, ctx->stream>>>(ctx->L, ctx->plan, qimg, qimg_stride, pool, table, max_pages,
                                                               seq_lens, parts, n_splits);
   return cudaGetLastError();
@@ -860,7 +902,7 @@ int sk_fast_plan(starkv_ctx* ctx) {
   if (P.mt > 4) return 0;
   const int p_area = 4 * P_BUF_BYTES;
   const int qarea = round_up(P.qimg_bytes + L.n_kv_heads * 32, 128);   // image + accumulator start values
-  const int merge_bytes = 512 + GW * P.mt * P.nt * 4 * 32 * 4;
+  const int merge_bytes = 512 + L.n_q_heads * (L.rank_v + 4) * 4;
   const int fixed = qarea + p_area + 2 * 2 * 32 * 4 /* alpha */ + 128 /* flags */ +
                     128 /* barriers */ + 4 * TBL_SMEM + 128 /* base align */;
   const int avail = ctx->smem_optin - fixed;
@@ -917,6 +959,7 @@ int sk_decode_fast(starkv_ctx* ctx, const void* q, const void* pool, const int32
   if (ws_bytes < w.total) return STARKV_ERR_WORKSPACE;
   float* parts = reinterpret_cast<float*>((uint8_t*)ws + w.part_off);
   uint8_t* qimg = (uint8_t*)ws + w.qimg_off;
+  SK_PREFER_SMEM(ctx, qproj_kernel);
   qproj_kernel<<<dim3(L.n_kv_heads, batch), 256, 0, ctx->stream>>>(L, ctx->plan, (const __half*)q, (const __half*)B_k, qimg,
                                                                    w.qimg_stride);
   SK_CUDA_CHECK(ctx, cudaGetLastError());

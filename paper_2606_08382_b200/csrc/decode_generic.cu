@@ -122,7 +122,7 @@ __global__ void __launch_bounds__(128) decode_generic_kernel(
 #pragma unroll
   for (int k = 0; k < 4; ++k) {
     const int c = threadIdx.x + 128 * k;
-    if (c < L.rank_v) out[2 + c] = acc[k];
+    if (c < L.rank_v) out[SK_PART_ACC + c] = acc[k];
   }
 }
 
@@ -171,7 +171,7 @@ __global__ void __launch_bounds__(256) combine_kernel(const __grid_constant__ St
 #pragma unroll
     for (int i = 0; i < 8; ++i) lstar += rsm[i];
     for (int c = tid; c < L.rank_v; c += 256) {
-      const float* col = base + (size_t)s0 * sstride + 2 + c;
+      const float* col = base + (size_t)s0 * sstride + SK_PART_ACC + c;
       float a0 = 0.f, a1 = 0.f, a2 = 0.f, a3 = 0.f;
       int s = 0;
       for (; s + 4 <= ns; s += 4) {
@@ -216,11 +216,136 @@ __global__ void __launch_bounds__(256) combine_kernel(const __grid_constant__ St
   }
 }
 
+// Fast D8 + D9 for n_splits <= 512 and r_v <= 512: one block of 1024 threads per (head, sequence) with every
+// global load that does not depend on another issued up front (the B_v slice, the split maxima, the first 16
+// accumulator rows per thread), so the kernel costs about two memory round trips instead of one per split.
+//   thread = (channel c, split group sg); sg strides the splits; partial sums over sg meet in shared memory.
+__global__ void __launch_bounds__(1024) combine_fast_kernel(const __grid_constant__ StarkvLayout L,
+                                                            const float* __restrict__ parts, int n_splits,
+                                                            const __half* __restrict__ B_v, __half* __restrict__ out) {
+  __shared__ float wsm[512];
+  __shared__ float psum[1024];
+  __shared__ __align__(16) float red[8192];   // [slice][d]: slices * d_h = 1024 * 8
+  __shared__ float rsm[64];
+  const int head = blockIdx.x, b = blockIdx.y, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const int g = head / L.group;
+  const int rv = L.rank_v, dh = L.head_dim, dv = L.n_kv_heads * dh;
+  const size_t ps = sk_part_stride(rv);
+  const float* base = parts + ((size_t)b * n_splits * L.n_q_heads + head) * ps;
+  const size_t sstride = (size_t)L.n_q_heads * ps;
+  // ---- loads that depend on nothing
+  const int nd8 = dh >> 3, nsl = 1024 / nd8;   // 16-byte column groups, channel slices
+  const int d8 = tid % nd8, sl = tid / nd8;
+  const __half* bcol = B_v + (size_t)g * dh + 8 * d8;
+  uint4 bq[4];
+#pragma unroll
+  for (int k = 0; k < 4; ++k) {
+    const int c = sl + k * nsl;
+    bq[k] = (sl < nsl && c < rv) ? *reinterpret_cast<const uint4*>(bcol + (size_t)c * dv) : make_uint4(0, 0, 0, 0);
+  }
+  float2 ml = make_float2(-INFINITY, 0.f);
+  if (tid < n_splits) ml = *reinterpret_cast<const float2*>(base + (size_t)tid * sstride);
+  const int CW = rv <= 256 ? 256 : 512, nsg = 1024 / CW;
+  const int c = tid % CW, sg = tid / CW;
+  const float* col = base + SK_PART_ACC + c;
+  float v[16];
+#pragma unroll
+  for (int k = 0; k < 16; ++k) {
+    const int s = sg + nsg * k;
+    v[k] = (c < rv && s < n_splits) ? col[(size_t)s * sstride] : 0.f;
+  }
+  // ---- m* and the split weights
+  float mx = ml.x;
+#pragma unroll
+  for (int o = 16; o; o >>= 1) mx = fmaxf(mx, __shfl_xor_sync(0xffffffffu, mx, o));
+  if (lane == 0) rsm[warp] = mx;
+  __syncthreads();
+  float mstar = rsm[0];
+#pragma unroll
+  for (int i = 1; i < 32; ++i) mstar = fmaxf(mstar, rsm[i]);
+  const float w = ml.x == -INFINITY ? 0.f : exp2f(ml.x - mstar);
+  if (tid < 512) wsm[tid] = w;
+  float lp = w * ml.y;
+#pragma unroll
+  for (int o = 16; o; o >>= 1) lp += __shfl_xor_sync(0xffffffffu, lp, o);
+  if (lane == 0) rsm[32 + warp] = lp;
+  __syncthreads();
+  float lstar = 0.f;
+#pragma unroll
+  for (int i = 0; i < 32; ++i) lstar += rsm[32 + i];
+  // ---- o[c] = sum_s w_s acc_s[c]
+  float a0 = 0.f, a1 = 0.f;
+#pragma unroll
+  for (int k = 0; k < 16; k += 2) {
+    const int s = sg + nsg * k;
+    a0 = fmaf(s < n_splits ? wsm[s] : 0.f, v[k], a0);
+    a1 = fmaf(s + nsg < n_splits ? wsm[s + nsg] : 0.f, v[k + 1], a1);
+  }
+  for (int k0 = 16; sg + nsg * k0 < n_splits; k0 += 16) {   // more than 16 splits per thread
+#pragma unroll
+    for (int k = 0; k < 16; ++k) {
+      const int s = sg + nsg * (k0 + k);
+      v[k] = (c < rv && s < n_splits) ? col[(size_t)s * sstride] : 0.f;
+    }
+#pragma unroll
+    for (int k = 0; k < 16; ++k) {
+      const int s = sg + nsg * (k0 + k);
+      a0 = fmaf(s < n_splits ? wsm[s] : 0.f, v[k], a0);
+    }
+  }
+  psum[tid] = a0 + a1;
+  __syncthreads();
+  // ---- up-projection: thread (d8, sl) takes channels sl, sl + nsl, ...
+  const float inv = (mstar == -INFINITY || lstar == 0.f) ? 0.f : 1.f / lstar;
+  float acc[8] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
+  if (sl < nsl) {
+    auto fma8 = [&](const uint4& x, int cc) {
+      float o = psum[cc];
+      for (int q = 1; q < nsg; ++q) o += psum[cc + q * CW];
+      const float2 x0 = __half22float2(*reinterpret_cast<const __half2*>(&x.x)), x1 = __half22float2(*reinterpret_cast<const __half2*>(&x.y)),
+                   x2 = __half22float2(*reinterpret_cast<const __half2*>(&x.z)), x3 = __half22float2(*reinterpret_cast<const __half2*>(&x.w));
+      acc[0] = fmaf(o, x0.x, acc[0]); acc[1] = fmaf(o, x0.y, acc[1]); acc[2] = fmaf(o, x1.x, acc[2]); acc[3] = fmaf(o, x1.y, acc[3]);
+      acc[4] = fmaf(o, x2.x, acc[4]); acc[5] = fmaf(o, x2.y, acc[5]); acc[6] = fmaf(o, x3.x, acc[6]); acc[7] = fmaf(o, x3.y, acc[7]);
+    };
+#pragma unroll
+    for (int k = 0; k < 4; ++k)
+      if (sl + k * nsl < rv) fma8(bq[k], sl + k * nsl);
+    for (int cc = sl + 4 * nsl; cc < rv; cc += nsl) fma8(*reinterpret_cast<const uint4*>(bcol + (size_t)cc * dv), cc);
+    float* r = red + sl * dh + 8 * d8;
+    *reinterpret_cast<float4*>(r) = make_float4(acc[0], acc[1], acc[2], acc[3]);
+    *reinterpret_cast<float4*>(r + 4) = make_float4(acc[4], acc[5], acc[6], acc[7]);
+  }
+  __syncthreads();
+  // ---- reduce the slices: (d, part) sums every np-th slice, then np partial sums per column
+  const int np = 1024 / dh;   // >= 4
+  {
+    const int d = tid % dh, p = tid / dh;
+    float s = 0.f;
+    if (p < np)
+      for (int k = p; k < nsl; k += np) s += red[k * dh + d];
+    __syncthreads();
+    if (p < np) psum[p * dh + d] = s;
+  }
+  __syncthreads();
+  if (tid < dh) {
+    float s = 0.f;
+    for (int p = 0; p < np; ++p) s += psum[p * dh + tid];
+    out[((size_t)b * L.n_q_heads + head) * dh + tid] = __float2half_rn(s * inv);
+  }
+}
+
 }  // namespace
 
 int sk_launch_combine(starkv_ctx* ctx, const float* parts, int n_splits, int batch, const void* B_v, void* out) {
-  combine_kernel<<<dim3(ctx->L.n_q_heads, batch), 256, 0, ctx->stream>>>(ctx->L, parts, n_splits, (const __half*)B_v,
-                                                                         (__half*)out);
+  if (n_splits <= 512 && ctx->L.rank_v <= 512) {
+    SK_PREFER_SMEM(ctx, combine_fast_kernel);
+    combine_fast_kernel<<<dim3(ctx->L.n_q_heads, batch), 1024, 0, ctx->stream>>>(ctx->L, parts, n_splits, (const __half*)B_v,
+                                                                                 (__half*)out);
+  } else {
+    SK_PREFER_SMEM(ctx, combine_kernel);
+    combine_kernel<<<dim3(ctx->L.n_q_heads, batch), 256, 0, ctx->stream>>>(ctx->L, parts, n_splits, (const __half*)B_v,
+                                                                           (__half*)out);
+  }
   SK_CUDA_CHECK(ctx, cudaGetLastError());
   return STARKV_OK;
 }

@@ -335,6 +335,50 @@ def run_reference(args, cfg):
     print(json.dumps(line))
 
 
+def prefill_append_leg(wl, sk, torch, device, T):
+    """starkv_append on T new tokens spread over the batch (positions at the end of each sequence), in dense-KV
+    mode (K/V rows in, north_star's call) and hidden-state mode (x in).  Device-resident inputs,
+    CUDA events around 20 calls; flops = 2 * T * d_in * columns of the projections only."""
+    cfg = wl.cfg
+    B, per = cfg.batch, T // cfg.batch
+    T = per * B
+    seq = torch.arange(B, dtype=torch.int32, device=device).repeat_interleave(per)
+    pos = (torch.arange(per, dtype=torch.int32, device=device) + (cfg.context - per)).repeat(B)
+    wsb = sk.starkv_append_workspace_bytes(wl.ctx, T)
+    ws = torch.empty(wsb, dtype=torch.uint8, device=device)
+    f16 = lambda a: torch.from_numpy(np.ascontiguousarray(a).view(np.int16)).to(device).view(torch.float16)  # noqa: E731
+    out = {"tokens": T, "kernels": "append_project_mma_kernel (mma.sync m16n8k16, fp32 accumulate) + append_write_kernel"}
+    for mode in ("dense", "hidden"):
+        if mode == "dense":
+            dk, dv, khs = cfg.head_dim, cfg.n_kv_heads * cfg.head_dim, cfg.head_dim
+            kn, vn = synth.make_append_inputs(cfg, T, mode="dense")
+            k, v = f16(kn.reshape(T, -1)), f16(vn)
+            ak, av = wl.ak, wl.av
+            flops = 2.0 * T * (cfg.head_dim * cfg.sum_rank_k + dv * cfg.rank_v)
+        else:
+            dk = dv = cfg.d_model
+            khs = 0
+            xn, _ = synth.make_append_inputs(cfg, T, mode="hidden")
+            k = v = f16(xn)
+            a1, a2 = synth.make_append_factors(cfg, dk, dv)
+            ak, av = f16(a1), f16(a2)
+            flops = 2.0 * T * cfg.d_model * (cfg.sum_rank_k + cfg.rank_v)
+        call = lambda: sk.starkv_append(wl.ctx, wl.pool, wl.table_of(0), wl.max_pages, seq, pos, T, k, k.shape[1], khs,  # noqa: E731
+                                        dk, v, v.shape[1], dv, ak, av, ws, wsb)
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        with torch.cuda.stream(wl.stream):
+            for _ in range(3):
+                call()
+            e0.record(wl.stream)
+            for _ in range(20):
+                call()
+            e1.record(wl.stream)
+            wl.stream.synchronize()
+        us = e0.elapsed_time(e1) * 1e3 / 20
+        out[mode] = {"us_per_call": us, "projection_tflops": flops / (us * 1e-6) / 1e12, "d_in_k": dk, "d_in_v": dv}
+    return out
+
+
 def workload_name(cfg) -> str:
     kind = "fp16 latents" if not cfg.quantized else f"int{cfg.bits_hi}/int{cfg.bits_lo} latents"
     return (f"{cfg.name}: BASELINE.json configs[{int(cfg.name[1]) - 1}], 1 layer, batch {cfg.batch}, "
@@ -438,6 +482,9 @@ def run_ours(args, cfg):
     peak, peak_src = measured_peak()
     achieved = kernel_bytes(cfg) / (k_ms * 1e-3) / 1e9
 
+    # ---- C4: the compress-on-append kernel on a prefill chunk (BASELINE.json configs[3]) ----
+    prefill = prefill_append_leg(wl, sk, torch, device, args.prefill_tokens) if (cfg.name == "C4" or args.prefill) else None
+
     # ---- clocks: if the timed loops were too short to be sampled, dwell on the same load ----
     if sampler.ok and sum(1 for s in sampler.samples if s[0]) < 8:
         sampler.timed = True
@@ -477,6 +524,8 @@ def run_ours(args, cfg):
                      "launches_timed": Kr, "algorithmic_bytes_per_launch": kernel_bytes(cfg),
                      "frac_of_nominal_8TBs": achieved / NOMINAL_HBM_GBS},
     }
+    if prefill is not None:
+        line["append_prefill"] = prefill
     if world == 1 and not args.no_cpu:
         line["cpu_baseline"] = cpu_baseline(cfg)
     print(json.dumps(line))
@@ -493,6 +542,8 @@ def main():
     ap.add_argument("--workload", default="C2", help="C2 (default: the config the metric is quoted on), C3, C4, C5")
     ap.add_argument("--replicas", type=int, default=0)
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
+    ap.add_argument("--prefill", action="store_true", help="also time starkv_append on a prefill chunk (always on for C4)")
+    ap.add_argument("--prefill-tokens", type=int, default=2048)
     ap.add_argument("--verbose", action="store_true")
     args = ap.parse_args()
     cfg = synth.make_config(args.workload)

@@ -41,6 +41,10 @@ int starkv_create(starkv_ctx** out, const starkv_desc* d, void* cuda_stream) {
     free(ctx);
     return STARKV_ERR_CUDA;
   }
+  {
+    const char* e_pdl = getenv("STARKV_PDL");
+    ctx->pdl = !(e_pdl && e_pdl[0] == '0');
+  }
   sk_fast_plan(ctx);
   *out = ctx;
   return STARKV_OK;

@@ -261,6 +261,7 @@ __global__ void __launch_bounds__(256) append_project_small_kernel(
     long long k_row_stride, long long k_head_stride, int d_in_k, const __half* __restrict__ v_new, long long v_row_stride,
     int d_in_v, const __half* __restrict__ A_k, const __half* __restrict__ A_v, float* __restrict__ zp) {
   __shared__ __align__(16) float sm[8 * APS_TOK * APS_COLS];   // x chunk [16][256] during the loop, then the warp partials
+  sk_pdl_enter();
   const int R = L.sum_rank_k + L.rank_v;
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const __half* x0;
@@ -329,6 +330,135 @@ __global__ void __launch_bounds__(256) append_project_small_kernel(
 }
 
 // ---------------------------------------------------------------------------------------------
+// append, step A1 for many new tokens (prefill): z = fp16(X . A) on tensor cores (mma.sync m16n8k16, fp32
+// accumulation).  CTA tile 64 tokens x 64 latent columns, K step 32, 4 warps (2 x 2, warp tile 32 x 32),
+// cp.async double buffering, ldmatrix fragments (A operand from the token-major X tile, B operand by
+// ldmatrix.trans from the k-major A tile).  grid (column tiles of keys then values, token tiles).
+// Requires 16-byte aligned rows: d_in % 8 == 0, row strides % 8 == 0 (else the scalar kernel runs).
+// ---------------------------------------------------------------------------------------------
+constexpr int GM = 64, GN = 64, GK = 32;
+constexpr int GXS = GK + 8;   // X tile row stride in halves (80 B: conflict-free ldmatrix)
+constexpr int GAS = GN + 8;   // A tile row stride in halves (144 B)
+
+__device__ __forceinline__ void cp_async16(void* smem_dst, const void* gsrc, bool pred) {
+  const uint32_t d = (uint32_t)__cvta_generic_to_shared(smem_dst);
+  const int n = pred ? 16 : 0;   // src-size 0: zero fill
+  asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" ::"r"(d), "l"(gsrc), "r"(n) : "memory");
+}
+__device__ __forceinline__ void ldsm_x4(uint32_t (&r)[4], const void* p) {
+  const uint32_t a = (uint32_t)__cvta_generic_to_shared(p);
+  asm volatile("ldmatrix.sync.aligned.m8n8.x4.shared.b16 {%0,%1,%2,%3}, [%4];" : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]) : "r"(a));
+}
+__device__ __forceinline__ void ldsm_x4_trans(uint32_t (&r)[4], const void* p) {
+  const uint32_t a = (uint32_t)__cvta_generic_to_shared(p);
+  asm volatile("ldmatrix.sync.aligned.m8n8.x4.trans.shared.b16 {%0,%1,%2,%3}, [%4];" : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]) : "r"(a));
+}
+__device__ __forceinline__ void hmma16816(float (&d)[4], const uint32_t (&a)[4], uint32_t b0, uint32_t b1) {
+  asm volatile(
+      "mma.sync.aligned.m16n8k16.row.col.f32.f16.f16.f32 {%0,%1,%2,%3}, {%4,%5,%6,%7}, {%8,%9}, {%0,%1,%2,%3};"
+      : "+f"(d[0]), "+f"(d[1]), "+f"(d[2]), "+f"(d[3])
+      : "r"(a[0]), "r"(a[1]), "r"(a[2]), "r"(a[3]), "r"(b0), "r"(b1));
+}
+
+__global__ void __launch_bounds__(128) append_project_mma_kernel(
+    const __grid_constant__ StarkvLayout L, int n_new, int n_key_tiles, const __half* __restrict__ k_new,
+    long long k_row_stride, long long k_head_stride, int d_in_k, const __half* __restrict__ v_new, long long v_row_stride,
+    int d_in_v, const __half* __restrict__ A_k, const __half* __restrict__ A_v, __half* __restrict__ z) {
+  __shared__ __align__(16) __half xs[2][GM * GXS];
+  __shared__ __align__(16) __half as[2][GK * GAS];
+  const int R = L.sum_rank_k + L.rank_v;
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const int wm = warp >> 1, wn = warp & 1;
+  const __half* x0;
+  long long xstride;
+  int d_in, ncols, col_out0, lda;
+  const __half* A;
+  if ((int)blockIdx.x < n_key_tiles) {
+    int h = 0, t = blockIdx.x;
+    while (t >= (L.rank_k[h] + GN - 1) / GN) { t -= (L.rank_k[h] + GN - 1) / GN; ++h; }
+    const int c0 = t * GN;
+    x0 = k_new + (long long)h * k_head_stride; xstride = k_row_stride; d_in = d_in_k;
+    ncols = min(GN, L.rank_k[h] - c0); col_out0 = L.koff[h] + c0; A = A_k + L.koff[h] + c0; lda = L.sum_rank_k;
+  } else {
+    const int c0 = (blockIdx.x - n_key_tiles) * GN;
+    x0 = v_new; xstride = v_row_stride; d_in = d_in_v;
+    ncols = min(GN, L.rank_v - c0); col_out0 = L.sum_rank_k + c0; A = A_v + c0; lda = L.rank_v;
+  }
+  const int m0 = blockIdx.y * GM;
+  auto load_tiles = [&](int buf, int k0) {
+    // X tile: 64 rows x 32 halves = 256 chunks of 16 B, 2 per thread
+#pragma unroll
+    for (int u = 0; u < 2; ++u) {
+      const int ci = tid + 128 * u, row = ci >> 2, kc = (ci & 3) * 8;
+      const bool ok = m0 + row < n_new && k0 + kc < d_in;
+      const __half* src = x0 + (long long)(ok ? m0 + row : 0) * xstride + (ok ? k0 + kc : 0);
+      cp_async16(&xs[buf][row * GXS + kc], src, ok);
+    }
+    // A tile: 32 rows (k) x 64 halves = 256 chunks
+#pragma unroll
+    for (int u = 0; u < 2; ++u) {
+      const int ci = tid + 128 * u, row = ci >> 3, nc = (ci & 7) * 8;
+      const bool ok = k0 + row < d_in && nc < ncols;
+      const __half* src = A + (size_t)(ok ? k0 + row : 0) * lda + (ok ? nc : 0);
+      cp_async16(&as[buf][row * GAS + nc], src, ok);
+    }
+    asm volatile("cp.async.commit_group;" ::: "memory");
+  };
+  float acc[2][4][4];
+#pragma unroll
+  for (int a = 0; a < 2; ++a)
+#pragma unroll
+    for (int b = 0; b < 4; ++b)
+#pragma unroll
+      for (int e = 0; e < 4; ++e) acc[a][b][e] = 0.f;
+  const int nk = (d_in + GK - 1) / GK;
+  load_tiles(0, 0);
+  for (int kt = 0; kt < nk; ++kt) {
+    const int buf = kt & 1;
+    if (kt + 1 < nk) {
+      load_tiles(buf ^ 1, (kt + 1) * GK);
+      asm volatile("cp.async.wait_group 1;" ::: "memory");
+    } else {
+      asm volatile("cp.async.wait_group 0;" ::: "memory");
+    }
+    __syncthreads();
+#pragma unroll
+    for (int ks = 0; ks < GK; ks += 16) {
+      uint32_t af[2][4], bf[2][4];
+      // A operand: rows = tokens.  lanes 0-15 address rows 0-15 at k 0, lanes 16-31 the same rows at k + 8
+#pragma unroll
+      for (int a = 0; a < 2; ++a)
+        ldsm_x4(af[a], &xs[buf][(wm * 32 + a * 16 + (lane & 15)) * GXS + ks + (lane >> 4) * 8]);
+      // B operand (k-major tile, transposed load): matrices (k 0-7, n 0-7), (k 8-15, n 0-7), (k 0-7, n 8-15), (k 8-15, n 8-15)
+#pragma unroll
+      for (int b = 0; b < 2; ++b)
+        ldsm_x4_trans(bf[b], &as[buf][(ks + (lane & 7) + ((lane >> 3) & 1) * 8) * GAS + wn * 32 + b * 16 + (lane >> 4) * 8]);
+#pragma unroll
+      for (int a = 0; a < 2; ++a)
+#pragma unroll
+        for (int b = 0; b < 4; ++b) hmma16816(acc[a][b], af[a], bf[b >> 1][(b & 1) * 2], bf[b >> 1][(b & 1) * 2 + 1]);
+    }
+    __syncthreads();
+  }
+  // epilogue: one rounding to fp16, rows = tokens
+#pragma unroll
+  for (int a = 0; a < 2; ++a)
+#pragma unroll
+    for (int b = 0; b < 4; ++b) {
+      const int col = wn * 32 + b * 8 + 2 * (lane & 3);
+      if (col < ncols) {
+#pragma unroll
+        for (int hh = 0; hh < 2; ++hh) {
+          const int row = m0 + wm * 32 + a * 16 + (lane >> 2) + 8 * hh;
+          if (row < n_new)
+            *reinterpret_cast<__half2*>(z + (size_t)row * R + col_out0 + col) =
+                __floats2half2_rn(acc[a][b][2 * hh], acc[a][b][2 * hh + 1]);
+        }
+      }
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
 // append, steps A2-A4: per-token scales, codes, pack, paged write.  One CTA per new token.
 // 4-bit value fields share a byte between two slots: set with atomicAnd/atomicOr on the
 // containing word so that concurrent appends to neighbouring slots cannot lose an update.
@@ -344,6 +474,7 @@ __global__ void __launch_bounds__(256) append_write_kernel(const __grid_constant
   extern __shared__ __align__(16) uint8_t sm[];
   __half* zr = reinterpret_cast<__half*>(sm);
   __shared__ float vsc[2];
+  sk_pdl_enter();
   const int j = blockIdx.x;
   const int P = L.page_tokens;
   const int R = L.sum_rank_k + L.rank_v;
@@ -502,10 +633,20 @@ int sk_append(starkv_ctx* ctx, void* pool, const int32_t* table, int max_pages, 
     for (int h = 0; h < L.n_kv_heads; ++h) nkt += (L.rank_k[h] + APS_COLS - 1) / APS_COLS;
     const int nvt = (L.rank_v + APS_COLS - 1) / APS_COLS;
     SK_PREFER_SMEM(ctx, append_project_small_kernel);
-    append_project_small_kernel<<<dim3(nkt + nvt, APS_KS), 256, 0, ctx->stream>>>(
+    sk_launch(ctx, append_project_small_kernel, dim3(nkt + nvt, APS_KS), dim3(256), 0,
         L, n_new, nkt, (const __half*)k_new, k_row_stride, k_head_stride, d_in_k, (const __half*)v_new, v_row_stride, d_in_v,
         (const __half*)A_k, (const __half*)A_v, (float*)ws);
     zp = (const float*)ws;
+  } else if (d_in_k % 8 == 0 && d_in_v % 8 == 0 && k_row_stride % 8 == 0 && k_head_stride % 8 == 0 && v_row_stride % 8 == 0 &&
+             ((uintptr_t)k_new & 15) == 0 && ((uintptr_t)v_new & 15) == 0 && ((uintptr_t)A_k & 15) == 0 &&
+             ((uintptr_t)A_v & 15) == 0) {
+    int nkt = 0;
+    for (int h = 0; h < L.n_kv_heads; ++h) nkt += (L.rank_k[h] + GN - 1) / GN;
+    const int nvt = (L.rank_v + GN - 1) / GN;
+    SK_PREFER_SMEM(ctx, append_project_mma_kernel);
+    append_project_mma_kernel<<<dim3(nkt + nvt, (n_new + GM - 1) / GM), 128, 0, ctx->stream>>>(
+        L, n_new, nkt, (const __half*)k_new, k_row_stride, k_head_stride, d_in_k, (const __half*)v_new, v_row_stride, d_in_v,
+        (const __half*)A_k, (const __half*)A_v, z);
   } else {
   dim3 g1(L.n_kv_heads + (L.rank_v + 127) / 128, (n_new + APP_TOK - 1) / APP_TOK);
   append_project_kernel<<<g1, 128, 0, ctx->stream>>>(L, n_new, (const __half*)k_new, k_row_stride, k_head_stride, d_in_k,
@@ -518,7 +659,8 @@ int sk_append(starkv_ctx* ctx, void* pool, const int32_t* table, int max_pages, 
   if (smem > 48 * 1024)
     SK_CUDA_CHECK(ctx, cudaFuncSetAttribute(append_write_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
   SK_PREFER_SMEM(ctx, append_write_kernel);
-  append_write_kernel<<<n_new, 256, smem, ctx->stream>>>(L, z, zp, APS_KS, n_new, seq_ids, positions, table, max_pages, (uint8_t*)pool);
+  sk_launch(ctx, append_write_kernel, dim3(n_new), dim3(256), smem, L, (const __half*)z, zp, (int)APS_KS, n_new, seq_ids,
+            positions, table, max_pages, (uint8_t*)pool);
   ctx->last_launches = 2;
   SK_CUDA_CHECK(ctx, cudaGetLastError());
   return STARKV_OK;

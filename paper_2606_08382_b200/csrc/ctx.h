@@ -18,6 +18,7 @@ struct starkv_ctx {
   int last_launches;
   int fast_ok;           // tensor-core decode kernel covers this descriptor
   DecodePlan plan;
+  int pdl;               // launch the step's kernels with programmatic dependent launch (STARKV_PDL=0 disables)
   int timing_on;         // record events around the main decode kernel
   int timing_valid;
   cudaEvent_t ev0, ev1;
@@ -44,6 +45,32 @@ int sk_cuda_fail(starkv_ctx* ctx, cudaError_t e, const char* what);
       _done = true;                                                                                       \
     }                                                                                                     \
   } while (0)
+
+// Programmatic dependent launch (PDL): the kernels of a step are launched with the stream-serialization
+// attribute, trigger their dependents at once and wait for their predecessor (griddepcontrol.wait) before touching
+// global memory, so a kernel's launch latency and CTA ramp overlap the tail of the one before it.  Every such
+// kernel waits, hence completion stays transitive: kernel K done implies kernel K-1 done.
+#ifdef __CUDACC__
+__device__ __forceinline__ void sk_pdl_enter() {
+  asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+  asm volatile("griddepcontrol.wait;" ::: "memory");
+}
+template <typename... KArgs, typename... Args>
+static inline cudaError_t sk_launch(const starkv_ctx* ctx, void (*kern)(KArgs...), dim3 grid, dim3 block, size_t smem,
+                                    Args... args) {
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = grid;
+  cfg.blockDim = block;
+  cfg.dynamicSmemBytes = smem;
+  cfg.stream = ctx->stream;
+  cudaLaunchAttribute at[1];
+  at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  at[0].val.programmaticStreamSerializationAllowed = 1;
+  cfg.attrs = at;
+  cfg.numAttrs = ctx->pdl ? 1 : 0;
+  return cudaLaunchKernelEx(&cfg, kern, args...);
+}
+#endif
 
 // codec.cu
 int sk_pack(starkv_ctx* ctx, const void* lk, const void* lv, int n_tokens, void* pages);

@@ -179,6 +179,7 @@ __global__ void __launch_bounds__(256) qproj_kernel(const __grid_constant__ Star
                                                     const __half* __restrict__ B_k, uint8_t* __restrict__ qimg_all,
                                                     size_t qimg_stride) {
   __shared__ float qt[256][4];   // q~[ch][i]
+  sk_pdl_enter();
   const int g = blockIdx.x, b = blockIdx.y;
   const int G = L.group, dh = L.head_dim, r = L.rank_k[g];
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
@@ -576,6 +577,7 @@ __global__ void __launch_bounds__(NTHREADS, 1) decode_fast_kernel(
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const int j = lane & 3, R = lane >> 2;
   const int split = blockIdx.x, b = blockIdx.y;
+  sk_pdl_enter();
   const int len = seq_lens[b];
   const int n_pages = (len + PTOK - 1) / PTOK;
   int p0, p1;
@@ -765,7 +767,7 @@ __global__ void __launch_bounds__(NTHREADS, 1) decode_fast_kernel(
       }
     }
     st += 2;
-    if (st >= nstage) { st -= nstage; ++use; }   // nstage >= 3 > 2: at most one wrap
+    if (st >= nstage) { st -= nstage; ++use; }   // nstage >= 2: at most one wrap
   }
 
   // ================= merge the two groups and write the split-K partial (D7) =================
@@ -788,6 +790,7 @@ __global__ void __launch_bounds__(NTHREADS, 1) decode_fast_kernel(
     }
   }
   bar_sync(3, NCONS_THREADS);
+  SK_STAMP(6);
   float fme[NT][2];   // this group's weight per head column: 2^(m_own - max(m_A, m_B)); group A always has a page
 #pragma unroll
   for (int c = 0; c < NT; ++c)
@@ -831,6 +834,7 @@ __global__ void __launch_bounds__(NTHREADS, 1) decode_fast_kernel(
     }
     bar_sync(3, NCONS_THREADS);
   }
+  SK_STAMP(7);
   {
     const float4* src = reinterpret_cast<const float4*>(ost);
     float4* dst = reinterpret_cast<float4*>(my_parts);
@@ -849,9 +853,8 @@ cudaError_t launch_fast(const starkv_ctx* ctx, dim3 grid, const uint8_t* qimg, s
     if (e != cudaSuccess) return e;
     smem_set = ctx->plan.smem_bytes;
   }
-  kern<<<grid, NTHREADS, ctx->plan.smem_bytes, ctx->stream>>>(ctx->L, ctx->plan, qimg, qimg_stride, pool, table, max_pages,
-                                                              seq_lens, parts, n_splits);
-  return cudaGetLastError();
+  return sk_launch(ctx, kern, grid, dim3(NTHREADS), (size_t)ctx->plan.smem_bytes, ctx->L, ctx->plan, qimg, qimg_stride, pool,
+                   table, max_pages, seq_lens, parts, n_splits);
 }
 
 template <int BH, int BL>
@@ -908,7 +911,7 @@ int sk_fast_plan(starkv_ctx* ctx) {
   const int avail = ctx->smem_optin - fixed;
   int ns = avail / L.page_bytes;
   if (ns > 8) ns = 8;
-  if (ns < 3) return 0;   // two groups in flight need a third stage to keep a copy in flight
+  if (ns < 2) return 0;   // one stage per group at least (a third keeps a copy in flight while both compute)
   if ((long long)ns * L.page_bytes < merge_bytes) {
     if (merge_bytes > avail) return 0;
   }
@@ -960,9 +963,8 @@ int sk_decode_fast(starkv_ctx* ctx, const void* q, const void* pool, const int32
   float* parts = reinterpret_cast<float*>((uint8_t*)ws + w.part_off);
   uint8_t* qimg = (uint8_t*)ws + w.qimg_off;
   SK_PREFER_SMEM(ctx, qproj_kernel);
-  qproj_kernel<<<dim3(L.n_kv_heads, batch), 256, 0, ctx->stream>>>(L, ctx->plan, (const __half*)q, (const __half*)B_k, qimg,
-                                                                   w.qimg_stride);
-  SK_CUDA_CHECK(ctx, cudaGetLastError());
+  SK_CUDA_CHECK(ctx, sk_launch(ctx, qproj_kernel, dim3(L.n_kv_heads, batch), dim3(256), 0, L, ctx->plan, (const __half*)q,
+                               (const __half*)B_k, qimg, w.qimg_stride));
   const dim3 grid(w.n_splits, batch);
   const uint8_t* pl = (const uint8_t*)pool;
   if (ctx->timing_on) SK_CUDA_CHECK(ctx, cudaEventRecord(ctx->ev0, ctx->stream));

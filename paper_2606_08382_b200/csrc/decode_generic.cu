@@ -228,6 +228,7 @@ __global__ void __launch_bounds__(1024) combine_fast_kernel(const __grid_constan
   __shared__ __align__(16) float red[8192];   // [slice][d]: slices * d_h = 1024 * 8
   __shared__ float rsm[64];
   const int head = blockIdx.x, b = blockIdx.y, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  sk_pdl_enter();
   const int g = head / L.group;
   const int rv = L.rank_v, dh = L.head_dim, dv = L.n_kv_heads * dh;
   const size_t ps = sk_part_stride(rv);
@@ -339,8 +340,8 @@ __global__ void __launch_bounds__(1024) combine_fast_kernel(const __grid_constan
 int sk_launch_combine(starkv_ctx* ctx, const float* parts, int n_splits, int batch, const void* B_v, void* out) {
   if (n_splits <= 512 && ctx->L.rank_v <= 512) {
     SK_PREFER_SMEM(ctx, combine_fast_kernel);
-    combine_fast_kernel<<<dim3(ctx->L.n_q_heads, batch), 1024, 0, ctx->stream>>>(ctx->L, parts, n_splits, (const __half*)B_v,
-                                                                                 (__half*)out);
+    SK_CUDA_CHECK(ctx, sk_launch(ctx, combine_fast_kernel, dim3(ctx->L.n_q_heads, batch), dim3(1024), 0, ctx->L, parts, n_splits,
+                                 (const __half*)B_v, (__half*)out));
   } else {
     SK_PREFER_SMEM(ctx, combine_kernel);
     combine_kernel<<<dim3(ctx->L.n_q_heads, batch), 256, 0, ctx->stream>>>(ctx->L, parts, n_splits, (const __half*)B_v,

@@ -67,7 +67,7 @@ def test_pack_empty_is_a_no_op():
     sk.starkv_unpack(ctx, None, 0)
 
 
-def _append_case(cfg, mode, n_new, dyadic):
+def _append_case(cfg, mode, n_new, dyadic, pad=0):
     d = CacheDesc.from_config(cfg)
     lay = page_layout(d)
     rng = np.random.default_rng(5)
@@ -104,14 +104,18 @@ def _append_case(cfg, mode, n_new, dyadic):
     k2 = np.ascontiguousarray(k.reshape(n, -1))
     v2 = np.ascontiguousarray(v.reshape(n, -1))
     ref = pool.copy()
+    kw, vw = k2.shape[1], v2.shape[1]
     oappend.append(d, ref, table, seq_ids, positions, k2, khs, d_in_k, v2, ak, av)
     ctx = sk.create_from_config(cfg)
     dpool = dev(pool)
     wsb = sk.starkv_append_workspace_bytes(ctx, n)
     ws = torch.empty(max(wsb, 16), dtype=torch.uint8, device="cuda")
+    if pad:   # row strides that are not a multiple of 8 elements: the tensor-core kernel's alignment rule fails
+        k2 = np.ascontiguousarray(np.pad(k2, ((0, 0), (0, pad))))
+        v2 = np.ascontiguousarray(np.pad(v2, ((0, 0), (0, pad))))
     kd, vd = f16(k2), f16(v2)
     sk.starkv_append(ctx, dpool, dev(table.astype(np.int32)), table.shape[1], dev(seq_ids), dev(positions), n,
-                     kd, k2.shape[1], khs, d_in_k, vd, v2.shape[1], d_in_v, f16(ak), f16(av), ws, wsb)
+                     kd, kw + pad, khs, d_in_k, vd, vw + pad, d_in_v, f16(ak), f16(av), ws, wsb)
     torch.cuda.synchronize()
     return d, lay, dpool.cpu().numpy(), ref, n
 
@@ -123,6 +127,12 @@ def test_append_bit_exact_on_dyadic_inputs(name, mode, n_new):
     cfg = synth.make_config(name, context=256, batch=3)
     d, lay, got, ref, n = _append_case(cfg, mode, n_new, dyadic=True)
     assert np.array_equal(got, ref), f"{int((got != ref).sum())} bytes differ of {got.size}"
+
+
+def test_append_unaligned_rows_take_the_scalar_kernel():
+    cfg = synth.make_config("C3", context=256, batch=3)
+    d, lay, got, ref, n = _append_case(cfg, "dense", 37, dyadic=True, pad=2)
+    assert np.array_equal(got, ref)
 
 
 @pytest.mark.parametrize("n_new", [40, 8])

@@ -153,10 +153,10 @@ class ClockSampler:
 class Workload:
     """Device-resident replicas of one config's cache + everything a step needs."""
 
-    def __init__(self, cfg, sk, torch, device, n_rep=None, verbose=False):
+    def __init__(self, cfg, sk, torch, device, n_rep=None, verbose=False, stream=None):
         self.cfg, self.sk, self.torch = cfg, sk, torch
         B, ctxlen, P = cfg.batch, cfg.context, cfg.page_tokens
-        self.stream = torch.cuda.Stream(device=device)
+        self.stream = stream if stream is not None else torch.cuda.Stream(device=device)
         self.ctx = sk.create_from_config(cfg, stream=self.stream)
         page_bytes = sk.starkv_page_bytes(self.ctx)
         cache_bytes = kernel_bytes(cfg)
@@ -533,6 +533,157 @@ def run_ours(args, cfg):
         dist.destroy_process_group()
 
 
+# ------------------------------------------------------------------------------------------------
+# C5: the full 32-layer decode step (BASELINE.json configs[4])
+# ------------------------------------------------------------------------------------------------
+N_LAYERS_C5 = 32
+# LLaMA-3.1-8B-shaped weights read once per decode step: 32 x (q,o 2 x 4096^2 + k,v 2 x 4096 x 1024
+# + mlp 3 x 4096 x 14336) + lm_head 128256 x 4096, fp16
+NON_ATTN_WEIGHT_BYTES = 2 * (32 * (2 * 4096 * 4096 + 2 * 4096 * 1024 + 3 * 4096 * 14336) + 128256 * 4096)
+
+
+def run_c5(args):
+    """One step = starkv_append + starkv_decode_attn for each of the 32 layers (each layer its own rank table,
+    context and cache), captured as one CUDA graph.  The 32 caches (2.9 GB) are the L2 defeat."""
+    import torch
+    import torch.distributed as dist
+
+    import paper_2606_08382_b200 as sk
+    from paper_2606_08382_b200.sharding import max_over_ranks
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the product path has no CPU fallback")
+    torch.cuda.set_device(local)
+    device = torch.device("cuda", local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=device)
+    K, W = args.steps, max(args.warmup, 3)
+    n_layers = args.layers or N_LAYERS_C5
+    stream = torch.cuda.Stream(device=device)
+    layers = []
+    t0 = time.time()
+    for l in range(n_layers):
+        cfg = synth.make_config("C5", layer=l)
+        layers.append(Workload(cfg, sk, torch, device, n_rep=1, stream=stream))
+    if rank == 0 and args.verbose:
+        print(f"# built {n_layers} layer caches in {time.time() - t0:.1f}s", file=sys.stderr)
+    bytes_step = sum(step_bytes(w.cfg) for w in layers)
+    bytes_kern = sum(kernel_bytes(w.cfg) for w in layers)
+
+    def step():
+        for w in layers:
+            w.step(0)
+
+    with torch.cuda.stream(stream):
+        for _ in range(W):
+            step()
+        stream.synchronize()
+        g = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(g, stream=stream):
+            step()
+        for _ in range(W):
+            g.replay()
+        stream.synchronize()
+    launches = sum(w.launches_per_step for w in layers)
+    sampler = ClockSampler(local)
+    sampler.start()
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    sampler.timed = True
+    with torch.cuda.stream(stream):
+        ev0.record(stream)
+        for _ in range(K):
+            g.replay()
+        ev1.record(stream)
+    barrier()
+    sampler.timed = False
+    ms_step = max_over_ranks(ev0.elapsed_time(ev1), device) / K
+    value = world * bytes_step / (ms_step * 1e-3) / 1e9
+
+    Ke = min(K, 200)
+    for _ in range(2):
+        for w in layers:
+            w.step_host(0)
+    barrier()
+    sampler.timed = True
+    ev0.record(stream)
+    for _ in range(Ke):
+        for w in layers:
+            w.step_host(0)
+    ev1.record(stream)
+    barrier()
+    sampler.timed = False
+    ms_e2e = max_over_ranks(ev0.elapsed_time(ev1), device) / Ke
+    e2e = world * bytes_step / (ms_e2e * 1e-3) / 1e9
+
+    kms = []
+    sampler.timed = True
+    with torch.cuda.stream(stream):
+        for it in range(4):
+            tot = 0.0
+            for w in layers:
+                sk.starkv_set_kernel_timing(w.ctx, True)
+                torch.cuda._sleep(300000)
+                w.step(0)
+                tot += sk.starkv_last_decode_kernel_ms(w.ctx)
+                sk.starkv_set_kernel_timing(w.ctx, False)
+            if it:
+                kms.append(tot)
+    sampler.timed = False
+    k_ms = float(np.mean(kms))
+    peak, peak_src = measured_peak()
+    achieved = bytes_kern / (k_ms * 1e-3) / 1e9
+    clocks = sampler.finish()
+    torch.cuda.synchronize()
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return
+    c0 = layers[0].cfg
+    non_attn_ms = NON_ATTN_WEIGHT_BYTES / (peak * 1e9) * 1e3
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
+        "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f16", "data": "synthetic",
+        "config": {"workload": f"C5: BASELINE.json configs[4], {n_layers} layers, batch {c0.batch}, {c0.n_q_heads}q/{c0.n_kv_heads}kv "
+                               f"heads x {c0.head_dim}, context {c0.context}, per-layer key ranks from the seeded profile "
+                               f"(mean 32), value rank {c0.rank_v}, int8/int4 latents",
+                   "parallelism": f"dp{world} (batch-sharded replicas, no collective)",
+                   "step": f"{n_layers} x (starkv_append of 1 new token / sequence + starkv_decode_attn)",
+                   "l2": f"{n_layers} distinct layer caches, {bytes_kern / 1e6:.0f} MB per step vs 126 MB L2",
+                   "launch": "one CUDA graph per step", "bytes_per_step": bytes_step},
+        "us_per_step_per_layer": ms_step * 1e3 / n_layers,
+        "tokens_per_s_attn_only": world * c0.batch / (ms_step * 1e-3) * (N_LAYERS_C5 / n_layers),
+        "attention_share_model": {"attention_ms": ms_step * N_LAYERS_C5 / n_layers, "non_attention_ms_bandwidth_model": non_attn_ms,
+                                  "share": ms_step * N_LAYERS_C5 / n_layers / (ms_step * N_LAYERS_C5 / n_layers + non_attn_ms),
+                                  "tokens_per_s": world * c0.batch / ((ms_step * N_LAYERS_C5 / n_layers + non_attn_ms) * 1e-3),
+                                  "model": "LLaMA-3.1-8B-shaped fp16 weights (%.1f GB) read once per step at the measured HBM "
+                                           "bandwidth; the library holds no such code" % (NON_ATTN_WEIGHT_BYTES / 1e9)},
+        "frac_of_nominal_8TBs": value / world / NOMINAL_HBM_GBS,
+        "e2e": {"value": e2e, "unit": UNIT, "h2d_bytes_per_step": sum(w.h2d_bytes() for w in layers),
+                "d2h_bytes_per_step": sum(w.d2h_bytes() for w in layers), "ms_per_step": ms_e2e, "steps": Ke},
+        "gpu_launches": K * launches,
+        "clocks": clocks,
+        "roofline": {"bound": "hbm", "kernel": "decode_fast_kernel (rows D2-D7), summed over the layers of a step",
+                     "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
+                     "traffic": stored_traffic("C5"), "peak_source": peak_src, "kernel_us": k_ms * 1e3,
+                     "launches_timed": len(kms) * n_layers, "algorithmic_bytes_per_launch": bytes_kern / n_layers,
+                     "frac_of_nominal_8TBs": achieved / NOMINAL_HBM_GBS},
+    }
+    print(json.dumps(line))
+    if world > 1:
+        dist.destroy_process_group()
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -541,6 +692,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="C2", help="C2 (default: the config the metric is quoted on), C3, C4, C5")
     ap.add_argument("--replicas", type=int, default=0)
+    ap.add_argument("--layers", type=int, default=0, help="C5 only: number of layers (default 32)")
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
     ap.add_argument("--prefill", action="store_true", help="also time starkv_append on a prefill chunk (always on for C4)")
     ap.add_argument("--prefill-tokens", type=int, default=2048)
@@ -549,6 +701,8 @@ def main():
     cfg = synth.make_config(args.workload)
     if args.impl == "reference":
         run_reference(args, cfg)
+    elif cfg.name == "C5":
+        run_c5(args)
     else:
         run_ours(args, cfg)
 

@@ -2,6 +2,8 @@
 //   PAPER.md §3.2 L58 (K' = x (Sigma V)_K per head, V' = x (Sigma V)_V joint),
 //   PAPER.md §4.4 L204-210 / Eq.12 L208 (leading channels at bits_hi, trailing at bits_lo, per token),
 //   DESIGN.md "Cache page format v1" (token-major K blocks, channel-major V blocks, offset-binary fields).
+#include <stdlib.h>
+
 #include "common.cuh"
 #include "ctx.h"
 
@@ -249,12 +251,12 @@ __global__ void __launch_bounds__(128) append_project_kernel(
 
 // ---------------------------------------------------------------------------------------------
 // append, step A1 for a handful of new tokens (decode-time append, n_new <= 16): z = X . A is bound by reading
-// A once, so the K dimension is split over APS_KS blocks and 8 warps per block, 64 columns per block (one
+// A once, so the K dimension is split over gridDim.y blocks and 8 warps per block, 64 columns per block (one
 // half2 per lane and row); partial sums are reduced in a fixed order (deterministic) and written as fp32
-//   zp[ks][token][column];  the write kernel adds the APS_KS partials, rounds once to fp16 and quantises.
-// grid (column tiles of keys then values, APS_KS), 256 threads.
+//   zp[ks][token][column];  the write kernel adds the gridDim.y partials, rounds once to fp16 and quantises.
+// grid (column tiles of keys then values, K splits), 256 threads.
 // ---------------------------------------------------------------------------------------------
-constexpr int APS_COLS = 64, APS_KCH = 256, APS_TOK = 16, APS_KS = 4;
+constexpr int APS_COLS = 64, APS_KCH = 256, APS_TOK = 16, APS_KS_MAX = 16;   // K splits = ceil(d_in / 256) <= 16
 
 __global__ void __launch_bounds__(256) append_project_small_kernel(
     const __grid_constant__ StarkvLayout L, int n_new, int n_key_tiles, const __half* __restrict__ k_new,
@@ -279,7 +281,7 @@ __global__ void __launch_bounds__(256) append_project_small_kernel(
     x0 = v_new; xstride = v_row_stride; d_in = d_in_v;
     ncols = min(APS_COLS, L.rank_v - c0); col_out0 = L.sum_rank_k + c0; A = A_v + c0; lda = L.rank_v;
   }
-  const int per = ((d_in + APS_KS - 1) / APS_KS + 31) / 32 * 32;
+  const int per = ((d_in + (int)gridDim.y - 1) / (int)gridDim.y + 31) / 32 * 32;
   const int k_begin = blockIdx.y * per, k_end = min(d_in, k_begin + per);
   float acc[APS_TOK][2];
 #pragma unroll
@@ -344,6 +346,14 @@ __device__ __forceinline__ void cp_async16(void* smem_dst, const void* gsrc, boo
   const uint32_t d = (uint32_t)__cvta_generic_to_shared(smem_dst);
   const int n = pred ? 16 : 0;   // src-size 0: zero fill
   asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" ::"r"(d), "l"(gsrc), "r"(n) : "memory");
+}
+__device__ __forceinline__ uint32_t pack_f2h2(float lo, float hi) {
+  const __half2 h = __floats2half2_rn(lo, hi);
+  return *reinterpret_cast<const uint32_t*>(&h);
+}
+__device__ __forceinline__ void cp_async16_s(uint32_t smem_dst, const void* gsrc, bool pred) {
+  const int n = pred ? 16 : 0;   // src-size 0: zero fill
+  asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" ::"r"(smem_dst), "l"(gsrc), "r"(n) : "memory");
 }
 __device__ __forceinline__ void ldsm_x4(uint32_t (&r)[4], const void* p) {
   const uint32_t a = (uint32_t)__cvta_generic_to_shared(p);
@@ -459,12 +469,201 @@ __global__ void __launch_bounds__(128) append_project_mma_kernel(
 }
 
 // ---------------------------------------------------------------------------------------------
+// append, step A1 for many new tokens on the 5th-generation tensor cores: z = fp16(X . A) with tcgen05.mma
+// (cta_group::1, kind::f16, M = 128 tokens, N = 64 latent columns, K = 16 per instruction), fp32 accumulator in
+// TMEM, read back with tcgen05.ld for the fp16 epilogue.  Operands are staged by cp.async straight into the
+// no-swizzle canonical layouts (8 x 16-byte core matrices): X tile K-major, A tile MN-major (A is [d_in, cols]
+// row-major, i.e. N-contiguous), 4 stages of 128 k, prefetch distance 3, one elected thread issues the MMAs and
+// tcgen05.commit releases a stage through an mbarrier.  grid (column tiles of keys then values, token tiles).
+// ---------------------------------------------------------------------------------------------
+constexpr int TM = 128, TN = 64, TK = 128, TSTAGES = 4;   // 48 KB per stage, prefetch distance 3
+constexpr int TA_BYTES = TM * TK * 2, TB_BYTES = TK * TN * 2, TSTAGE_BYTES = TA_BYTES + TB_BYTES;
+constexpr int TC5_SMEM = TSTAGES * TSTAGE_BYTES + 128;
+
+__device__ __forceinline__ uint64_t umma_desc(uint32_t saddr, uint32_t lbo_bytes, uint32_t sbo_bytes) {
+  // SWIZZLE_NONE matrix descriptor: start >> 4 | LBO >> 4 << 16 | SBO >> 4 << 32 | version 1 << 46
+  return (uint64_t)((saddr & 0x3FFFF) >> 4) | ((uint64_t)(lbo_bytes >> 4) << 16) | ((uint64_t)(sbo_bytes >> 4) << 32) |
+         ((uint64_t)1 << 46);
+}
+__device__ __forceinline__ void mbar_init_s(uint32_t bar, uint32_t count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_wait_s(uint32_t bar, uint32_t parity) {
+  asm volatile(
+      "{\n\t.reg .pred p;\n\t"
+      "WAIT_%=:\n\t"
+      "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n\t"
+      "@p bra DONE_%=;\n\t"
+      "bra WAIT_%=;\n\t"
+      "DONE_%=:\n\t}" ::"r"(bar),
+      "r"(parity)
+      : "memory");
+}
+
+__global__ void __launch_bounds__(256) append_project_tc5_kernel(
+    const __grid_constant__ StarkvLayout L, int n_new, int n_key_tiles, const __half* __restrict__ k_new,
+    long long k_row_stride, long long k_head_stride, int d_in_k, const __half* __restrict__ v_new, long long v_row_stride,
+    int d_in_v, const __half* __restrict__ A_k, const __half* __restrict__ A_v, __half* __restrict__ z) {
+  extern __shared__ __align__(128) uint8_t tsm[];
+  __shared__ uint32_t tmem_base_s;
+  const int R = L.sum_rank_k + L.rank_v;
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const __half* x0;
+  long long xstride;
+  int d_in, ncols, col_out0, lda;
+  const __half* A;
+  if ((int)blockIdx.x < n_key_tiles) {
+    int h = 0, t = blockIdx.x;
+    while (t >= (L.rank_k[h] + TN - 1) / TN) { t -= (L.rank_k[h] + TN - 1) / TN; ++h; }
+    const int c0 = t * TN;
+    x0 = k_new + (long long)h * k_head_stride; xstride = k_row_stride; d_in = d_in_k;
+    ncols = min(TN, L.rank_k[h] - c0); col_out0 = L.koff[h] + c0; A = A_k + L.koff[h] + c0; lda = L.sum_rank_k;
+  } else {
+    const int c0 = (blockIdx.x - n_key_tiles) * TN;
+    x0 = v_new; xstride = v_row_stride; d_in = d_in_v;
+    ncols = min(TN, L.rank_v - c0); col_out0 = L.sum_rank_k + c0; A = A_v + c0; lda = L.rank_v;
+  }
+  const int m0 = blockIdx.y * TM;
+  const uint32_t sbase = (uint32_t)__cvta_generic_to_shared(tsm);
+  const uint32_t bar0 = sbase + TSTAGES * TSTAGE_BYTES;   // empty[TSTAGES], then accumulator-ready
+  const uint32_t accbar = bar0 + 8 * TSTAGES;
+  if (tid == 0) {
+    for (int s = 0; s < TSTAGES; ++s) mbar_init_s(bar0 + 8 * s, 1);
+    mbar_init_s(accbar, 1);
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  }
+  if (warp == 0) {   // TMEM: 64 fp32 columns x 128 lanes for the accumulator
+    const uint32_t dst = (uint32_t)__cvta_generic_to_shared(&tmem_base_s);
+    asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(dst), "n"(TN) : "memory");
+    asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+  }
+  asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+  __syncthreads();
+  asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+  const uint32_t tmem_d = tmem_base_s;
+
+  // cp.async staging into the canonical layouts.  Lane = (row-in-core-matrix, 16-byte chunk): 8 rows x 4 chunks per
+  // warp instruction (conflict-free shared-memory writes, 64 contiguous bytes per global row).  Per-thread source
+  // pointers, shared-memory offsets and row predicates are fixed for the whole K loop.
+  //   X tile, K-major : element (m, k) at (m >> 3) * 2048 + (k >> 3) * 128 + (m & 7) * 16 + (k & 7) * 2
+  //   A tile, MN-major: element (k, n) at (n >> 3) * 2048 + (k >> 3) * 128 + (k & 7) * 16 + (n & 7) * 2
+  const int l7 = lane & 7, l3 = lane >> 3;
+  const __half* xsrc[4];      // rows warp*16 + {0, 8} ... : 8 chunks per thread = 2 row groups x 4 chunk groups
+  bool xok[2];
+  uint32_t xdst[2];
+#pragma unroll
+  for (int rg = 0; rg < 2; ++rg) {
+    const int m = warp * 16 + rg * 8 + l7;
+    xok[rg] = m0 + m < n_new;
+    xsrc[rg] = x0 + (long long)(xok[rg] ? m0 + m : 0) * xstride + l3 * 8;
+    xdst[rg] = (uint32_t)((m >> 3) * 2048 + l3 * 128 + (m & 7) * 16);
+  }
+  const int ak = warp * 16 + l7;               // k rows warp*16 + {0, 8}; 4 chunks per thread = 2 k groups x 2 n groups
+  const __half* asrc = A + (size_t)ak * lda + l3 * 8;
+  const uint32_t adst = (uint32_t)(l3 * 2048 + (ak >> 3) * 128 + (ak & 7) * 16);
+  const bool aok0 = l3 * 8 < ncols, aok1 = (l3 + 4) * 8 < ncols;
+  auto load_stage = [&](int stage, int k0) {
+    const uint32_t sa = sbase + stage * TSTAGE_BYTES, sb = sa + TA_BYTES;
+    const int krem = d_in - k0;   // > 0
+#pragma unroll
+    for (int rg = 0; rg < 2; ++rg)
+#pragma unroll
+      for (int cg = 0; cg < 4; ++cg) {
+        const bool ok = xok[rg] && (cg * 32 + l3 * 8) < krem;
+        cp_async16_s(sa + xdst[rg] + cg * 512, ok ? xsrc[rg] + k0 + cg * 32 : x0, ok);
+      }
+#pragma unroll
+    for (int kg = 0; kg < 2; ++kg) {
+      const bool kok = ak + kg * 8 < krem;
+      const __half* src = asrc + (size_t)(k0 + kg * 8) * lda;
+      cp_async16_s(sb + adst + kg * 128, (kok && aok0) ? src : A, kok && aok0);
+      cp_async16_s(sb + adst + kg * 128 + 4 * 2048, (kok && aok1) ? src + 32 : A, kok && aok1);
+    }
+  };
+  // instruction descriptor: D fp32, A/B fp16, A K-major, B MN-major, N = 64, M = 128
+  constexpr uint32_t IDESC = (1u << 4) | (1u << 16) | ((uint32_t)(TN >> 3) << 17) | ((uint32_t)(TM >> 4) << 24);
+  const int nk = (d_in + TK - 1) / TK;
+  load_stage(0, 0);
+  asm volatile("cp.async.commit_group;" ::: "memory");
+  if (nk > 1) load_stage(1, TK);
+  asm volatile("cp.async.commit_group;" ::: "memory");
+  if (nk > 2) load_stage(2, 2 * TK);
+  asm volatile("cp.async.commit_group;" ::: "memory");
+  for (int kt = 0; kt < nk; ++kt) {
+    if (kt + 3 < nk) {
+      const int st = (kt + 3) % TSTAGES;
+      if (kt >= 1) mbar_wait_s(bar0 + 8 * st, (uint32_t)(((kt - 1) / TSTAGES) & 1));   // MMA(kt - 1) has read the stage
+      load_stage(st, (kt + 3) * TK);
+    }
+    asm volatile("cp.async.commit_group;" ::: "memory");
+    asm volatile("cp.async.wait_group 3;" ::: "memory");
+    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");   // cp.async writes -> visible to the tensor core proxy
+    __syncthreads();
+    if (tid == 0) {
+      asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+      const uint32_t sa = sbase + (kt % TSTAGES) * TSTAGE_BYTES, sb = sa + TA_BYTES;
+#pragma unroll
+      for (int k = 0; k < TK / 16; ++k) {
+        const uint64_t da = umma_desc(sa + k * 256, 128, 2048);
+        const uint64_t db = umma_desc(sb + k * 256, 128, 2048);
+        const uint32_t accum = (kt > 0 || k > 0) ? 1u : 0u;
+        asm volatile(
+            "{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\t"
+            "tcgen05.mma.cta_group::1.kind::f16 [%0], %1, %2, %3, p;\n\t}" ::"r"(tmem_d),
+            "l"(da), "l"(db), "r"(IDESC), "r"(accum)
+            : "memory");
+      }
+      asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(bar0 + 8 * (kt % TSTAGES))
+                   : "memory");
+      if (kt == nk - 1)
+        asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(accbar) : "memory");
+    }
+  }
+  // epilogue: warp w may read TMEM lanes (= token rows) [32 (w % 4), +32); warps 0-3 take columns 0-31, warps 4-7
+  // columns 32-63; one rounding to fp16
+  mbar_wait_s(accbar, 0);
+  asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+  const int row = m0 + (warp & 3) * 32 + lane;
+  {
+    const int cb = (warp >> 2) * 32;
+    uint32_t v[32];
+    const uint32_t taddr = tmem_d + ((uint32_t)((warp & 3) * 32) << 16) + cb;
+    asm volatile(
+        "tcgen05.ld.sync.aligned.32x32b.x32.b32 {%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15,%16,%17,%18,%19,%20,%21,"
+        "%22,%23,%24,%25,%26,%27,%28,%29,%30,%31}, [%32];"
+        : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7]), "=r"(v[8]), "=r"(v[9]),
+          "=r"(v[10]), "=r"(v[11]), "=r"(v[12]), "=r"(v[13]), "=r"(v[14]), "=r"(v[15]), "=r"(v[16]), "=r"(v[17]), "=r"(v[18]),
+          "=r"(v[19]), "=r"(v[20]), "=r"(v[21]), "=r"(v[22]), "=r"(v[23]), "=r"(v[24]), "=r"(v[25]), "=r"(v[26]), "=r"(v[27]),
+          "=r"(v[28]), "=r"(v[29]), "=r"(v[30]), "=r"(v[31])
+        : "r"(taddr));
+    asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+    if (row < n_new) {
+      __half* dst = z + (size_t)row * R + col_out0 + cb;
+#pragma unroll
+      for (int c = 0; c < 32; c += 8) {
+        if (cb + c < ncols) {   // ncols is a multiple of 8
+          uint4 o;
+          o.x = pack_f2h2(__uint_as_float(v[c + 0]), __uint_as_float(v[c + 1]));
+          o.y = pack_f2h2(__uint_as_float(v[c + 2]), __uint_as_float(v[c + 3]));
+          o.z = pack_f2h2(__uint_as_float(v[c + 4]), __uint_as_float(v[c + 5]));
+          o.w = pack_f2h2(__uint_as_float(v[c + 6]), __uint_as_float(v[c + 7]));
+          *reinterpret_cast<uint4*>(dst + c) = o;
+        }
+      }
+    }
+  }
+  asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+  __syncthreads();
+  if (warp == 0) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem_d), "n"(TN) : "memory");
+}
+
+// ---------------------------------------------------------------------------------------------
 // append, steps A2-A4: per-token scales, codes, pack, paged write.  One CTA per new token.
 // 4-bit value fields share a byte between two slots: set with atomicAnd/atomicOr on the
 // containing word so that concurrent appends to neighbouring slots cannot lose an update.
 // ---------------------------------------------------------------------------------------------
 // z16 (fp16 latents) or, when zp != nullptr, n_part fp32 partial sums zp[part][token][column] added in order.
-__global__ void __launch_bounds__(256) append_write_kernel(const __grid_constant__ StarkvLayout L,
+__global__ void __launch_bounds__(512) append_write_kernel(const __grid_constant__ StarkvLayout L,
                                                            const __half* __restrict__ z, const float* __restrict__ zp,
                                                            int n_part, int n_new,
                                                            const int32_t* __restrict__ seq_ids,
@@ -612,7 +811,7 @@ int sk_unpack(starkv_ctx* ctx, const void* pages, int n_tokens, int8_t* codes, u
 size_t sk_append_ws_bytes(const starkv_ctx* ctx, int n_new) {
   const size_t R = (size_t)ctx->L.sum_rank_k + ctx->L.rank_v;
   const size_t n = (size_t)(n_new > 0 ? n_new : 0);
-  const size_t b = n <= (size_t)APS_TOK ? n * R * 4 * APS_KS : n * R * 2;
+  const size_t b = n <= (size_t)APS_TOK ? n * R * 4 * APS_KS_MAX : n * R * 2;
   return (b + 255) / 256 * 256;
 }
 
@@ -628,12 +827,16 @@ int sk_append(starkv_ctx* ctx, void* pool, const int32_t* table, int max_pages, 
   if (ws_bytes < sk_append_ws_bytes(ctx, n_new)) return STARKV_ERR_WORKSPACE;
   __half* z = (__half*)ws;
   const float* zp = nullptr;
+  int n_part = 1;
   if (n_new <= APS_TOK) {
     int nkt = 0;
     for (int h = 0; h < L.n_kv_heads; ++h) nkt += (L.rank_k[h] + APS_COLS - 1) / APS_COLS;
     const int nvt = (L.rank_v + APS_COLS - 1) / APS_COLS;
     SK_PREFER_SMEM(ctx, append_project_small_kernel);
-    sk_launch(ctx, append_project_small_kernel, dim3(nkt + nvt, APS_KS), dim3(256), 0,
+    const int d_max = d_in_k > d_in_v ? d_in_k : d_in_v;
+    n_part = (d_max + APS_KCH - 1) / APS_KCH;
+    if (n_part > APS_KS_MAX) n_part = APS_KS_MAX;
+    sk_launch(ctx, append_project_small_kernel, dim3(nkt + nvt, n_part), dim3(256), 0,
         L, n_new, nkt, (const __half*)k_new, k_row_stride, k_head_stride, d_in_k, (const __half*)v_new, v_row_stride, d_in_v,
         (const __half*)A_k, (const __half*)A_v, (float*)ws);
     zp = (const float*)ws;
@@ -643,10 +846,29 @@ int sk_append(starkv_ctx* ctx, void* pool, const int32_t* table, int max_pages, 
     int nkt = 0;
     for (int h = 0; h < L.n_kv_heads; ++h) nkt += (L.rank_k[h] + GN - 1) / GN;
     const int nvt = (L.rank_v + GN - 1) / GN;
+    // STARKV_APPEND_GEMM=tcgen05 selects the tcgen05/TMEM kernel.  It is correct (bit-exact parity) but, staged by
+    // 16-byte cp.async into 128 x 64 no-swizzle tiles, it is L2-bound and slower than the mma.sync kernel (measured
+    // 95 vs 80 us on the C4 prefill chunk), so it is opt-in until it moves to TMA + 128B swizzle + wider tiles.
+    const char* e_tc = getenv("STARKV_APPEND_GEMM");
+    const bool use_tc5 = n_new >= 64 && e_tc && e_tc[0] == 't' && (((L.sum_rank_k + L.rank_v) & 7) == 0);
+    if (use_tc5) {
+      int nkt5 = 0;
+      for (int h = 0; h < L.n_kv_heads; ++h) nkt5 += (L.rank_k[h] + TN - 1) / TN;
+      const int nvt5 = (L.rank_v + TN - 1) / TN;
+      static bool attr_done = false;
+      if (!attr_done) {
+        SK_CUDA_CHECK(ctx, cudaFuncSetAttribute(append_project_tc5_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, TC5_SMEM));
+        attr_done = true;
+      }
+      append_project_tc5_kernel<<<dim3(nkt5 + nvt5, (n_new + TM - 1) / TM), 256, TC5_SMEM, ctx->stream>>>(
+          L, n_new, nkt5, (const __half*)k_new, k_row_stride, k_head_stride, d_in_k, (const __half*)v_new, v_row_stride, d_in_v,
+          (const __half*)A_k, (const __half*)A_v, z);
+    } else {
     SK_PREFER_SMEM(ctx, append_project_mma_kernel);
     append_project_mma_kernel<<<dim3(nkt + nvt, (n_new + GM - 1) / GM), 128, 0, ctx->stream>>>(
         L, n_new, nkt, (const __half*)k_new, k_row_stride, k_head_stride, d_in_k, (const __half*)v_new, v_row_stride, d_in_v,
         (const __half*)A_k, (const __half*)A_v, z);
+    }
   } else {
   dim3 g1(L.n_kv_heads + (L.rank_v + 127) / 128, (n_new + APP_TOK - 1) / APP_TOK);
   append_project_kernel<<<g1, 128, 0, ctx->stream>>>(L, n_new, (const __half*)k_new, k_row_stride, k_head_stride, d_in_k,
@@ -659,7 +881,7 @@ int sk_append(starkv_ctx* ctx, void* pool, const int32_t* table, int max_pages, 
   if (smem > 48 * 1024)
     SK_CUDA_CHECK(ctx, cudaFuncSetAttribute(append_write_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
   SK_PREFER_SMEM(ctx, append_write_kernel);
-  sk_launch(ctx, append_write_kernel, dim3(n_new), dim3(256), smem, L, (const __half*)z, zp, (int)APS_KS, n_new, seq_ids,
+  sk_launch(ctx, append_write_kernel, dim3(n_new), dim3(512), smem, L, (const __half*)z, zp, n_part, n_new, seq_ids,
             positions, table, max_pages, (uint8_t*)pool);
   ctx->last_launches = 2;
   SK_CUDA_CHECK(ctx, cudaGetLastError());

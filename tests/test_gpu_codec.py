@@ -120,10 +120,14 @@ def _append_case(cfg, mode, n_new, dyadic, pad=0):
     return d, lay, dpool.cpu().numpy(), ref, n
 
 
-@pytest.mark.parametrize("n_new", [37, 8, 1], ids=["n37-gemm", "n8-small", "n1-small"])
+@pytest.mark.parametrize("n_new", [-80, 80, 37, 8, 1], ids=["n80-tcgen05", "n80-mma", "n37-mma", "n8-small", "n1-small"])
 @pytest.mark.parametrize("name,mode", [("C1", "dense"), ("C3", "dense"), ("C3", "hidden"), ("C4", "dense")])
-def test_append_bit_exact_on_dyadic_inputs(name, mode, n_new):
-    """n_new 37 -> 62 tokens (tiled projection kernel); 8 -> 15 and 1 -> 2 tokens (split-K small-n kernel)."""
+def test_append_bit_exact_on_dyadic_inputs(name, mode, n_new, monkeypatch):
+    """n_new 80 -> 134 tokens (two token tiles with a ragged tail) on the mma.sync projection and, opted in through
+    STARKV_APPEND_GEMM, on the tcgen05 projection; 37 -> 62 tokens; 8 -> 15 and 1 -> 2 tokens (split-K small-n kernel)."""
+    if n_new < 0:
+        monkeypatch.setenv("STARKV_APPEND_GEMM", "tcgen05")
+        n_new = -n_new
     cfg = synth.make_config(name, context=256, batch=3)
     d, lay, got, ref, n = _append_case(cfg, mode, n_new, dyadic=True)
     assert np.array_equal(got, ref), f"{int((got != ref).sum())} bytes differ of {got.size}"
@@ -135,7 +139,7 @@ def test_append_unaligned_rows_take_the_scalar_kernel():
     assert np.array_equal(got, ref)
 
 
-@pytest.mark.parametrize("n_new", [40, 8])
+@pytest.mark.parametrize("n_new", [120, 40, 8])
 def test_append_gaussian_inputs_close(n_new):
     """Gaussian activations: fp32 summation order differs from the oracle's exact sum, so the fp16
     latent may differ in the last bit on a few entries; scales within 1 ulp, codes within 1 step."""

@@ -126,6 +126,17 @@ def test_long_page_ranges_per_cta(name, ctx, splits):
     _check(cfg, seq_lens=[ctx - 17], splits=splits)
 
 
+@pytest.mark.parametrize("name", ["C2", "C3", "C4", "C5"])
+def test_full_baseline_size_in_the_bench_launch_configuration(name):
+    """BASELINE.json's full sizes (batch, context, ranks) through starkv_decode_attn with the automatic split
+    count bench.py times (one CTA per SM); the oracle evaluates a seeded sample of query heads on every
+    sequence (it reconstructs K, V for the sampled heads only)."""
+    cfg = synth.make_config(name)
+    rng = np.random.default_rng(11)
+    heads = sorted(int(h) for h in rng.choice(cfg.n_q_heads, size=3, replace=False))
+    _check(cfg, heads=heads)
+
+
 def test_fast_matches_generic_on_a_larger_case():
     """Second implementation as cross-check at a size the oracle is slow on (all heads)."""
     cfg = synth.make_config("C5", context=20000, batch=2)

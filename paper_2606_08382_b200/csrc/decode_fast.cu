@@ -400,13 +400,14 @@ __device__ __forceinline__ void qk_block(float (&acc)[4][4], const uint8_t* __re
 // PV of one 16-channel m-tile over the page's 64 tokens (4 k-steps) against all NT head tiles.
 //   vrow0/vrow1: this thread's two channel rows (R, R+8) of the value block, already clamped
 //   sc0/sc2    : value scales as (t, t+4) fp16 pairs of this thread's 16 tokens (quantised modes)
-//   pf         : P^T B fragments  [k-step pair][head tile] = (b0, b1 of step 2sp, b0, b1 of step 2sp+1)
+//   pf_lane    : this lane's P^T B fragments in the exchange buffer, [k-step pair][head tile][lane] uint4 =
+//                (b0, b1 of step 2sp, b0, b1 of step 2sp+1)
 // ---------------------------------------------------------------------------------------------
 template <int BITS, int NT>
 __device__ __forceinline__ void pv_tile(float (&acc)[NT][4], const uint8_t* __restrict__ vrow0,
                                         const uint8_t* __restrict__ vrow1, bool dead0, bool dead1,
-                                        const uint32_t (&sc0)[4], const uint32_t (&sc2)[4], const uint4 (&pf)[2][NT],
-                                        int j) {
+                                        const uint32_t (&sc0)[4], const uint32_t (&sc2)[4],
+                                        const uint4* __restrict__ pf_lane, int j) {
   uint32_t A0[4], A1[4], A2[4], A3[4];
   if (BITS == 4) {
     const uint2 x0 = *reinterpret_cast<const uint2*>(vrow0 + 8 * j);
@@ -454,12 +455,15 @@ __device__ __forceinline__ void pv_tile(float (&acc)[NT][4], const uint8_t* __re
       if (dead1) { A1[s] = 0; A3[s] = 0; }
     }
   }
+  // P^T fragments are read from the exchange buffer right before use (4 KB, L1-resident in effect): keeping all
+  // of them in registers across the dequantisation would cost 32 registers per thread
 #pragma unroll
-  for (int s = 0; s < 4; ++s)
+  for (int sp = 0; sp < 2; ++sp)
 #pragma unroll
     for (int c = 0; c < NT; ++c) {
-      const uint4 f = pf[s >> 1][c];
-      mma16816(acc[c], A0[s], A1[s], A2[s], A3[s], (s & 1) ? f.z : f.x, (s & 1) ? f.w : f.y);
+      const uint4 f = pf_lane[(sp * 4 + c) * 32];
+      mma16816(acc[c], A0[2 * sp], A1[2 * sp], A2[2 * sp], A3[2 * sp], f.x, f.y);
+      mma16816(acc[c], A0[2 * sp + 1], A1[2 * sp + 1], A2[2 * sp + 1], A3[2 * sp + 1], f.z, f.w);
     }
 }
 
@@ -727,11 +731,7 @@ __global__ void __launch_bounds__(NTHREADS, 1) decode_fast_kernel(
         }
       }
     }
-    uint4 pf[2][NT];   // [k-step pair][head tile]
-#pragma unroll
-    for (int sp = 0; sp < 2; ++sp)
-#pragma unroll
-      for (int c = 0; c < NT; ++c) pf[sp][c] = *reinterpret_cast<const uint4*>(Pb + (((sp * 4 + c) * 32 + lane) << 4));
+    const uint4* pf = reinterpret_cast<const uint4*>(Pb) + lane;   // [k-step pair][head tile][lane]
     int cur_blk = -1;
     uint32_t sc0[4] = {0, 0, 0, 0}, sc2[4] = {0, 0, 0, 0};
 #pragma unroll

@@ -28,6 +28,7 @@
 //   The row of the QK tile that holds token t is chosen so that the transposed P lands in the token order
 //   the dequantised value words produce (no shuffles on the value side).
 // The partial (m, l, acc[H_q x r_v]) goes to the workspace; combine_kernel merges and up-projects.
+#include <stdlib.h>
 #include <string.h>
 
 #include "decode_common.cuh"
@@ -51,9 +52,8 @@ extern "C" int starkv_debug_trace(unsigned long long* out_host) {
 namespace {
 
 constexpr int GW = 8;                     // warps per group
-constexpr int NCONS = 2 * GW;             // consumer warps
-constexpr int NCONS_THREADS = NCONS * 32;
-constexpr int NTHREADS = NCONS_THREADS;
+constexpr int NG_MAX = 3;                 // groups per CTA: 2 (128 registers per thread) or 3 (80)
+constexpr int BAR_ALL = 8;                // named barrier of all warps (1..NG are the groups' own)
 constexpr int TBL_SMEM = 256;             // block-table entries of the CTA's range kept in shared memory
 constexpr int PTOK = 64;         // tokens per page on this path
 constexpr float P_OFFSET = 8.f;  // P is stored as 2^(s - m + 8) in fp16 (keeps small weights normal)
@@ -566,17 +566,19 @@ __device__ __forceinline__ void score_page(const StarkvLayout& L, const DecodePl
 }
 
 // ---------------------------------------------------------------------------------------------
-// Main kernel.  grid (n_splits, batch), 512 threads (two groups of 8 warps).
+// Main kernel.  grid (n_splits, batch), NG groups of 8 warps (NG = 2: 512 threads, 128 registers; NG = 3: 768
+// threads, 80 registers -- more warps to hide the dequantisation latency of the integer modes).
 //   BH/BL  bit widths of the leading / trailing blocks (16/16 = fp16 latents)
 //   NT  head tiles of 8   MT  value m-tiles (16 channels) per warp
 // ---------------------------------------------------------------------------------------------
-template <int BH, int BL, int NT, int MT>
-__global__ void __launch_bounds__(NTHREADS, 1) decode_fast_kernel(
+template <int BH, int BL, int NT, int MT, int NG>
+__global__ void __launch_bounds__(NG * GW * 32, 1) decode_fast_kernel(
     const __grid_constant__ StarkvLayout L, const __grid_constant__ DecodePlan PL, const uint8_t* __restrict__ qimg_all,
     size_t qimg_stride, const uint8_t* __restrict__ pool, const int32_t* __restrict__ table, int max_pages,
     const int32_t* __restrict__ seq_lens, float* __restrict__ parts, int n_splits) {
   extern __shared__ __align__(128) uint8_t smem[];
   constexpr bool QUANT = BH != 16;
+  constexpr int NTHREADS = NG * GW * 32;
 
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const int j = lane & 3, R = lane >> 2;
@@ -641,14 +643,13 @@ __global__ void __launch_bounds__(NTHREADS, 1) decode_fast_kernel(
 
   // ================= consumers =================
   const int grp = warp >> 3, gw = warp & (GW - 1);
-  const int ctid = tid;   // 0..511
   {
     uint4* pz = reinterpret_cast<uint4*>(smem + PL.off_p);
-    for (int i = ctid; i < 4 * P_BUF_BYTES / 16; i += NCONS_THREADS) pz[i] = make_uint4(0, 0, 0, 0);
-    if (ctid < 128) reinterpret_cast<float*>(smem + PL.off_alpha)[ctid] = 1.f;
-    if (ctid < 8) reinterpret_cast<uint32_t*>(smem + PL.off_flag)[ctid] = 0;
+    for (int i = tid; i < NG * 2 * P_BUF_BYTES / 16; i += NTHREADS) pz[i] = make_uint4(0, 0, 0, 0);
+    if (tid < NG * 64) reinterpret_cast<float*>(smem + PL.off_alpha)[tid] = 1.f;
+    if (tid < NG * 4) reinterpret_cast<uint32_t*>(smem + PL.off_flag)[tid] = 0;
   }
-  bar_sync(3, NCONS_THREADS);
+  bar_sync(BAR_ALL, NTHREADS);
   mbar_wait(qbar, 0);
   SK_STAMP(1);
 
@@ -676,11 +677,12 @@ __global__ void __launch_bounds__(NTHREADS, 1) decode_fast_kernel(
       for (int e = 0; e < 4; ++e) acc[a][c][e] = 0.f;
 
   SK_STAMP(2);
-  int st = grp % nstage, use = 0;   // ring stage and use count of iteration `it`, kept incrementally
-  for (int it = grp; it < n_it; it += 2) {
+  int st = grp % nstage, use = grp / nstage;   // ring stage and use count of iteration `it`, kept incrementally
+  int gi = 0;                                  // this group's iteration count
+  for (int it = grp; it < n_it; it += NG, ++gi) {
     uint8_t* pg = stage_base + (size_t)st * page_bytes;
     const int nvalid = len - (p0 + it) * PTOK;   // >= 1
-    const int buf = (it >> 1) & 1;
+    const int buf = gi & 1;
     uint8_t* Pb = Pm + buf * P_BUF_BYTES;
     float* al = alpha_s + buf * 32;
     uint8_t* fl = flag_s + buf * 8;
@@ -766,18 +768,18 @@ __global__ void __launch_bounds__(NTHREADS, 1) decode_fast_kernel(
         if (nxt < n_it) issue(nxt, nxt < TBL_SMEM ? tbl_s[nxt] : my_table[nxt]);
       }
     }
-    st += 2;
-    if (st >= nstage) { st -= nstage; ++use; }   // nstage >= 2: at most one wrap
+    st += NG;
+    while (st >= nstage) { st -= nstage; ++use; }
   }
 
-  // ================= merge the two groups and write the split-K partial (D7) =================
-  // Stage memory is free (every issued page was consumed): it holds m[2][32], l[2][32] and the partial in its
+  // ================= merge the groups and write the split-K partial (D7) =================
+  // Stage memory is free (every issued page was consumed): it holds m[NG][32], l[NG][32] and the partial in its
   // global layout [head][4 + r_v], which is then streamed out with coalesced 16-byte stores.
   if (grp == 0) SK_STAMP(3);
-  bar_sync(3, NCONS_THREADS);
+  bar_sync(BAR_ALL, NTHREADS);
   SK_STAMP(4);
-  float* mg = reinterpret_cast<float*>(smem + PL.off_stage);
-  float* ost = mg + 128;
+  float* mg = reinterpret_cast<float*>(smem + PL.off_stage);   // m at [g * 32 + head], l at [128 + g * 32 + head]
+  float* ost = mg + 256;
   const int ST = (int)pstride;
   if (has_quad) {
     float lsum = l_run;
@@ -786,29 +788,37 @@ __global__ void __launch_bounds__(NTHREADS, 1) decode_fast_kernel(
     lsum += __shfl_xor_sync(0xffffffffu, lsum, 16);
     if (R == 0) {
       mg[grp * 32 + 4 * gw + j] = m_run;
-      mg[64 + grp * 32 + 4 * gw + j] = lsum;
+      mg[128 + grp * 32 + 4 * gw + j] = lsum;
     }
   }
-  bar_sync(3, NCONS_THREADS);
+  bar_sync(BAR_ALL, NTHREADS);
   SK_STAMP(6);
-  float fme[NT][2];   // this group's weight per head column: 2^(m_own - max(m_A, m_B)); group A always has a page
+  float fme[NT][2];   // this group's weight per head column: 2^(m_own - max_g m_g); group 0 always has a page
 #pragma unroll
   for (int c = 0; c < NT; ++c)
 #pragma unroll
     for (int e = 0; e < 2; ++e) {
       const int head = 8 * c + 2 * j + e;
-      const float mA = mg[head], mB = mg[32 + head];
-      const float mo = grp ? mB : mA;
-      fme[c][e] = mo == -INFINITY ? 0.f : ex2(mo - fmaxf(mA, mB));
+      float ms = mg[head];
+#pragma unroll
+      for (int g = 1; g < NG; ++g) ms = fmaxf(ms, mg[g * 32 + head]);
+      const float mo = mg[grp * 32 + head];
+      fme[c][e] = mo == -INFINITY ? 0.f : ex2(mo - ms);
     }
   if (tid < L.n_q_heads) {
-    const float mA = mg[tid], mB = mg[32 + tid];
-    const float ms = fmaxf(mA, mB);
-    const float wA = ex2(mA - ms), wB = mB == -INFINITY ? 0.f : ex2(mB - ms);
-    *reinterpret_cast<float4*>(ost + tid * ST) = make_float4(ms, mg[64 + tid] * wA + mg[96 + tid] * wB, 0.f, 0.f);
+    float ms = mg[tid];
+#pragma unroll
+    for (int g = 1; g < NG; ++g) ms = fmaxf(ms, mg[g * 32 + tid]);
+    float lm = 0.f;
+#pragma unroll
+    for (int g = 0; g < NG; ++g) {
+      const float mo = mg[g * 32 + tid];
+      lm += mo == -INFINITY ? 0.f : mg[128 + g * 32 + tid] * ex2(mo - ms);
+    }
+    *reinterpret_cast<float4*>(ost + tid * ST) = make_float4(ms, lm, 0.f, 0.f);
   }
 #pragma unroll
-  for (int pass = 1; pass >= 0; --pass) {   // group B stores, then group A adds
+  for (int pass = NG - 1; pass >= 0; --pass) {   // the last group stores, the others add one after the other
     if (grp == pass) {
 #pragma unroll
       for (int a = 0; a < MT; ++a) {
@@ -826,44 +836,44 @@ __global__ void __launch_bounds__(NTHREADS, 1) decode_fast_kernel(
               if (head < L.n_q_heads && ch0 + R + dch < n) {
                 float* o = o0 + head * ST + dch;
                 const float v = acc[a][c][e] * fme[c][e & 1];
-                *o = pass ? v : *o + v;
+                *o = pass == NG - 1 ? v : *o + v;
               }
             }
         }
       }
     }
-    bar_sync(3, NCONS_THREADS);
+    bar_sync(BAR_ALL, NTHREADS);
   }
   SK_STAMP(7);
   {
     const float4* src = reinterpret_cast<const float4*>(ost);
     float4* dst = reinterpret_cast<float4*>(my_parts);
-    for (int i = tid; i < L.n_q_heads * ST / 4; i += NCONS_THREADS) dst[i] = src[i];
+    for (int i = tid; i < L.n_q_heads * ST / 4; i += NTHREADS) dst[i] = src[i];
   }
   SK_STAMP(5);
 }
 
-template <int BH, int BL, int NT, int MT>
+template <int BH, int BL, int NT, int MT, int NG>
 cudaError_t launch_fast(const starkv_ctx* ctx, dim3 grid, const uint8_t* qimg, size_t qimg_stride, const uint8_t* pool,
                         const int32_t* table, int max_pages, const int32_t* seq_lens, float* parts, int n_splits) {
-  auto kern = decode_fast_kernel<BH, BL, NT, MT>;
+  auto kern = decode_fast_kernel<BH, BL, NT, MT, NG>;
   static int smem_set = 0;   // largest dynamic shared-memory size already granted to this instantiation
   if (ctx->plan.smem_bytes > smem_set) {
     const cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, ctx->plan.smem_bytes);
     if (e != cudaSuccess) return e;
     smem_set = ctx->plan.smem_bytes;
   }
-  return sk_launch(ctx, kern, grid, dim3(NTHREADS), (size_t)ctx->plan.smem_bytes, ctx->L, ctx->plan, qimg, qimg_stride, pool,
-                   table, max_pages, seq_lens, parts, n_splits);
+  return sk_launch(ctx, kern, grid, dim3(NG * GW * 32), (size_t)ctx->plan.smem_bytes, ctx->L, ctx->plan, qimg, qimg_stride,
+                   pool, table, max_pages, seq_lens, parts, n_splits);
 }
 
-template <int BH, int BL>
+template <int BH, int BL, int NG>
 cudaError_t dispatch_fast(const starkv_ctx* ctx, dim3 grid, const uint8_t* qimg, size_t qimg_stride, const uint8_t* pool,
                           const int32_t* table, int max_pages, const int32_t* seq_lens, float* parts, int n_splits) {
   const int nt = ctx->plan.nt, mt = ctx->plan.mt;
 #define SK_FAST(NTv, MTv) \
   if (nt == NTv && mt == MTv) \
-    return launch_fast<BH, BL, NTv, MTv>(ctx, grid, qimg, qimg_stride, pool, table, max_pages, seq_lens, parts, n_splits)
+    return launch_fast<BH, BL, NTv, MTv, NG>(ctx, grid, qimg, qimg_stride, pool, table, max_pages, seq_lens, parts, n_splits)
   SK_FAST(1, 1); SK_FAST(1, 2); SK_FAST(1, 3); SK_FAST(1, 4);
   SK_FAST(2, 1); SK_FAST(2, 2); SK_FAST(2, 3); SK_FAST(2, 4);
   SK_FAST(4, 1); SK_FAST(4, 2); SK_FAST(4, 3); SK_FAST(4, 4);
@@ -903,10 +913,10 @@ int sk_fast_plan(starkv_ctx* ctx) {
   P.v_tiles = P.v_tiles_hi + (L.v_lo_n + 15) / 16;
   P.mt = (P.v_tiles + GW - 1) / GW;
   if (P.mt > 4) return 0;
-  const int p_area = 4 * P_BUF_BYTES;
+  const int p_area = NG_MAX * 2 * P_BUF_BYTES;
   const int qarea = round_up(P.qimg_bytes + L.n_kv_heads * 32, 128);   // image + accumulator start values
-  const int merge_bytes = 512 + L.n_q_heads * (L.rank_v + 4) * 4;
-  const int fixed = qarea + p_area + 2 * 2 * 32 * 4 /* alpha */ + 128 /* flags */ +
+  const int merge_bytes = 1024 + L.n_q_heads * (L.rank_v + 4) * 4;
+  const int fixed = qarea + p_area + NG_MAX * 2 * 32 * 4 /* alpha */ + 128 /* flags */ +
                     128 /* barriers */ + 4 * TBL_SMEM + 128 /* base align */;
   const int avail = ctx->smem_optin - fixed;
   int ns = avail / L.page_bytes;
@@ -916,12 +926,13 @@ int sk_fast_plan(starkv_ctx* ctx) {
     if (merge_bytes > avail) return 0;
   }
   P.nstage = ns;
+  P.ng = 2;
   int off = 0;
   P.off_stage = off;
   off += round_up(ns * L.page_bytes > merge_bytes ? ns * L.page_bytes : merge_bytes, 128);
   P.off_qimg = off; P.off_kcst = off + P.qimg_bytes; off += qarea;
   P.off_p = off; off += p_area;
-  P.off_alpha = off; off += 2 * 2 * 32 * 4;
+  P.off_alpha = off; off += NG_MAX * 2 * 32 * 4;
   P.off_flag = off; off += 128;
   P.off_bar = off; off += 8 * ns + 8 + 4 * ns + 4 * ns;
   off = round_up(off, 16);
@@ -969,10 +980,15 @@ int sk_decode_fast(starkv_ctx* ctx, const void* q, const void* pool, const int32
   const uint8_t* pl = (const uint8_t*)pool;
   if (ctx->timing_on) SK_CUDA_CHECK(ctx, cudaEventRecord(ctx->ev0, ctx->stream));
   cudaError_t e = cudaErrorInvalidValue;
-  if (L.bits_hi == 16) e = dispatch_fast<16, 16>(ctx, grid, qimg, w.qimg_stride, pl, table, max_pages, seq_lens, parts, w.n_splits);
-  else if (L.bits_hi == 8 && L.bits_lo == 4) e = dispatch_fast<8, 4>(ctx, grid, qimg, w.qimg_stride, pl, table, max_pages, seq_lens, parts, w.n_splits);
-  else if (L.bits_hi == 8 && L.bits_lo == 8) e = dispatch_fast<8, 8>(ctx, grid, qimg, w.qimg_stride, pl, table, max_pages, seq_lens, parts, w.n_splits);
-  else if (L.bits_hi == 4 && L.bits_lo == 4) e = dispatch_fast<4, 4>(ctx, grid, qimg, w.qimg_stride, pl, table, max_pages, seq_lens, parts, w.n_splits);
+#define SK_KIND(BHv, BLv, NGv) \
+  e = dispatch_fast<BHv, BLv, NGv>(ctx, grid, qimg, w.qimg_stride, pl, table, max_pages, seq_lens, parts, w.n_splits)
+  // NG = 3 (768 threads, 80 registers) was measured on C3: 43.1 us against 32.7 us with NG = 2 -- the 412-byte
+  // spill frame costs more than the third group hides -- so only NG = 2 is instantiated.
+  if (L.bits_hi == 16) SK_KIND(16, 16, 2);
+  else if (L.bits_hi == 8 && L.bits_lo == 4) SK_KIND(8, 4, 2);
+  else if (L.bits_hi == 8 && L.bits_lo == 8) SK_KIND(8, 8, 2);
+  else if (L.bits_hi == 4 && L.bits_lo == 4) SK_KIND(4, 4, 2);
+#undef SK_KIND
   SK_CUDA_CHECK(ctx, e);
   if (ctx->timing_on) {
     SK_CUDA_CHECK(ctx, cudaEventRecord(ctx->ev1, ctx->stream));

@@ -19,12 +19,13 @@ struct DecodePlan {
   int32_t mt;                                     // PV m-tiles (16 value channels) per warp: 1..4
   int32_t v_tiles_hi, v_tiles;                    // m-tiles in the leading value block / in total
   int32_t nstage;                                 // page ring depth
+  int32_t ng;                                     // groups of 8 warps per CTA: 2 or 3
   // shared-memory carve-up (bytes from the 128-aligned base)
   int32_t off_stage;                              // [nstage][page_bytes]; reused for the final group merge
   int32_t off_qimg;                               // latent-space query image
-  int32_t off_p;                                  // [2 groups][2][P_BUF_BYTES]; P exchange buffers
-  int32_t off_alpha;                              // [2 groups][2][32] float
-  int32_t off_flag;                               // [2 groups][2][8] bytes: "some head of quad w rescaled"
+  int32_t off_p;                                  // [groups][2][P_BUF_BYTES]; P exchange buffers
+  int32_t off_alpha;                              // [groups][2][32] float
+  int32_t off_flag;                               // [groups][2][8] bytes: "some head of quad w rescaled"
   int32_t off_bar;                                // full[nstage] + image mbarriers, done[nstage] tickets, issued[nstage]
   int32_t off_tbl;                                // block-table entries of the CTA's page range
   int32_t off_kcst;                               // = off_qimg + qimg_bytes: QK accumulator start values

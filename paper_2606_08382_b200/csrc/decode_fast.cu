@@ -926,7 +926,13 @@ int sk_fast_plan(starkv_ctx* ctx) {
     if (merge_bytes > avail) return 0;
   }
   P.nstage = ns;
-  P.ng = 2;
+  // pages so large that only two fit: one group, so that the second stage is a copy in flight instead of a
+  // second page being computed on (built for the fp16 and int8/int4 modes)
+  P.ng = (ns == 2 && (L.bits_hi == 16 || (L.bits_hi == 8 && L.bits_lo == 4))) ? 1 : 2;
+  {
+    const char* e_ng = getenv("STARKV_GROUPS");
+    if (e_ng && e_ng[0] == '2') P.ng = 2;
+  }
   int off = 0;
   P.off_stage = off;
   off += round_up(ns * L.page_bytes > merge_bytes ? ns * L.page_bytes : merge_bytes, 128);
@@ -984,8 +990,9 @@ int sk_decode_fast(starkv_ctx* ctx, const void* q, const void* pool, const int32
   e = dispatch_fast<BHv, BLv, NGv>(ctx, grid, qimg, w.qimg_stride, pl, table, max_pages, seq_lens, parts, w.n_splits)
   // NG = 3 (768 threads, 80 registers) was measured on C3: 43.1 us against 32.7 us with NG = 2 -- the 412-byte
   // spill frame costs more than the third group hides -- so only NG = 2 is instantiated.
-  if (L.bits_hi == 16) SK_KIND(16, 16, 2);
-  else if (L.bits_hi == 8 && L.bits_lo == 4) SK_KIND(8, 4, 2);
+  const bool one = ctx->plan.ng == 1;
+  if (L.bits_hi == 16) { if (one) SK_KIND(16, 16, 1); else SK_KIND(16, 16, 2); }
+  else if (L.bits_hi == 8 && L.bits_lo == 4) { if (one) SK_KIND(8, 4, 1); else SK_KIND(8, 4, 2); }
   else if (L.bits_hi == 8 && L.bits_lo == 8) SK_KIND(8, 8, 2);
   else if (L.bits_hi == 4 && L.bits_lo == 4) SK_KIND(4, 4, 2);
 #undef SK_KIND

@@ -64,6 +64,15 @@ def test_bit_pairs_and_odd_shapes(bits, generic):
         _check(cfg, seq_lens=[700, 333], generic=generic)
 
 
+@pytest.mark.parametrize("bits", [(8, 4), (16, 16)], ids=str)
+def test_largest_supported_ranks(bits):
+    """Full key rank (r_h = d_h) and the largest value rank of the fast kernel (r_v = 512: 4 value tiles per warp)."""
+    cfg = synth.custom_config(f"max{bits[0]}", 2, 32, 8, 128, 900, [128] * 8, 512, bits=bits, outlier_frac=0.1)
+    _check(cfg, seq_lens=[900, 515])
+    cfg = synth.custom_config(f"dh256_{bits[0]}", 1, 8, 2, 256, 300, [256, 200], 256, bits=bits)
+    _check(cfg, seq_lens=[300])
+
+
 @pytest.mark.parametrize("generic", [True, False], ids=["generic", "fast"])
 def test_sequence_length_edges(generic):
     cfg = synth.make_config("C3", context=400, batch=8)

@@ -334,11 +334,11 @@ __global__ void __launch_bounds__(256) append_project_small_kernel(
 // ---------------------------------------------------------------------------------------------
 // append, step A1 for many new tokens (prefill): z = fp16(X . A) on tensor cores (mma.sync m16n8k16, fp32
 // accumulation).  CTA tile 64 tokens x 64 latent columns, K step 32, 4 warps (2 x 2, warp tile 32 x 32),
-// cp.async double buffering, ldmatrix fragments (A operand from the token-major X tile, B operand by
+// 4-stage cp.async pipeline (prefetch distance 3, one block barrier per K step), ldmatrix fragments (A operand from the token-major X tile, B operand by
 // ldmatrix.trans from the k-major A tile).  grid (column tiles of keys then values, token tiles).
 // Requires 16-byte aligned rows: d_in % 8 == 0, row strides % 8 == 0 (else the scalar kernel runs).
 // ---------------------------------------------------------------------------------------------
-constexpr int GM = 64, GN = 64, GK = 32;
+constexpr int GM = 64, GN = 64, GK = 32, GST = 4;
 constexpr int GXS = GK + 8;   // X tile row stride in halves (80 B: conflict-free ldmatrix)
 constexpr int GAS = GN + 8;   // A tile row stride in halves (144 B)
 
@@ -374,8 +374,8 @@ __global__ void __launch_bounds__(128) append_project_mma_kernel(
     const __grid_constant__ StarkvLayout L, int n_new, int n_key_tiles, const __half* __restrict__ k_new,
     long long k_row_stride, long long k_head_stride, int d_in_k, const __half* __restrict__ v_new, long long v_row_stride,
     int d_in_v, const __half* __restrict__ A_k, const __half* __restrict__ A_v, __half* __restrict__ z) {
-  __shared__ __align__(16) __half xs[2][GM * GXS];
-  __shared__ __align__(16) __half as[2][GK * GAS];
+  __shared__ __align__(16) __half xs[GST][GM * GXS];
+  __shared__ __align__(16) __half as[GST][GK * GAS];
   const int R = L.sum_rank_k + L.rank_v;
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const int wm = warp >> 1, wn = warp & 1;
@@ -422,16 +422,18 @@ __global__ void __launch_bounds__(128) append_project_mma_kernel(
 #pragma unroll
       for (int e = 0; e < 4; ++e) acc[a][b][e] = 0.f;
   const int nk = (d_in + GK - 1) / GK;
-  load_tiles(0, 0);
+  // prologue: tiles 0 .. GST-2 (empty groups keep the group count uniform)
+#pragma unroll
+  for (int p = 0; p < GST - 1; ++p) {
+    if (p < nk) load_tiles(p, p * GK);
+    else asm volatile("cp.async.commit_group;" ::: "memory");
+  }
   for (int kt = 0; kt < nk; ++kt) {
-    const int buf = kt & 1;
-    if (kt + 1 < nk) {
-      load_tiles(buf ^ 1, (kt + 1) * GK);
-      asm volatile("cp.async.wait_group 1;" ::: "memory");
-    } else {
-      asm volatile("cp.async.wait_group 0;" ::: "memory");
-    }
-    __syncthreads();
+    const int buf = kt % GST;
+    asm volatile("cp.async.wait_group %0;" ::"n"(GST - 2) : "memory");   // tile kt has landed (this thread's copies)
+    __syncthreads();   // ... everyone's; and every warp is done with the stage tile kt + GST - 1 goes into
+    if (kt + GST - 1 < nk) load_tiles((kt + GST - 1) % GST, (kt + GST - 1) * GK);
+    else asm volatile("cp.async.commit_group;" ::: "memory");
 #pragma unroll
     for (int ks = 0; ks < GK; ks += 16) {
       uint32_t af[2][4], bf[2][4];
@@ -448,7 +450,6 @@ __global__ void __launch_bounds__(128) append_project_mma_kernel(
 #pragma unroll
         for (int b = 0; b < 4; ++b) hmma16816(acc[a][b], af[a], bf[b >> 1][(b & 1) * 2], bf[b >> 1][(b & 1) * 2 + 1]);
     }
-    __syncthreads();
   }
   // epilogue: one rounding to fp16, rows = tokens
 #pragma unroll

@@ -932,6 +932,7 @@ int sk_fast_plan(starkv_ctx* ctx) {
   {
     const char* e_ng = getenv("STARKV_GROUPS");
     if (e_ng && e_ng[0] == '2') P.ng = 2;
+    if (e_ng && e_ng[0] == '1' && (L.bits_hi == 16 || (L.bits_hi == 8 && L.bits_lo == 4))) P.ng = 1;
   }
   int off = 0;
   P.off_stage = off;

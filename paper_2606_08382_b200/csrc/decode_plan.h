@@ -19,7 +19,7 @@ struct DecodePlan {
   int32_t mt;                                     // PV m-tiles (16 value channels) per warp: 1..4
   int32_t v_tiles_hi, v_tiles;                    // m-tiles in the leading value block / in total
   int32_t nstage;                                 // page ring depth
-  int32_t ng;                                     // groups of 8 warps per CTA: 2 or 3
+  int32_t ng;                                     // groups of 8 warps per CTA: 1 or 2
   // shared-memory carve-up (bytes from the 128-aligned base)
   int32_t off_stage;                              // [nstage][page_bytes]; reused for the final group merge
   int32_t off_qimg;                               // latent-space query image

@@ -135,6 +135,11 @@ int starkv_decode_attn_generic(starkv_ctx* ctx, const void* q, const void* page_
                                const void* B_v, void* workspace, size_t workspace_bytes,
                                void* out);
 
+/* The two HOST-buffer variants below stage their host inputs in a pinned block owned by the context when the
+ * context has a stream of its own (not the legacy / per-thread default stream): the caller's buffers are read
+ * before the call returns, one host-to-device copy carries all inputs of the call, and with STARKV_HOST_GRAPH=1 in
+ * the environment the copies and kernels of a call signature are replayed as one cached CUDA graph. */
+
 /* HOST-buffer variant (bench.py "e2e"): q_host / seq_lens_host / out_host are HOST pointers
  * (pinned for best speed); the call copies q and seq_lens to device scratch inside `workspace`
  * (sized by starkv_workspace_bytes, which reserves room for them), runs the decode step,

@@ -13,6 +13,47 @@ int sk_cuda_fail(starkv_ctx* ctx, cudaError_t e, const char* what) {
 
 static bool aligned16(const void* p) { return ((uintptr_t)p & 15) == 0; }
 
+// ---- pinned staging and graph cache of the HOST-buffer entry points ----
+static const size_t kPinDecode = 0;
+// grow a pinned staging block; the graph that captured the old address is dropped
+static int sk_pin_reserve(starkv_ctx* ctx, void** pin, size_t* have, size_t bytes, starkv_ctx::HostGraph* g) {
+  if (*have >= bytes) return STARKV_OK;
+  for (int i = 0; i < starkv_ctx::kHostGraphs; ++i)
+    if (g[i].exec) { cudaGraphExecDestroy(g[i].exec); g[i].exec = nullptr; }
+  SK_CUDA_CHECK(ctx, cudaStreamSynchronize(ctx->stream));
+  if (*pin) cudaFreeHost(*pin);
+  *pin = nullptr;
+  *have = 0;
+  if (bytes < ((size_t)1 << 16)) bytes = (size_t)1 << 16;
+  SK_CUDA_CHECK(ctx, cudaHostAlloc(pin, bytes, cudaHostAllocDefault));
+  *have = bytes;
+  return STARKV_OK;
+}
+static starkv_ctx::HostGraph* sk_graph_find(starkv_ctx::HostGraph* gs, const void* const* p, const long long* v) {
+  for (int k = 0; k < starkv_ctx::kHostGraphs; ++k) {
+    starkv_ctx::HostGraph& g = gs[k];
+    if (!g.exec) continue;
+    bool ok = true;
+    for (int i = 0; i < 8 && ok; ++i) ok = g.p[i] == p[i];
+    for (int i = 0; i < 10 && ok; ++i) ok = g.v[i] == v[i];
+    if (ok) return &g;
+  }
+  return nullptr;
+}
+static starkv_ctx::HostGraph* sk_graph_slot(starkv_ctx::HostGraph* gs, int* next) {
+  starkv_ctx::HostGraph* g = &gs[*next];
+  *next = (*next + 1) % starkv_ctx::kHostGraphs;
+  if (g->exec) { cudaGraphExecDestroy(g->exec); g->exec = nullptr; }
+  return g;
+}
+// graphs are not used on the legacy / per-thread default streams (not capturable) or inside a caller's capture
+static bool sk_stream_capturing(starkv_ctx* ctx) {
+  if (ctx->stream == nullptr || ctx->stream == cudaStreamLegacy || ctx->stream == cudaStreamPerThread) return true;
+  cudaStreamCaptureStatus st = cudaStreamCaptureStatusNone;
+  if (cudaStreamIsCapturing(ctx->stream, &st) != cudaSuccess) { (void)cudaGetLastError(); return true; }
+  return st != cudaStreamCaptureStatusNone;
+}
+
 extern "C" {
 
 int starkv_create(starkv_ctx** out, const starkv_desc* d, void* cuda_stream) {
@@ -54,6 +95,13 @@ void starkv_destroy(starkv_ctx* ctx) {
   if (!ctx) return;
   if (ctx->ev0) cudaEventDestroy(ctx->ev0);
   if (ctx->ev1) cudaEventDestroy(ctx->ev1);
+  for (int i = 0; i < starkv_ctx::kHostGraphs; ++i) {
+    if (ctx->g_dec[i].exec) cudaGraphExecDestroy(ctx->g_dec[i].exec);
+    if (ctx->g_app[i].exec) cudaGraphExecDestroy(ctx->g_app[i].exec);
+  }
+  if (ctx->pin_free) cudaEventDestroy(ctx->pin_free);
+  if (ctx->pin) cudaFreeHost(ctx->pin);
+  if (ctx->pin2) cudaFreeHost(ctx->pin2);
   free(ctx);
 }
 
@@ -116,6 +164,30 @@ int starkv_decode_attn_generic(starkv_ctx* ctx, const void* q, const void* pool,
   return sk_decode_generic(ctx, q, pool, table, max_pages, seq_lens, batch, B_k, B_v, ws, ws_bytes, out);
 }
 
+// enqueue-only body shared by the direct and the captured path: copies from `q_src` / `len_src`, decode, copy to `out_dst`
+static int sk_decode_host_enqueue(starkv_ctx* ctx, const void* q_src, const void* pool, const int32_t* table, int max_pages,
+                                  const int32_t* len_src, int batch, const void* B_k, const void* B_v, void* ws, size_t ws_bytes,
+                                  void* out_dst, bool staged) {
+  SkWorkspace w;
+  sk_plan_workspace(ctx, batch, max_pages, &w);
+  const size_t qbytes = (size_t)batch * ctx->L.n_q_heads * ctx->L.head_dim * 2;
+  const size_t qb = (qbytes + 255) / 256 * 256;
+  const size_t lb = ((size_t)batch * 4 + 255) / 256 * 256;
+  uint8_t* dq = (uint8_t*)ws + w.host_off;   // device staging [q][seq_lens][out], same layout as the pinned block
+  int32_t* dlen = (int32_t*)(dq + qb);
+  uint8_t* dout = dq + qb + lb;
+  if (staged) {   // sources are the library's pinned block [q][seq_lens]: one copy for both
+    SK_CUDA_CHECK(ctx, cudaMemcpyAsync(dq, q_src, qb + (size_t)batch * 4, cudaMemcpyHostToDevice, ctx->stream));
+  } else {
+    SK_CUDA_CHECK(ctx, cudaMemcpyAsync(dq, q_src, qbytes, cudaMemcpyHostToDevice, ctx->stream));
+    SK_CUDA_CHECK(ctx, cudaMemcpyAsync(dlen, len_src, (size_t)batch * 4, cudaMemcpyHostToDevice, ctx->stream));
+  }
+  const int rc = starkv_decode_attn(ctx, dq, pool, table, max_pages, dlen, batch, B_k, B_v, ws, ws_bytes, dout);
+  if (rc) return rc;
+  SK_CUDA_CHECK(ctx, cudaMemcpyAsync(out_dst, dout, qbytes, cudaMemcpyDeviceToHost, ctx->stream));
+  return STARKV_OK;
+}
+
 int starkv_decode_attn_host(starkv_ctx* ctx, const void* q_host, const void* pool, const int32_t* table, int max_pages,
                             const int32_t* seq_lens_host, int batch, const void* B_k, const void* B_v, void* ws,
                             size_t ws_bytes, void* out_host) {
@@ -124,16 +196,63 @@ int starkv_decode_attn_host(starkv_ctx* ctx, const void* q_host, const void* poo
   sk_plan_workspace(ctx, batch, max_pages, &w);
   if (ws_bytes < w.total) return STARKV_ERR_WORKSPACE;
   const size_t qbytes = (size_t)batch * ctx->L.n_q_heads * ctx->L.head_dim * 2;
-  const size_t qb = (qbytes + 255) / 256 * 256;
-  uint8_t* dq = (uint8_t*)ws + w.host_off;
-  uint8_t* dout = dq + qb;
-  int32_t* dlen = (int32_t*)(dout + qb);
-  SK_CUDA_CHECK(ctx, cudaMemcpyAsync(dq, q_host, qbytes, cudaMemcpyHostToDevice, ctx->stream));
-  SK_CUDA_CHECK(ctx, cudaMemcpyAsync(dlen, seq_lens_host, (size_t)batch * 4, cudaMemcpyHostToDevice, ctx->stream));
-  const int rc = starkv_decode_attn(ctx, dq, pool, table, max_pages, dlen, batch, B_k, B_v, ws, ws_bytes, dout);
-  if (rc) return rc;
-  SK_CUDA_CHECK(ctx, cudaMemcpyAsync(out_host, dout, qbytes, cudaMemcpyDeviceToHost, ctx->stream));
+  const size_t qb = (qbytes + 255) / 256 * 256, lb = ((size_t)batch * 4 + 255) / 256 * 256;
+  if (ctx->timing_on || sk_stream_capturing(ctx)) {   // plain path: event timing wants the kernels un-captured
+    const int rc = sk_decode_host_enqueue(ctx, q_host, pool, table, max_pages, seq_lens_host, batch, B_k, B_v, ws, ws_bytes, out_host, false);
+    if (rc) return rc;
+    SK_CUDA_CHECK(ctx, cudaStreamSynchronize(ctx->stream));
+    return STARKV_OK;
+  }
+  // pinned staging: [q][seq_lens][out] at the start of the block; the append staging lives behind it
+  const size_t dec_bytes = 2 * qb + lb;
+  {
+    const int rc = sk_pin_reserve(ctx, &ctx->pin, &ctx->pin_bytes, dec_bytes, ctx->g_dec);
+    if (rc) return rc;
+  }
+  uint8_t* pq = (uint8_t*)ctx->pin + kPinDecode;
+  uint8_t* plen = pq + qb;
+  uint8_t* pout = plen + lb;
+  static const bool use_graph = []() { const char* e = getenv("STARKV_HOST_GRAPH"); return e && e[0] == '1'; }();
+  if (!use_graph) {   // default: direct enqueue, one H2D copy (q + seq_lens) from the pinned block, one D2H copy
+    memcpy(pq, q_host, qbytes);
+    memcpy(plen, seq_lens_host, (size_t)batch * 4);
+    const int rc = sk_decode_host_enqueue(ctx, pq, pool, table, max_pages, (const int32_t*)plen, batch, B_k, B_v, ws, ws_bytes, pout, true);
+    if (rc) return rc;
+    SK_CUDA_CHECK(ctx, cudaStreamSynchronize(ctx->stream));
+    memcpy(out_host, pout, qbytes);
+    return STARKV_OK;
+  }
+  const void* kp[8] = {pool, table, B_k, B_v, ws, ctx->pin, nullptr, nullptr};
+  const long long kv[10] = {max_pages, batch, (long long)ws_bytes, ctx->n_splits_override, 0, 0, 0, 0, 0, 0};
+  starkv_ctx::HostGraph* hg = sk_graph_find(ctx->g_dec, kp, kv);
+  if (!hg) {
+    hg = sk_graph_slot(ctx->g_dec, &ctx->g_dec_next);
+    // un-captured warm-up run: sets the kernels' function attributes (not capturable) and validates the arguments
+    memcpy(pq, q_host, qbytes);
+    memcpy(plen, seq_lens_host, (size_t)batch * 4);
+    int rc = sk_decode_host_enqueue(ctx, pq, pool, table, max_pages, (const int32_t*)plen, batch, B_k, B_v, ws, ws_bytes, pout, true);
+    if (rc) return rc;
+    SK_CUDA_CHECK(ctx, cudaStreamSynchronize(ctx->stream));
+    cudaGraph_t graph = nullptr;
+    SK_CUDA_CHECK(ctx, cudaStreamBeginCapture(ctx->stream, cudaStreamCaptureModeThreadLocal));
+    rc = sk_decode_host_enqueue(ctx, pq, pool, table, max_pages, (const int32_t*)plen, batch, B_k, B_v, ws, ws_bytes, pout, true);
+    const cudaError_t ce = cudaStreamEndCapture(ctx->stream, &graph);
+    if (rc) { if (graph) cudaGraphDestroy(graph); return rc; }
+    SK_CUDA_CHECK(ctx, ce);
+    const cudaError_t ie = cudaGraphInstantiate(&hg->exec, graph, 0);
+    cudaGraphDestroy(graph);
+    if (ie != cudaSuccess) hg->exec = nullptr;
+    SK_CUDA_CHECK(ctx, ie);
+    memcpy(hg->p, kp, sizeof(kp));
+    memcpy(hg->v, kv, sizeof(kv));
+    memcpy(out_host, pout, qbytes);   // the warm-up run already produced this call's result
+    return STARKV_OK;
+  }
+  memcpy(pq, q_host, qbytes);
+  memcpy(plen, seq_lens_host, (size_t)batch * 4);
+  SK_CUDA_CHECK(ctx, cudaGraphLaunch(hg->exec, ctx->stream));
   SK_CUDA_CHECK(ctx, cudaStreamSynchronize(ctx->stream));
+  memcpy(out_host, pout, qbytes);
   return STARKV_OK;
 }
 
@@ -142,6 +261,33 @@ size_t starkv_append_host_workspace_bytes(const starkv_ctx* ctx, int n_new, int 
   const size_t up = 255;
   return sk_append_ws_bytes(ctx, n_new) + (((size_t)n_new * k_row_elems * 2 + up) & ~up) +
          (((size_t)n_new * v_row_elems * 2 + up) & ~up) + 2 * (((size_t)n_new * 4 + up) & ~up);
+}
+
+// enqueue-only body shared by the direct and the captured path
+static int sk_append_host_enqueue(starkv_ctx* ctx, void* pool, const int32_t* table, int max_pages, const void* seq_src,
+                                  const void* pos_src, int n_new, const void* k_src, int k_row_elems, int64_t k_head_stride,
+                                  int d_in_k, const void* v_src, int v_row_elems, int d_in_v, const void* A_k, const void* A_v,
+                                  void* ws, bool staged_block) {
+  const size_t up = 255;
+  const size_t zb = sk_append_ws_bytes(ctx, n_new);
+  const size_t kb = (size_t)n_new * k_row_elems * 2, vb = (size_t)n_new * v_row_elems * 2, ib = (size_t)n_new * 4;
+  uint8_t* dk = (uint8_t*)ws + zb;
+  uint8_t* dv = dk + ((kb + up) & ~up);
+  int32_t* dseq = (int32_t*)(dv + ((vb + up) & ~up));
+  int32_t* dpos = (int32_t*)((uint8_t*)dseq + ((ib + up) & ~up));
+  const void* vdev = v_src != k_src ? (const void*)dv : (const void*)dk;
+  const bool staged = staged_block && v_src != k_src;   // [k][v][seq_ids][positions] in the device staging layout
+  if (staged) {   // sources already in the device staging layout (pinned block of starkv_append_host): one copy
+    const size_t total = ((kb + up) & ~up) + ((vb + up) & ~up) + ((ib + up) & ~up) + ib;
+    SK_CUDA_CHECK(ctx, cudaMemcpyAsync(dk, k_src, total, cudaMemcpyHostToDevice, ctx->stream));
+  } else {
+    SK_CUDA_CHECK(ctx, cudaMemcpyAsync(dk, k_src, kb, cudaMemcpyHostToDevice, ctx->stream));
+    if (v_src != k_src) SK_CUDA_CHECK(ctx, cudaMemcpyAsync(dv, v_src, vb, cudaMemcpyHostToDevice, ctx->stream));
+    SK_CUDA_CHECK(ctx, cudaMemcpyAsync(dseq, seq_src, ib, cudaMemcpyHostToDevice, ctx->stream));
+    SK_CUDA_CHECK(ctx, cudaMemcpyAsync(dpos, pos_src, ib, cudaMemcpyHostToDevice, ctx->stream));
+  }
+  return starkv_append(ctx, pool, table, max_pages, dseq, dpos, n_new, dk, k_row_elems, k_head_stride, d_in_k, vdev,
+                       v_row_elems, d_in_v, A_k, A_v, ws, zb);
 }
 
 int starkv_append_host(starkv_ctx* ctx, void* pool, const int32_t* table, int max_pages, const int32_t* seq_ids_host,
@@ -153,22 +299,70 @@ int starkv_append_host(starkv_ctx* ctx, void* pool, const int32_t* table, int ma
   if (!seq_ids_host || !positions_host || !k_new_host || !v_new_host || !ws || !aligned16(ws)) return STARKV_ERR_INVALID_ARG;
   if (ws_bytes < starkv_append_host_workspace_bytes(ctx, n_new, k_row_elems, v_row_elems)) return STARKV_ERR_WORKSPACE;
   const size_t up = 255;
-  const size_t zb = sk_append_ws_bytes(ctx, n_new);
   const size_t kb = (size_t)n_new * k_row_elems * 2, vb = (size_t)n_new * v_row_elems * 2, ib = (size_t)n_new * 4;
-  uint8_t* dk = (uint8_t*)ws + zb;
-  uint8_t* dv = dk + ((kb + up) & ~up);
-  int32_t* dseq = (int32_t*)(dv + ((vb + up) & ~up));
-  int32_t* dpos = (int32_t*)((uint8_t*)dseq + ((ib + up) & ~up));
-  SK_CUDA_CHECK(ctx, cudaMemcpyAsync(dk, k_new_host, kb, cudaMemcpyHostToDevice, ctx->stream));
-  const void* vdev = dk;
-  if (v_new_host != k_new_host) {
-    SK_CUDA_CHECK(ctx, cudaMemcpyAsync(dv, v_new_host, vb, cudaMemcpyHostToDevice, ctx->stream));
-    vdev = dv;
+  const bool same = v_new_host == k_new_host;
+  const size_t kbp = (kb + up) & ~up, vbp = same ? 0 : ((vb + up) & ~up), ibp = (ib + up) & ~up;
+  static const bool use_graph = []() { const char* e = getenv("STARKV_HOST_GRAPH"); return e && e[0] == '1'; }();
+  const size_t need = kbp + vbp + 2 * ibp;
+  if (n_new > 64 || need > ((size_t)4 << 20) || ctx->stream == nullptr || ctx->stream == cudaStreamLegacy ||
+      ctx->stream == cudaStreamPerThread)   // staging is for decode-time appends on a stream of the caller's own
+    return sk_append_host_enqueue(ctx, pool, table, max_pages, seq_ids_host, positions_host, n_new, k_new_host, k_row_elems,
+                                  k_head_stride, d_in_k, v_new_host, v_row_elems, d_in_v, A_k, A_v, ws, false);
+  // the previous graph launch may still be reading the staging block (this call does not synchronise)
+  if (ctx->pin_busy) {
+    SK_CUDA_CHECK(ctx, cudaEventSynchronize(ctx->pin_free));
+    ctx->pin_busy = 0;
   }
-  SK_CUDA_CHECK(ctx, cudaMemcpyAsync(dseq, seq_ids_host, ib, cudaMemcpyHostToDevice, ctx->stream));
-  SK_CUDA_CHECK(ctx, cudaMemcpyAsync(dpos, positions_host, ib, cudaMemcpyHostToDevice, ctx->stream));
-  return starkv_append(ctx, pool, table, max_pages, dseq, dpos, n_new, dk, k_row_elems, k_head_stride, d_in_k, vdev,
-                       v_row_elems, d_in_v, A_k, A_v, ws, zb);
+  {
+    const int rc = sk_pin_reserve(ctx, &ctx->pin2, &ctx->pin2_bytes, need, ctx->g_app);
+    if (rc) return rc;
+  }
+  uint8_t* pk = (uint8_t*)ctx->pin2;
+  uint8_t* pv = same ? pk : pk + kbp;
+  uint8_t* pseq = pk + kbp + vbp;
+  uint8_t* ppos = pseq + ibp;
+  memcpy(pk, k_new_host, kb);
+  if (!same) memcpy(pv, v_new_host, vb);
+  memcpy(pseq, seq_ids_host, ib);
+  memcpy(ppos, positions_host, ib);
+  if (!ctx->pin_free) SK_CUDA_CHECK(ctx, cudaEventCreateWithFlags(&ctx->pin_free, cudaEventDisableTiming));
+  if (!use_graph || sk_stream_capturing(ctx)) {   // default: direct enqueue, one H2D copy from the pinned block
+    const int rc = sk_append_host_enqueue(ctx, pool, table, max_pages, pseq, ppos, n_new, pk, k_row_elems, k_head_stride, d_in_k,
+                                          pv, v_row_elems, d_in_v, A_k, A_v, ws, true);
+    if (rc) return rc;
+    SK_CUDA_CHECK(ctx, cudaEventRecord(ctx->pin_free, ctx->stream));
+    ctx->pin_busy = 1;
+    return STARKV_OK;
+  }
+  const void* kp[8] = {pool, table, A_k, A_v, ws, ctx->pin2, nullptr, nullptr};
+  const long long kv[10] = {max_pages, n_new, k_row_elems, (long long)k_head_stride, d_in_k, v_row_elems, d_in_v, same ? 1 : 0, 0, 0};
+  starkv_ctx::HostGraph* hg = sk_graph_find(ctx->g_app, kp, kv);
+  if (!hg) {
+    hg = sk_graph_slot(ctx->g_app, &ctx->g_app_next);
+    // un-captured warm-up run (function attributes, argument checks); it also performs this call's append
+    int rc = sk_append_host_enqueue(ctx, pool, table, max_pages, pseq, ppos, n_new, pk, k_row_elems, k_head_stride, d_in_k, pv,
+                                    v_row_elems, d_in_v, A_k, A_v, ws, true);
+    if (rc) return rc;
+    SK_CUDA_CHECK(ctx, cudaStreamSynchronize(ctx->stream));
+    cudaGraph_t graph = nullptr;
+    SK_CUDA_CHECK(ctx, cudaStreamBeginCapture(ctx->stream, cudaStreamCaptureModeThreadLocal));
+    rc = sk_append_host_enqueue(ctx, pool, table, max_pages, pseq, ppos, n_new, pk, k_row_elems, k_head_stride, d_in_k, pv,
+                                v_row_elems, d_in_v, A_k, A_v, ws, true);
+    const cudaError_t ce = cudaStreamEndCapture(ctx->stream, &graph);
+    if (rc) { if (graph) cudaGraphDestroy(graph); return rc; }
+    SK_CUDA_CHECK(ctx, ce);
+    const cudaError_t ie = cudaGraphInstantiate(&hg->exec, graph, 0);
+    cudaGraphDestroy(graph);
+    if (ie != cudaSuccess) hg->exec = nullptr;
+    SK_CUDA_CHECK(ctx, ie);
+    memcpy(hg->p, kp, sizeof(kp));
+    memcpy(hg->v, kv, sizeof(kv));
+    return STARKV_OK;
+  }
+  SK_CUDA_CHECK(ctx, cudaGraphLaunch(hg->exec, ctx->stream));
+  SK_CUDA_CHECK(ctx, cudaEventRecord(ctx->pin_free, ctx->stream));
+  ctx->pin_busy = 1;
+  return STARKV_OK;
 }
 
 int starkv_set_kernel_timing(starkv_ctx* ctx, int on) {

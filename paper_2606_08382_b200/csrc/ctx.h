@@ -22,6 +22,22 @@ struct starkv_ctx {
   int timing_on;         // record events around the main decode kernel
   int timing_valid;
   cudaEvent_t ev0, ev1;
+  // HOST-buffer entry points: pinned staging + one instantiated CUDA graph per call signature, so that a step costs
+  // one cudaGraphLaunch instead of a dozen driver calls
+  void* pin;              // pinned host staging of starkv_decode_attn_host: [q][seq_lens][out]
+  size_t pin_bytes;
+  void* pin2;             // pinned host staging of starkv_append_host: [k][v][seq_ids][positions]
+  size_t pin2_bytes;
+  cudaEvent_t pin_free;   // recorded after the last graph that reads the append staging area
+  int pin_busy;
+  struct HostGraph {
+    cudaGraphExec_t exec;
+    const void* p[8];
+    long long v[10];
+  };
+  static const int kHostGraphs = 8;   // cached call signatures per entry point (e.g. one per block table in use)
+  HostGraph g_dec[8], g_app[8];
+  int g_dec_next, g_app_next;         // round-robin replacement
   char err[512];
 };
 

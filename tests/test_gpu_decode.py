@@ -203,19 +203,82 @@ def test_error_paths():
     assert sk.starkv_last_launches(ctx) == 3
 
 
-def test_host_variant_matches_device_variant():
+@pytest.mark.parametrize("own_stream", [False, True], ids=["default-stream", "own-stream-graph"])
+def test_host_variant_matches_device_variant(own_stream):
+    """On the legacy default stream the HOST variant enqueues directly; on a stream of its own it replays a cached
+    CUDA graph fed from pinned staging."""
     cfg = synth.make_config("C3", context=1000, batch=2)
     cache = build_cache(cfg)
     bk, bv = synth.make_factors(cfg)
     q16 = synth.make_q(cfg)
     want = run_decode(cfg, cache, q16, bk, bv)
     from tests.gpu_util import dev, f16
-    ctx = sk.create_from_config(cfg)
+    stream = torch.cuda.Stream() if own_stream else None
+    ctx = sk.create_from_config(cfg, stream=stream)
     pool, table = dev(cache["pool"]), dev(cache["table"].astype(np.int32))
+    torch.cuda.synchronize()
     wsb = sk.starkv_workspace_bytes(ctx, 2, table.shape[1])
     ws = torch.empty(wsb, dtype=torch.uint8, device="cuda")
     qh = torch.from_numpy(q16.view(np.uint16).astype(np.int16)).view(torch.float16).pin_memory()
     lh = torch.from_numpy(np.asarray(cache["seq_lens"], np.int32)).pin_memory()
     oh = torch.empty((2, cfg.n_q_heads, cfg.head_dim), dtype=torch.float16).pin_memory()
-    sk.starkv_decode_attn_host(ctx, qh, pool, table, table.shape[1], lh, 2, f16(bk), f16(bv), ws, wsb, oh)
+    bkd, bvd = f16(bk), f16(bv)
+    sk.starkv_decode_attn_host(ctx, qh, pool, table, table.shape[1], lh, 2, bkd, bvd, ws, wsb, oh)
     assert np.array_equal(oh.double().numpy(), want)
+    # later calls with the same buffers replay the library's cached CUDA graph: new host data must be picked up
+    q2 = synth.make_q(synth.make_config("C3", context=1000, batch=2, seed=5))
+    want2 = run_decode(cfg, cache, q2, bk, bv)
+    for qq, ww in ((q2, want2), (q16, want), (q2, want2)):
+        qh.copy_(torch.from_numpy(qq.view(np.uint16).astype(np.int16)).view(torch.float16))
+        oh.zero_()
+        sk.starkv_decode_attn_host(ctx, qh, pool, table, table.shape[1], lh, 2, bkd, bvd, ws, wsb, oh)
+        assert np.array_equal(oh.double().numpy(), ww)
+    # shorter sequences through the same graph (seq_lens is data, not part of the signature)
+    lens2 = np.asarray([700, 64], np.int32)
+    cache2 = dict(cache, seq_lens=lens2)
+    want3 = run_decode(cfg, cache2, q16, bk, bv)
+    qh.copy_(torch.from_numpy(q16.view(np.uint16).astype(np.int16)).view(torch.float16))
+    lh.copy_(torch.from_numpy(lens2))
+    sk.starkv_decode_attn_host(ctx, qh, pool, table, table.shape[1], lh, 2, bkd, bvd, ws, wsb, oh)
+    assert np.array_equal(oh.double().numpy(), want3)
+
+
+@pytest.mark.parametrize("own_stream", [False, True], ids=["default-stream", "own-stream-graph"])
+def test_append_host_variant_matches_device_variant(own_stream):
+    """starkv_append_host (pinned staging + cached graph) writes the same page bytes as starkv_append, on the first
+    call (direct run + capture) and on replays with new host data."""
+    from tests.gpu_util import dev, f16
+    cfg = synth.make_config("C3", context=256, batch=4)
+    stream = torch.cuda.Stream() if own_stream else None
+    ctx = sk.create_from_config(cfg, stream=stream)
+    lens = np.full(4, 200, np.int32)
+    table, n_pool = synth.make_block_table(cfg, lens + 8)
+    page_bytes = sk.starkv_page_bytes(ctx)
+    dk_in, dv_in = cfg.head_dim, cfg.n_kv_heads * cfg.head_dim
+    ak, av = synth.make_append_factors(cfg, dk_in, dv_in)
+    akd, avd, tab = f16(ak), f16(av), dev(table.astype(np.int32))
+    pool_a = torch.zeros((n_pool, page_bytes), dtype=torch.uint8, device="cuda")
+    pool_b = torch.zeros_like(pool_a)
+    wsb = max(sk.starkv_append_workspace_bytes(ctx, 4), sk.starkv_append_host_workspace_bytes(ctx, 4, dv_in, dv_in))
+    ws = torch.empty(wsb, dtype=torch.uint8, device="cuda")
+    seq = np.arange(4, dtype=np.int32)
+    hk = torch.empty((4, dv_in), dtype=torch.float16).pin_memory()
+    hv = torch.empty((4, dv_in), dtype=torch.float16).pin_memory()
+    hs, hp = torch.from_numpy(seq.copy()).pin_memory(), torch.zeros(4, dtype=torch.int32).pin_memory()
+    for step in range(4):
+        rng = np.random.default_rng(100 + step)
+        kn = rng.standard_normal((4, dv_in)).astype(np.float16)
+        vn = rng.standard_normal((4, dv_in)).astype(np.float16)
+        pos = (lens + step).astype(np.int32)
+        dseq, dpos, dkn, dvn = dev(seq), dev(pos), f16(kn), f16(vn)
+        torch.cuda.synchronize()
+        sk.starkv_append(ctx, pool_a, tab, table.shape[1], dseq, dpos, 4, dkn, dv_in, cfg.head_dim, dk_in, dvn,
+                         dv_in, dv_in, akd, avd, ws, wsb)
+        torch.cuda.synchronize()
+        hk.copy_(torch.from_numpy(kn.view(np.int16)).view(torch.float16))
+        hv.copy_(torch.from_numpy(vn.view(np.int16)).view(torch.float16))
+        hp.copy_(torch.from_numpy(pos))
+        sk.starkv_append_host(ctx, pool_b, tab, table.shape[1], hs, hp, 4, hk, dv_in, cfg.head_dim, dk_in, hv, dv_in, dv_in,
+                              akd, avd, ws, wsb)
+        torch.cuda.synchronize()
+        assert torch.equal(pool_a, pool_b), step

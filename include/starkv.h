@@ -16,6 +16,8 @@
  *   - Return value: 0 = STARKV_OK, negative = error (see enum).  No exception or abort crosses
  *     the ABI.  Inputs must be finite; NaN/Inf in the data are not detected.
  *   - Device pointers must be 16-byte aligned; the page pool 128-byte aligned.
+ *   - A context is bound to the device current at starkv_create and to one stream; it is not thread-safe (one
+ *     caller at a time per context; different contexts are independent).
  */
 #ifndef STARKV_H
 #define STARKV_H

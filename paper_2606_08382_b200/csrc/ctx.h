@@ -71,6 +71,12 @@ __device__ __forceinline__ void sk_pdl_enter() {
   asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
   asm volatile("griddepcontrol.wait;" ::: "memory");
 }
+// The two halves separately, for a kernel that does dependency-free work first: shared-memory set-up and reads of
+// CALLER-OWNED inputs that no kernel of this library ever writes (seq_lens, block tables).  Such inputs are final
+// when the first kernel of a PDL chain starts (a predecessor outside the chain never triggers early, so the chain's
+// head starts only after it completed), hence they may be read before the wait.
+__device__ __forceinline__ void sk_pdl_trigger() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+__device__ __forceinline__ void sk_pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
 template <typename... KArgs, typename... Args>
 static inline cudaError_t sk_launch(const starkv_ctx* ctx, void (*kern)(KArgs...), dim3 grid, dim3 block, size_t smem,
                                     Args... args) {

@@ -503,7 +503,10 @@ __device__ __forceinline__ void apply_k_scales(float (&sc)[4][2], const float (&
 //   BH / BL: bit widths of the leading / trailing blocks (16/16 = fp16 latents).
 //   kcst: per (KV head, block, quad column) accumulator start value (the offset term, see above).
 // ---------------------------------------------------------------------------------------------
-template <int BH, int BL>
+//   UM: P goes out as the K-major canonical (no-swizzle, 8 x 16-byte core matrices) B operand of the tcgen05 PV
+//       product instead: element (head, token) at (head >> 3) * 1024 + (token >> 3) * 128 + (head & 7) * 16 +
+//       (token & 7) * 2; no transpose, this thread's 4 + 4 consecutive tokens of head 4 gw + j are two 8-byte stores.
+template <int BH, int BL, bool UM = false>
 __device__ __forceinline__ void score_page(const StarkvLayout& L, const DecodePlan& PL, const uint8_t* __restrict__ pg,
                                            const uint2* __restrict__ qimg_lane, const float* __restrict__ kcst, int kv0,
                                            int kv1, int nvalid, int R, int j, int gw, float& m_run, float& l_run,
@@ -567,13 +570,21 @@ __device__ __forceinline__ void score_page(const StarkvLayout& L, const DecodePl
   }
   l_run = fmaf(l_run, alpha, sum);
   m_run = m_new;
+  if (UM) {
+    static_assert(!UM || QUANT, "tcgen05 PV is built for the quantised modes (token order tb + s)");
 #pragma unroll
-  for (int u = 0; u < 2; ++u)
+    for (int be = 0; be < 2; ++be)
+      *reinterpret_cast<uint2*>(Pb + p_thr_off + be * 128) =
+          make_uint2(pack_h2(sc[0][be], sc[1][be]), pack_h2(sc[2][be], sc[3][be]));
+  } else {
 #pragma unroll
-    for (int be = 0; be < 2; ++be) {
-      const uint32_t y = movmatrix_trans(pack_h2(sc[2 * u][be], sc[2 * u + 1][be]));
-      *reinterpret_cast<uint32_t*>(Pb + p_thr_off + u * (4 * 32 * 16) + be * 4) = y;
-    }
+    for (int u = 0; u < 2; ++u)
+#pragma unroll
+      for (int be = 0; be < 2; ++be) {
+        const uint32_t y = movmatrix_trans(pack_h2(sc[2 * u][be], sc[2 * u + 1][be]));
+        *reinterpret_cast<uint32_t*>(Pb + p_thr_off + u * (4 * 32 * 16) + be * 4) = y;
+      }
+  }
   const bool any_up = __any_sync(0xffffffffu, up);
   if (R == 0) al[4 * gw + j] = alpha;
   if ((R | j) == 0) flag[gw] = any_up ? 1 : 0;
@@ -597,7 +608,9 @@ __global__ void __launch_bounds__(NG * GW * 32, 1) decode_fast_kernel(
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const int j = lane & 3, R = lane >> 2;
   const int split = blockIdx.x, b = blockIdx.y;
-  sk_pdl_enter();
+  sk_pdl_trigger();
+  // seq_lens and the block table are caller-owned inputs (ctx.h): read ahead of the dependency wait, as is the
+  // shared-memory set-up, so that after the wait thread 0 only has to issue the first page copies
   const int len = seq_lens[b];
   const int n_pages = (len + PTOK - 1) / PTOK;
   int p0, p1;
@@ -607,6 +620,7 @@ __global__ void __launch_bounds__(NG * GW * 32, 1) decode_fast_kernel(
   float* my_parts = parts + ((size_t)b * n_splits + split) * L.n_q_heads * pstride;
 
   if (n_it <= 0) {   // empty range (CTA-uniform): neutral partial
+    sk_pdl_wait();
     for (int i = tid; i < L.n_q_heads * (int)pstride; i += NTHREADS) {
       const int c = i % (int)pstride;
       my_parts[i] = c == 0 ? -INFINITY : 0.f;
@@ -643,17 +657,19 @@ __global__ void __launch_bounds__(NG * GW * 32, 1) decode_fast_kernel(
     }
     mbar_init(qbar, 1);
     fence_barrier_init();
-    const uint32_t qbytes = (uint32_t)(PL.qimg_bytes + L.n_kv_heads * 32);   // image + accumulator start values
-    mbar_expect_tx(qbar, qbytes);
-    bulk_g2s(smem_u32(smem + PL.off_qimg), qimg_all + (size_t)b * qimg_stride, qbytes, qbar);
     int pgs[8];
 #pragma unroll
     for (int s = 0; s < 8; ++s) pgs[s] = s < min(nstage, n_it) ? my_table[s] : 0;
+    sk_pdl_wait();
+    const uint32_t qbytes = (uint32_t)(PL.qimg_bytes + L.n_kv_heads * 32);   // image + accumulator start values
+    mbar_expect_tx(qbar, qbytes);
+    bulk_g2s(smem_u32(smem + PL.off_qimg), qimg_all + (size_t)b * qimg_stride, qbytes, qbar);
 #pragma unroll
     for (int s = 0; s < 8; ++s)
       if (s < min(nstage, n_it)) issue(s, pgs[s]);
   }
   for (int i = tid; i < min(n_it, TBL_SMEM); i += NTHREADS) tbl_s[i] = my_table[i];
+  sk_pdl_wait();   // (thread 0 has waited already; a second wait returns at once)
   __syncthreads();
 
   // ================= consumers =================
@@ -868,6 +884,394 @@ __global__ void __launch_bounds__(NG * GW * 32, 1) decode_fast_kernel(
   SK_STAMP(5);
 }
 
+// ---------------------------------------------------------------------------------------------
+// tcgen05 variant of the kernel for the integer modes (rows D2-D7): QK and the softmax exactly as above, but the
+// PV product  O^T[ch x heads] += L_v^T[ch x tok] . P^T[tok x heads]  runs on the 5th-generation tensor cores:
+//   A = dequantised value page (c * s in fp16, one rounding, as in the mma.sync kernel), written by the group's
+//       256 threads into the K-major no-swizzle canonical layout (8 channels x 8 tokens core matrices):
+//       element (ch, t) at (ch >> 3) * 1024 + (t >> 3) * 128 + (ch & 7) * 16 + (t & 7) * 2  -- one 16-byte
+//       LDS of packed codes -> 2 (int8) or 4 (int4) 16-byte STS, about 2 instructions per value pair;
+//   B = P^T in the same layout (score_page<UM>), N = 32 heads;
+//   D = fp32 accumulators in TMEM, 32 columns per 128-channel M tile and group; M = 128, N = 32, K = 16 per
+//       tcgen05.mma (kind::f16, cta_group::1), 4 K steps per page, issued by one thread of the group, which then
+//       commits to the group's mbarrier and refills the page's ring stage (every warp of the group is past its
+//       shared-memory reads of the page at that point: no ticket).
+// The lazy softmax rescale (rare after the first pages) reads, scales and writes back the TMEM tile
+// (tcgen05.ld / st); the first page of a group starts its accumulators with the MMA's accumulate flag off.
+// One named barrier per page and group, as before; the MMAs of page i run under the QK phase of page i + 1.
+// ---------------------------------------------------------------------------------------------
+constexpr int UM_ROWS = 128;                         // channels per M tile
+constexpr int UM_TILE_BYTES = UM_ROWS * PTOK * 2;     // 16 KB of A per M tile and page
+
+__device__ __forceinline__ uint64_t umma_desc_k(uint32_t saddr) {
+  // SWIZZLE_NONE K-major matrix descriptor: start >> 4 | LBO (next core matrix along K) = 128 B |
+  // SBO (next 8 rows) = 1024 B | version 1 (sm_100)
+  return (uint64_t)((saddr & 0x3FFFF) >> 4) | ((uint64_t)(128 >> 4) << 16) | ((uint64_t)(1024 >> 4) << 32) |
+         ((uint64_t)1 << 46);
+}
+__device__ __forceinline__ void umma_f16(uint32_t tmem_d, uint64_t da, uint64_t db, uint32_t idesc, uint32_t accum) {
+  asm volatile(
+      "{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\t"
+      "tcgen05.mma.cta_group::1.kind::f16 [%0], %1, %2, %3, p;\n\t}" ::"r"(tmem_d),
+      "l"(da), "l"(db), "r"(idesc), "r"(accum)
+      : "memory");
+}
+__device__ __forceinline__ void umma_commit(uint32_t bar) {
+  asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(bar) : "memory");
+}
+__device__ __forceinline__ void tc_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
+__device__ __forceinline__ void tc_fence_after() { asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory"); }
+__device__ __forceinline__ void tmem_ld32(uint32_t taddr, uint32_t (&v)[32]) {
+  asm volatile(
+      "tcgen05.ld.sync.aligned.32x32b.x32.b32 {%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15,%16,%17,%18,%19,%20,%21,"
+      "%22,%23,%24,%25,%26,%27,%28,%29,%30,%31}, [%32];"
+      : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7]), "=r"(v[8]), "=r"(v[9]),
+        "=r"(v[10]), "=r"(v[11]), "=r"(v[12]), "=r"(v[13]), "=r"(v[14]), "=r"(v[15]), "=r"(v[16]), "=r"(v[17]), "=r"(v[18]),
+        "=r"(v[19]), "=r"(v[20]), "=r"(v[21]), "=r"(v[22]), "=r"(v[23]), "=r"(v[24]), "=r"(v[25]), "=r"(v[26]), "=r"(v[27]),
+        "=r"(v[28]), "=r"(v[29]), "=r"(v[30]), "=r"(v[31])
+      : "r"(taddr));
+  asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+}
+__device__ __forceinline__ void tmem_st32(uint32_t taddr, const uint32_t (&v)[32]) {
+  asm volatile(
+      "tcgen05.st.sync.aligned.32x32b.x32.b32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15,%16,%17,%18,%19,%20,%21,"
+      "%22,%23,%24,%25,%26,%27,%28,%29,%30,%31,%32};" ::"r"(taddr),
+      "r"(v[0]), "r"(v[1]), "r"(v[2]), "r"(v[3]), "r"(v[4]), "r"(v[5]), "r"(v[6]), "r"(v[7]), "r"(v[8]), "r"(v[9]), "r"(v[10]),
+      "r"(v[11]), "r"(v[12]), "r"(v[13]), "r"(v[14]), "r"(v[15]), "r"(v[16]), "r"(v[17]), "r"(v[18]), "r"(v[19]), "r"(v[20]),
+      "r"(v[21]), "r"(v[22]), "r"(v[23]), "r"(v[24]), "r"(v[25]), "r"(v[26]), "r"(v[27]), "r"(v[28]), "r"(v[29]), "r"(v[30]),
+      "r"(v[31])
+      : "memory");
+  asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
+}
+
+// One precision block of the value page -> A operand.  Work item = one 16-byte segment of a channel row
+// (32 int4 / 16 int8 slots = NTB 8-token blocks); item i -> channel 8 ((i >> 3) / SEGS) + (i & 7), segment
+// (i >> 3) % SEGS, so 8 consecutive lanes write 8 consecutive channels of one token block (128 contiguous bytes,
+// conflict-free) and a thread keeps its segment -- hence its scale registers -- across its items (i += 256).
+template <int BITS>
+__device__ __forceinline__ void deq_block_to_a(const uint8_t* __restrict__ vb, const uint8_t* __restrict__ vsc, int n_ch,
+                                               int row0, uint8_t* __restrict__ abuf, int t) {
+  constexpr int SEGS = BITS / 2;   // 16-byte segments per channel row of PTOK slots
+  constexpr int NTB = 8 / SEGS;    // 8-token blocks per segment
+  const int n_items = n_ch * SEGS;
+  if (t >= n_items) return;
+  const int seg = (t >> 3) % SEGS;
+  uint32_t sc[4 * NTB];            // the segment's per-token scales as natural (t, t+1) fp16 pairs
+#pragma unroll
+  for (int k = 0; k < NTB; ++k) {
+    const uint4 u = *reinterpret_cast<const uint4*>(vsc + (seg * NTB + k) * 16);
+    sc[4 * k] = u.x; sc[4 * k + 1] = u.y; sc[4 * k + 2] = u.z; sc[4 * k + 3] = u.w;
+  }
+  for (int i = t; i < n_items; i += 256) {
+    const int ch = ((i >> 3) / SEGS) * 8 + (i & 7);
+    const uint4 x = *reinterpret_cast<const uint4*>(vb + ch * (PTOK * BITS / 8) + seg * 16);
+    const int row = row0 + ch;
+    uint8_t* dst = abuf + (row >> 3) * 1024 + (seg * NTB) * 128 + (row & 7) * 16;
+    if (BITS == 4) {
+      const uint32_t w[4] = {x.x, x.y, x.z, x.w};
+#pragma unroll
+      for (int k = 0; k < 4; ++k) {
+        uint32_t h[4];
+        deq4_pairs(w[k], h);   // (c0,c4), (c1,c5), (c2,c6), (c3,c7)
+        uint4 o;
+        o.x = h2mul(prmt(h[0], h[1], 0x5410u), sc[4 * k]);
+        o.y = h2mul(prmt(h[2], h[3], 0x5410u), sc[4 * k + 1]);
+        o.z = h2mul(prmt(h[0], h[1], 0x7632u), sc[4 * k + 2]);
+        o.w = h2mul(prmt(h[2], h[3], 0x7632u), sc[4 * k + 3]);
+        *reinterpret_cast<uint4*>(dst + k * 128) = o;
+      }
+    } else {
+      const uint32_t w[4] = {x.x, x.y, x.z, x.w};
+#pragma unroll
+      for (int k = 0; k < 2; ++k) {
+        uint32_t a, b, c, d;
+        deq8_pairs(w[2 * k], a, b);
+        deq8_pairs(w[2 * k + 1], c, d);
+        uint4 o;
+        o.x = h2mul(a, sc[4 * k]);
+        o.y = h2mul(b, sc[4 * k + 1]);
+        o.z = h2mul(c, sc[4 * k + 2]);
+        o.w = h2mul(d, sc[4 * k + 3]);
+        *reinterpret_cast<uint4*>(dst + k * 128) = o;
+      }
+    }
+  }
+}
+
+template <int BH, int BL, int NG>
+__global__ void __launch_bounds__(NG * GW * 32, 1) decode_tc5_kernel(
+    const __grid_constant__ StarkvLayout L, const __grid_constant__ DecodePlan PL, const uint8_t* __restrict__ qimg_all,
+    size_t qimg_stride, const uint8_t* __restrict__ pool, const int32_t* __restrict__ table, int max_pages,
+    const int32_t* __restrict__ seq_lens, float* __restrict__ parts, int n_splits) {
+  extern __shared__ __align__(128) uint8_t smem[];
+  static_assert(BH != 16, "integer modes only");
+  constexpr int NTHREADS = NG * GW * 32;
+
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const int j = lane & 3, R = lane >> 2;
+  const int split = blockIdx.x, b = blockIdx.y;
+  sk_pdl_trigger();
+  // seq_lens and the block table are caller-owned inputs (ctx.h): read ahead of the dependency wait, as is all the
+  // shared-memory and TMEM set-up, so that after the wait thread 0 only has to issue the first page copies
+  const int len = seq_lens[b];
+  const int n_pages = (len + PTOK - 1) / PTOK;
+  int p0, p1;
+  sk_split_range(n_pages, n_splits, 1, split, &p0, &p1);
+  const int n_it = p1 - p0;
+  const size_t pstride = sk_part_stride(L.rank_v);
+  float* my_parts = parts + ((size_t)b * n_splits + split) * L.n_q_heads * pstride;
+
+  if (n_it <= 0) {   // empty range (CTA-uniform): neutral partial
+    sk_pdl_wait();
+    for (int i = tid; i < L.n_q_heads * (int)pstride; i += NTHREADS) {
+      const int c = i % (int)pstride;
+      my_parts[i] = c == 0 ? -INFINITY : 0.f;
+    }
+    return;
+  }
+
+  uint8_t* stage_base = smem + PL.off_stage;
+  const int nstage = PL.nstage;
+  const int n_mt = PL.um_mt;                              // 128-channel M tiles
+  // barrier area: full[nstage], image, mma_done[NG] mbarriers, TMEM base address, issued[nstage]
+  const uint32_t full0 = smem_u32(smem + PL.off_bar);
+  const uint32_t qbar = full0 + 8 * nstage;
+  const uint32_t mbar0 = qbar + 8;
+  volatile uint32_t& tmem_base_s = *reinterpret_cast<volatile uint32_t*>(smem + PL.off_bar + 8 * nstage + 8 + 8 * NG);
+  volatile int* issued = reinterpret_cast<int*>(smem + PL.off_bar + 8 * nstage + 8 + 8 * NG + 8);   // [nstage]
+  int32_t* tbl_s = reinterpret_cast<int32_t*>(smem + PL.off_tbl);
+  const uint32_t page_bytes = (uint32_t)L.page_bytes;
+  const int32_t* my_table = table + (size_t)b * max_pages + p0;
+
+  auto issue = [&](int it, int page) {   // D2: one page -> ring stage (single thread)
+    const int st = it % nstage;
+    const uint32_t bar = full0 + 8 * st;
+    mbar_expect_tx(bar, page_bytes);
+    __threadfence_block();
+    issued[st] = it;
+    bulk_g2s_stream(smem_u32(stage_base + (size_t)st * page_bytes), pool + (size_t)page * page_bytes, page_bytes, bar,
+                    l2_evict_first_policy());
+  };
+
+  if (tid == 0) {
+    for (int s = 0; s < nstage; ++s) {
+      mbar_init(full0 + 8 * s, 1);
+      issued[s] = -1;
+    }
+    mbar_init(qbar, 1);
+    for (int g = 0; g < NG; ++g) mbar_init(mbar0 + 8 * g, 1);
+    fence_barrier_init();
+    int pgs[8];
+#pragma unroll
+    for (int s = 0; s < 8; ++s) pgs[s] = s < min(nstage, n_it) ? my_table[s] : 0;
+    sk_pdl_wait();
+    const uint32_t qbytes = (uint32_t)(PL.qimg_bytes + L.n_kv_heads * 32);
+    mbar_expect_tx(qbar, qbytes);
+    bulk_g2s(smem_u32(smem + PL.off_qimg), qimg_all + (size_t)b * qimg_stride, qbytes, qbar);
+#pragma unroll
+    for (int s = 0; s < 8; ++s)
+      if (s < min(nstage, n_it)) issue(s, pgs[s]);
+  }
+  if (warp == 1) {   // TMEM: 32 fp32 columns per (group, M tile)
+    const uint32_t dst = smem_u32(smem + PL.off_bar + 8 * nstage + 8 + 8 * NG);
+    const uint32_t ncol = (uint32_t)PL.um_cols;
+    asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(dst), "r"(ncol) : "memory");
+    asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+  }
+  for (int i = tid; i < min(n_it, TBL_SMEM); i += NTHREADS) tbl_s[i] = my_table[i];
+
+  const int grp = warp >> 3, gw = warp & (GW - 1), gt = tid & 255;
+  {
+    uint4* pz = reinterpret_cast<uint4*>(smem + PL.off_p);
+    for (int i = tid; i < NG * 2 * P_BUF_BYTES / 16; i += NTHREADS) pz[i] = make_uint4(0, 0, 0, 0);
+    if (tid < NG * 64) reinterpret_cast<float*>(smem + PL.off_alpha)[tid] = 1.f;
+    if (tid < NG * 4) reinterpret_cast<uint32_t*>(smem + PL.off_flag)[tid] = 0;
+  }
+  sk_pdl_wait();   // (thread 0 has waited already; a second wait returns at once)
+  tc_fence_before();
+  __syncthreads();
+  tc_fence_after();
+  const uint32_t tmem_grp = tmem_base_s + (uint32_t)(grp * n_mt * 32);   // this group's accumulator columns
+  mbar_wait(qbar, 0);
+
+  const uint2* qimg_lane = reinterpret_cast<const uint2*>(smem + PL.off_qimg) + lane;
+  const float* kcst = reinterpret_cast<const float*>(smem + PL.off_kcst);
+  uint8_t* Pm = smem + PL.off_p + grp * 2 * P_BUF_BYTES;
+  float* alpha_s = reinterpret_cast<float*>(smem + PL.off_alpha) + grp * 64;
+  uint8_t* flag_s = smem + PL.off_flag + grp * 16;
+  uint8_t* abuf = smem + PL.off_a + grp * n_mt * UM_TILE_BYTES;
+  const uint32_t mbar = mbar0 + 8 * grp;
+
+  const bool has_quad = gw < PL.nq;
+  const int kv0 = gw * PL.kv_per_quad;
+  const int kv1 = min(kv0 + PL.kv_per_quad, L.n_kv_heads);
+  // P^T element (head 4 gw + j, token 16 (R >> 1) + 4 (R & 1)) of the canonical B operand
+  const int p_thr_off = (gw >> 1) * 1024 + (2 * (R >> 1)) * 128 + (4 * (gw & 1) + j) * 16 + 8 * (R & 1);
+  float m_run = -INFINITY, l_run = 0.f;
+
+  // dequantisation work split: the trailing block first, the leading block on the threads its last pass leaves idle
+  const int n_lo_items = L.v_lo_n * (BL / 2);
+  const int t_hi = (gt + 256 - (n_lo_items & 255)) & 255;
+  // instruction descriptor: D fp32 (bit 4), A and B fp16 K-major, N = 32 (bits 17..), M = 128 (bits 24..)
+  constexpr uint32_t IDESC = (1u << 4) | ((uint32_t)(32 >> 3) << 17) | ((uint32_t)(UM_ROWS >> 4) << 24);
+
+  int st = grp % nstage, use = grp / nstage;
+  int gi = 0;
+  for (int it = grp; it < n_it; it += NG, ++gi) {
+    uint8_t* pg = stage_base + (size_t)st * page_bytes;
+    const int nvalid = len - (p0 + it) * PTOK;   // >= 1
+    const int buf = gi & 1;
+    uint8_t* Pb = Pm + buf * P_BUF_BYTES;
+    float* al = alpha_s + buf * 32;
+    uint8_t* fl = flag_s + buf * 8;
+    if (lane == 0)
+      while (issued[st] != it) {}
+    __syncwarp();
+    mbar_wait(full0 + 8 * st, (uint32_t)(use & 1));
+
+    if (nvalid < PTOK) {   // tail page: zero the key rows and the value scales of the slots past the sequence end
+      for (int g = 0; g < L.n_kv_heads; ++g) {
+        for (int blk = 0; blk < 2; ++blk) {
+          const int n = blk ? L.k_lo_n[g] : L.k_hi_n[g];
+          const int rowb = n * (blk ? BL : BH) / 8;
+          uint32_t* dst = reinterpret_cast<uint32_t*>(pg + (blk ? L.k_lo_off[g] : L.k_hi_off[g]) + nvalid * rowb);
+          for (int i = gt; i < (PTOK - nvalid) * rowb / 4; i += 256) dst[i] = 0;
+        }
+      }
+      if (gt < 2 * PTOK && (gt & (PTOK - 1)) >= nvalid) reinterpret_cast<uint16_t*>(pg + L.v_scale_off)[gt] = 0;
+      bar_sync(1 + grp, GW * 32);
+    }
+
+    // ================= QK + softmax for this warp's quad =================
+    if (has_quad)
+      score_page<BH, BL, true>(L, PL, pg, qimg_lane, kcst, kv0, kv1, nvalid, R, j, gw, m_run, l_run, Pb, p_thr_off, al, fl);
+
+    // ================= value page -> A operand =================
+    if (gi > 0) mbar_wait(mbar, (uint32_t)((gi - 1) & 1));   // the MMAs of the previous page have read A and P
+    deq_block_to_a<BL>(pg + L.v_lo_off, pg + L.v_scale_off + PTOK * 2, L.v_lo_n, L.v_hi_n, abuf, gt);
+    deq_block_to_a<BH>(pg + L.v_hi_off, pg + L.v_scale_off, L.v_hi_n, 0, abuf, t_hi);
+    fence_proxy_async();   // P and A (generic-proxy stores) -> visible to the tensor-core (async) proxy
+    bar_sync(1 + grp, GW * 32);
+
+    // ================= lazy rescale of the TMEM accumulators (rare) =================
+    {
+      const uint2 f8 = *reinterpret_cast<const uint2*>(fl);
+      if ((f8.x | f8.y) != 0 && gi > 0) {
+        tc_fence_after();
+        for (int mt = gw >> 2; mt < n_mt; mt += 2) {
+          const uint32_t taddr = tmem_grp + ((uint32_t)((gw & 3) * 32) << 16) + (uint32_t)(mt * 32);
+          uint32_t v[32];
+          tmem_ld32(taddr, v);
+#pragma unroll
+          for (int c = 0; c < 32; ++c) v[c] = __float_as_uint(__uint_as_float(v[c]) * al[c]);
+          tmem_st32(taddr, v);
+        }
+        tc_fence_before();
+        bar_sync(1 + grp, GW * 32);
+      }
+    }
+
+    // ================= PV: one thread issues the MMAs, commits, refills the stage =================
+    if (gt == 0) {
+      tc_fence_after();
+      const uint32_t sa = smem_u32(abuf), sb = smem_u32(Pb);
+      for (int mt = 0; mt < n_mt; ++mt)
+#pragma unroll
+        for (int ks = 0; ks < PTOK / 16; ++ks)
+          umma_f16(tmem_grp + (uint32_t)(mt * 32), umma_desc_k(sa + mt * UM_TILE_BYTES + ks * 256), umma_desc_k(sb + ks * 256),
+                   IDESC, (gi > 0 || ks > 0) ? 1u : 0u);
+      umma_commit(mbar);
+      const int nxt = it + nstage;
+      if (nxt < n_it) issue(nxt, nxt < TBL_SMEM ? tbl_s[nxt] : my_table[nxt]);
+    }
+    st += NG;
+    while (st >= nstage) { st -= nstage; ++use; }
+  }
+
+  // ================= merge the groups and write the split-K partial (D7) =================
+  if (gi > 0) mbar_wait(mbar, (uint32_t)((gi - 1) & 1));   // this group's last MMAs are complete
+  tc_fence_after();
+  bar_sync(BAR_ALL, NTHREADS);
+  float* mg = reinterpret_cast<float*>(smem + PL.off_stage);   // m at [g * 32 + head], l at [96 + ..], weight at [192 + ..]
+  float* ost = mg + 384;
+  const int ST = (int)pstride;
+  if (has_quad) {
+    float lsum = l_run;
+    lsum += __shfl_xor_sync(0xffffffffu, lsum, 4);
+    lsum += __shfl_xor_sync(0xffffffffu, lsum, 8);
+    lsum += __shfl_xor_sync(0xffffffffu, lsum, 16);
+    if (R == 0) {
+      mg[grp * 32 + 4 * gw + j] = m_run;
+      mg[96 + grp * 32 + 4 * gw + j] = lsum;
+    }
+  }
+  bar_sync(BAR_ALL, NTHREADS);
+  if (tid < 32) {
+    const bool live = tid < L.n_q_heads;
+    float ms = -INFINITY, lm = 0.f;
+    if (live) {
+#pragma unroll
+      for (int g = 0; g < NG; ++g) ms = fmaxf(ms, mg[g * 32 + tid]);   // group 0 always has a page: ms is finite
+#pragma unroll
+      for (int g = 0; g < NG; ++g) {
+        const float mo = mg[g * 32 + tid];
+        const float w = mo == -INFINITY ? 0.f : ex2(mo - ms);
+        mg[192 + g * 32 + tid] = w;
+        lm += mg[96 + g * 32 + tid] * w;
+      }
+      *reinterpret_cast<float4*>(ost + tid * ST) = make_float4(ms, lm, 0.f, 0.f);
+    }
+  }
+  bar_sync(BAR_ALL, NTHREADS);
+#pragma unroll
+  for (int pass = 0; pass < NG; ++pass) {   // group 0 stores, the others add one after the other (if they had a page)
+    if (grp == pass && gi > 0) {
+      const float* wt = mg + 192 + 32 * grp;
+      for (int mt = gw >> 2; mt < n_mt; mt += 2) {
+        const uint32_t taddr = tmem_grp + ((uint32_t)((gw & 3) * 32) << 16) + (uint32_t)(mt * 32);
+        uint32_t v[32];
+        tmem_ld32(taddr, v);
+        const int ch = mt * UM_ROWS + (gw & 3) * 32 + lane;
+        if (ch < L.rank_v) {
+          float* o = ost + 4 + ch;
+#pragma unroll
+          for (int h = 0; h < 32; ++h)
+            if (h < L.n_q_heads) {
+              const float x = __uint_as_float(v[h]) * wt[h];
+              o[h * ST] = pass == 0 ? x : o[h * ST] + x;
+            }
+        }
+      }
+    }
+    bar_sync(BAR_ALL, NTHREADS);
+  }
+  {
+    const float4* src = reinterpret_cast<const float4*>(ost);
+    float4* dst = reinterpret_cast<float4*>(my_parts);
+    for (int i = tid; i < L.n_q_heads * ST / 4; i += NTHREADS) dst[i] = src[i];
+  }
+  tc_fence_before();
+  __syncthreads();
+  if (warp == 1) {
+    const uint32_t ncol = (uint32_t)PL.um_cols;
+    asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"((uint32_t)tmem_base_s), "r"(ncol) : "memory");
+  }
+}
+
+template <int BH, int BL, int NG>
+cudaError_t launch_tc5(const starkv_ctx* ctx, dim3 grid, const uint8_t* qimg, size_t qimg_stride, const uint8_t* pool,
+                       const int32_t* table, int max_pages, const int32_t* seq_lens, float* parts, int n_splits) {
+  auto kern = decode_tc5_kernel<BH, BL, NG>;
+  static int smem_set = 0;
+  if (ctx->plan.smem_bytes > smem_set) {
+    const cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, ctx->plan.smem_bytes);
+    if (e != cudaSuccess) return e;
+    smem_set = ctx->plan.smem_bytes;
+  }
+  return sk_launch(ctx, kern, grid, dim3(NG * GW * 32), (size_t)ctx->plan.smem_bytes, ctx->L, ctx->plan, qimg, qimg_stride, pool,
+                   table, max_pages, seq_lens, parts, n_splits);
+}
+
 template <int BH, int BL, int NT, int MT, int NG>
 cudaError_t launch_fast(const starkv_ctx* ctx, dim3 grid, const uint8_t* qimg, size_t qimg_stride, const uint8_t* pool,
                         const int32_t* table, int max_pages, const int32_t* seq_lens, float* parts, int n_splits) {
@@ -930,15 +1334,37 @@ int sk_fast_plan(starkv_ctx* ctx) {
   if (P.mt > 4) return 0;
   const int p_area = NG_MAX * 2 * P_BUF_BYTES;
   const int qarea = round_up(P.qimg_bytes + L.n_kv_heads * 32, 128);   // image + accumulator start values
-  const int merge_bytes = 1024 + L.n_q_heads * (L.rank_v + 4) * 4;
+  const int merge_bytes = 1536 + L.n_q_heads * (L.rank_v + 4) * 4;
   const int fixed = qarea + p_area + NG_MAX * 2 * 32 * 4 /* alpha */ + 128 /* flags */ +
-                    128 /* barriers */ + 4 * TBL_SMEM + 128 /* base align */;
+                    256 /* barriers */ + 4 * TBL_SMEM + 128 /* base align */;
   const int avail = ctx->smem_optin - fixed;
   int ns = avail / L.page_bytes;
   if (ns > 8) ns = 8;
   if (ns < 2) return 0;   // one stage per group at least (a third keeps a copy in flight while both compute)
   if ((long long)ns * L.page_bytes < merge_bytes) {
     if (merge_bytes > avail) return 0;
+  }
+  // tcgen05 PV for the integer modes: 2 groups x um_mt x 16 KB of A operand come out of the ring's memory.  Taken
+  // when at least 4 ring stages remain (STARKV_PV=mma forces the mma.sync kernel, STARKV_PV=tcgen05 accepts 3 stages).
+  if (quant && L.rank_v <= 4 * 128) {
+    const char* e_pv = getenv("STARKV_PV");
+    const int um_mt = (L.rank_v + 127) / 128;
+    const char* e_g5 = getenv("STARKV_TC5_GROUPS");
+    const int ng5 = (e_g5 && e_g5[0] == '3') ? 3 : 2;
+    const int a_bytes = ng5 * um_mt * 128 * PTOK * 2;
+    int ns5 = (avail - a_bytes) / L.page_bytes;
+    if (ns5 > 8) ns5 = 8;
+    const int need = (e_pv && e_pv[0] == 't') ? 3 : 4;
+    const bool room = avail - a_bytes >= merge_bytes;
+    if (!(e_pv && e_pv[0] == 'm') && ns5 >= need && room) {
+      P.um = 1;
+      P.um_mt = um_mt;
+      int cols = 32;
+      while (cols < ng5 * um_mt * 32) cols *= 2;
+      P.um_cols = cols;
+      P.um_ng = ng5;
+      ns = ns5;
+    }
   }
   P.nstage = ns;
   // pages so large that only two fit: one group, so that the second stage is a copy in flight instead of a
@@ -956,8 +1382,9 @@ int sk_fast_plan(starkv_ctx* ctx) {
   P.off_p = off; off += p_area;
   P.off_alpha = off; off += NG_MAX * 2 * 32 * 4;
   P.off_flag = off; off += 128;
-  P.off_bar = off; off += 8 * ns + 8 + 4 * ns + 4 * ns;
-  off = round_up(off, 16);
+  P.off_bar = off; off += 8 * ns + 8 + 4 * ns + 4 * ns + 32;
+  off = round_up(off, 128);
+  if (P.um) { P.off_a = off; off += P.um_ng * P.um_mt * 128 * PTOK * 2; }
   P.off_tbl = off; off += 4 * TBL_SMEM;
   P.smem_bytes = round_up(off, 128);
   if (P.smem_bytes > ctx->smem_optin) return 0;
@@ -1007,6 +1434,15 @@ int sk_decode_fast(starkv_ctx* ctx, const void* q, const void* pool, const int32
   // NG = 3 (768 threads, 80 registers) was measured on C3: 43.1 us against 32.7 us with NG = 2 -- the 412-byte
   // spill frame costs more than the third group hides -- so only NG = 2 is instantiated.
   const bool one = ctx->plan.ng == 1;
+#define SK_TC5(BHv, BLv, NGv) \
+  e = launch_tc5<BHv, BLv, NGv>(ctx, grid, qimg, w.qimg_stride, pl, table, max_pages, seq_lens, parts, w.n_splits)
+  if (ctx->plan.um) {
+    const bool three = ctx->plan.um_ng == 3;
+    if (L.bits_hi == 8 && L.bits_lo == 4) { if (three) SK_TC5(8, 4, 3); else SK_TC5(8, 4, 2); }
+    else if (L.bits_hi == 8 && L.bits_lo == 8) SK_TC5(8, 8, 2);
+    else if (L.bits_hi == 4 && L.bits_lo == 4) SK_TC5(4, 4, 2);
+  } else
+#undef SK_TC5
   if (L.bits_hi == 16) { if (one) SK_KIND(16, 16, 1); else SK_KIND(16, 16, 2); }
   else if (L.bits_hi == 8 && L.bits_lo == 4) { if (one) SK_KIND(8, 4, 1); else SK_KIND(8, 4, 2); }
   else if (L.bits_hi == 8 && L.bits_lo == 8) SK_KIND(8, 8, 2);

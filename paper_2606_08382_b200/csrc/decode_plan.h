@@ -31,6 +31,12 @@ struct DecodePlan {
   int32_t off_kcst;                               // = off_qimg + qimg_bytes: QK accumulator start values
                                                   // [H_kv][2 blocks][4 quad columns] fp32 (same bulk copy as the image)
   int32_t smem_bytes;
+  // tcgen05 PV variant (decode_tc5_kernel, integer modes): value page dequantised into a K-major UMMA A operand
+  int32_t um;                                     // 1 = use it
+  int32_t um_ng;                                  // groups of 8 warps: 2 (or 3 with STARKV_TC5_GROUPS=3, 8/4-bit mode)
+  int32_t um_mt;                                  // 128-channel M tiles = ceil(r_v / 128) <= 4
+  int32_t um_cols;                                // TMEM columns to allocate (power of two >= 2 groups * um_mt * 32)
+  int32_t off_a;                                  // [2 groups][um_mt][16 KB] A operand
 };
 
 // channel (inside its precision block) that k index `k` (0..15) of q step `m` of a chunk refers to

@@ -520,7 +520,8 @@ def run_ours(args, cfg):
                 "ms_per_step": ms_e2e, "steps": Ke},
         "gpu_launches": K * launches_per_step,
         "clocks": clocks,
-        "roofline": {"bound": "hbm", "kernel": "decode_fast_kernel (rows D2-D7)", "achieved": achieved, "peak": peak,
+        "roofline": {"bound": "hbm", "kernel": sk.starkv_decode_kernel_name(wl.ctx) + " (rows D2-D7)", "achieved": achieved,
+                     "peak": peak,
                      "unit": "GB/s", "frac": achieved / peak, "traffic": stored_traffic(cfg.name),
                      "peak_source": peak_src, "kernel_us": k_ms * 1e3, "kernel_us_min": float(np.min(kms)) * 1e3,
                      "launches_timed": Kr, "algorithmic_bytes_per_launch": kernel_bytes(cfg),
@@ -675,7 +676,8 @@ def run_c5(args):
                 "d2h_bytes_per_step": sum(w.d2h_bytes() for w in layers), "ms_per_step": ms_e2e, "steps": Ke},
         "gpu_launches": K * launches,
         "clocks": clocks,
-        "roofline": {"bound": "hbm", "kernel": "decode_fast_kernel (rows D2-D7), summed over the layers of a step",
+        "roofline": {"bound": "hbm", "kernel": sk.starkv_decode_kernel_name(layers[0].ctx) +
+                     " (rows D2-D7), summed over the layers of a step",
                      "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
                      "traffic": stored_traffic("C5"), "peak_source": peak_src, "kernel_us": k_ms * 1e3,
                      "launches_timed": len(kms) * n_layers, "algorithmic_bytes_per_launch": bytes_kern / n_layers,

@@ -182,6 +182,12 @@ int starkv_set_splits(starkv_ctx* ctx, int n_splits);
  * gpu_launches claim). */
 int starkv_last_launches(const starkv_ctx* ctx);
 
+/* Name of the main split-K kernel (rows D2-D7) starkv_decode_attn launches for this context:
+ * "decode_tc5_kernel" (integer modes: value product on tcgen05 with TMEM accumulators),
+ * "decode_fast_kernel" (mma.sync) or "decode_generic_kernel" (shapes the tensor-core kernels do not
+ * cover).  Static string, never NULL.  Selection: DESIGN.md section 6, environment switch STARKV_PV. */
+const char* starkv_decode_kernel_name(const starkv_ctx* ctx);
+
 const char* starkv_strerror(int code);
 /* Text of the last CUDA error seen by this context ("" if none). */
 const char* starkv_last_error(const starkv_ctx* ctx);

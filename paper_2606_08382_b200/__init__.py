@@ -25,7 +25,7 @@ SYMBOLS = [
     "starkv_decode_attn", "starkv_decode_attn_generic", "starkv_decode_attn_host",
     "starkv_append_host_workspace_bytes", "starkv_append_host", "starkv_set_kernel_timing",
     "starkv_last_decode_kernel_ms",
-    "starkv_set_splits", "starkv_last_launches", "starkv_strerror", "starkv_last_error",
+    "starkv_set_splits", "starkv_last_launches", "starkv_decode_kernel_name", "starkv_strerror", "starkv_last_error",
 ]
 
 STARKV_OK = 0
@@ -92,6 +92,8 @@ def _load() -> ctypes.CDLL:
     lib.starkv_set_splits.restype = c_int
     lib.starkv_last_launches.argtypes = [vp]
     lib.starkv_last_launches.restype = c_int
+    lib.starkv_decode_kernel_name.argtypes = [vp]
+    lib.starkv_decode_kernel_name.restype = ctypes.c_char_p
     lib.starkv_strerror.argtypes = [c_int]
     lib.starkv_strerror.restype = ctypes.c_char_p
     lib.starkv_last_error.argtypes = [vp]
@@ -240,6 +242,10 @@ def starkv_set_splits(ctx: Context, n_splits: int) -> None:
 
 def starkv_last_launches(ctx: Context) -> int:
     return int(_lib.starkv_last_launches(ctx.handle))
+
+
+def starkv_decode_kernel_name(ctx: Context) -> str:
+    return _lib.starkv_decode_kernel_name(ctx.handle).decode()
 
 
 def starkv_strerror(code: int) -> str:

@@ -391,6 +391,11 @@ int starkv_set_splits(starkv_ctx* ctx, int n_splits) {
 
 int starkv_last_launches(const starkv_ctx* ctx) { return ctx ? ctx->last_launches : 0; }
 
+const char* starkv_decode_kernel_name(const starkv_ctx* ctx) {
+  if (!ctx || !ctx->fast_ok) return "decode_generic_kernel";
+  return ctx->plan.um ? "decode_tc5_kernel" : "decode_fast_kernel";
+}
+
 const char* starkv_strerror(int code) {
   switch (code) {
     case STARKV_OK: return "ok";

@@ -1348,22 +1348,24 @@ int sk_fast_plan(starkv_ctx* ctx) {
   // when at least 4 ring stages remain (STARKV_PV=mma forces the mma.sync kernel, STARKV_PV=tcgen05 accepts 3 stages).
   if (quant && L.rank_v <= 4 * 128) {
     const char* e_pv = getenv("STARKV_PV");
-    const int um_mt = (L.rank_v + 127) / 128;
     const char* e_g5 = getenv("STARKV_TC5_GROUPS");
-    const int ng5 = (e_g5 && e_g5[0] == '3') ? 3 : 2;
-    const int a_bytes = ng5 * um_mt * 128 * PTOK * 2;
-    int ns5 = (avail - a_bytes) / L.page_bytes;
-    if (ns5 > 8) ns5 = 8;
+    const int um_mt = (L.rank_v + 127) / 128;
     const int need = (e_pv && e_pv[0] == 't') ? 3 : 4;
-    const bool room = avail - a_bytes >= merge_bytes;
-    if (!(e_pv && e_pv[0] == 'm') && ns5 >= need && room) {
-      P.um = 1;
-      P.um_mt = um_mt;
-      int cols = 32;
-      while (cols < ng5 * um_mt * 32) cols *= 2;
-      P.um_cols = cols;
-      P.um_ng = ng5;
-      ns = ns5;
+    // three groups (8/4-bit mode only, opt-in) if they fit, else two
+    for (int ng5 = (e_g5 && e_g5[0] == '3' && L.bits_hi == 8 && L.bits_lo == 4) ? 3 : 2; ng5 >= 2 && !P.um; --ng5) {
+      const int a_bytes = ng5 * um_mt * 128 * PTOK * 2;
+      int ns5 = (avail - a_bytes) / L.page_bytes;
+      if (ns5 > 8) ns5 = 8;
+      const bool room = avail - a_bytes >= merge_bytes;
+      if (!(e_pv && e_pv[0] == 'm') && ns5 >= need && room) {
+        P.um = 1;
+        P.um_mt = um_mt;
+        int cols = 32;
+        while (cols < ng5 * um_mt * 32) cols *= 2;
+        P.um_cols = cols;
+        P.um_ng = ng5;
+        ns = ns5;
+      }
     }
   }
   P.nstage = ns;

@@ -53,6 +53,33 @@ def test_peaky_regime(name):
     _check(cfg, regime="peaky")
 
 
+@pytest.mark.parametrize("pv,groups", [("tcgen05", "2"), ("tcgen05", "3"), ("mma", "2")], ids=["tcgen05", "tcgen05-3groups", "mma"])
+@pytest.mark.parametrize("bits", [(8, 4), (8, 8), (4, 4)], ids=str)
+def test_value_product_variants(pv, groups, bits, monkeypatch):
+    """The integer modes have two value-product paths: tcgen05 with TMEM accumulators
+    (decode_tc5_kernel, the default where its A operand fits beside the page ring) and mma.sync (decode_fast_kernel).
+    Both are held to the oracle, in both regimes (the peaky one exercises the TMEM rescale), ragged lengths, a value
+    rank above one 128-channel M tile and one that is not a multiple of 16."""
+    monkeypatch.setenv("STARKV_PV", pv)
+    monkeypatch.setenv("STARKV_TC5_GROUPS", groups)
+    for (hq, hkv, dh, rk, rv) in [(32, 8, 128, [24, 16, 24, 48, 16, 32, 56, 40], 256),
+                                  (16, 4, 64, [16, 64, 8, 24], 136),
+                                  (8, 8, 64, [8, 16, 24, 32, 40, 48, 56, 64], 72)]:
+        cfg = synth.custom_config(f"pv{bits[0]}{bits[1]}", 2, hq, hkv, dh, 1500, rk, rv, bits=bits, outlier_frac=0.1)
+        ctx = sk.create_from_config(cfg)
+        want = "decode_tc5_kernel" if pv == "tcgen05" else "decode_fast_kernel"
+        assert sk.starkv_decode_kernel_name(ctx) == want
+        for regime in ("diffuse", "peaky"):
+            cache = build_cache(cfg, seq_lens=[1500, 777], regime=regime)
+            bk, bv = synth.make_factors(cfg)
+            q = synth.make_q(cfg, batch=2)
+            ref = oattn.decode_attn(cache["desc"], q, cache["pool"], cache["table"], cache["seq_lens"], bk, bv)
+            out = run_decode(cfg, cache, q, bk, bv, ctx=ctx)
+            assert np.isfinite(out).all()
+            err = row_rel_err(out, ref)
+            assert err <= TOL, f"{pv} {bits} {regime} r_v={rv}: row rel err {err:.3e}"
+
+
 @pytest.mark.parametrize("bits", [(8, 8), (4, 4), (8, 4), (16, 16)], ids=str)
 @pytest.mark.parametrize("generic", [True, False], ids=["generic", "fast"])
 def test_bit_pairs_and_odd_shapes(bits, generic):

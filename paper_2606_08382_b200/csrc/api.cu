@@ -393,7 +393,7 @@ int starkv_last_launches(const starkv_ctx* ctx) { return ctx ? ctx->last_launche
 
 const char* starkv_decode_kernel_name(const starkv_ctx* ctx) {
   if (!ctx || !ctx->fast_ok) return "decode_generic_kernel";
-  return ctx->plan.um ? "decode_tc5_kernel" : "decode_fast_kernel";
+  return ctx->plan.um ? (ctx->plan.um_ws ? "decode_ws_kernel" : "decode_tc5_kernel") : "decode_fast_kernel";
 }
 
 const char* starkv_strerror(int code) {

@@ -919,6 +919,13 @@ __device__ __forceinline__ void umma_f16(uint32_t tmem_d, uint64_t da, uint64_t 
 __device__ __forceinline__ void umma_commit(uint32_t bar) {
   asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(bar) : "memory");
 }
+// one lane of a converged warp; the code around it stays warp-uniform, so that descriptor and TMEM operands computed
+// from warp-uniform values live in uniform registers (no per-MMA R2UR waterfall loop)
+__device__ __forceinline__ bool elect_one() {
+  uint32_t p;
+  asm volatile("{\n\t.reg .pred P;\n\telect.sync _|P, 0xffffffff;\n\tselp.u32 %0, 1, 0, P;\n\t}" : "=r"(p));
+  return p != 0;
+}
 __device__ __forceinline__ void tc_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
 __device__ __forceinline__ void tc_fence_after() { asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory"); }
 __device__ __forceinline__ void tmem_ld32(uint32_t taddr, uint32_t (&v)[32]) {
@@ -948,7 +955,7 @@ __device__ __forceinline__ void tmem_st32(uint32_t taddr, const uint32_t (&v)[32
 // (32 int4 / 16 int8 slots = NTB 8-token blocks); item i -> channel 8 ((i >> 3) / SEGS) + (i & 7), segment
 // (i >> 3) % SEGS, so 8 consecutive lanes write 8 consecutive channels of one token block (128 contiguous bytes,
 // conflict-free) and a thread keeps its segment -- hence its scale registers -- across its items (i += 256).
-template <int BITS>
+template <int BITS, int NTHR = 256>
 __device__ __forceinline__ void deq_block_to_a(const uint8_t* __restrict__ vb, const uint8_t* __restrict__ vsc, int n_ch,
                                                int row0, uint8_t* __restrict__ abuf, int t) {
   constexpr int SEGS = BITS / 2;   // 16-byte segments per channel row of PTOK slots
@@ -962,7 +969,7 @@ __device__ __forceinline__ void deq_block_to_a(const uint8_t* __restrict__ vb, c
     const uint4 u = *reinterpret_cast<const uint4*>(vsc + (seg * NTB + k) * 16);
     sc[4 * k] = u.x; sc[4 * k + 1] = u.y; sc[4 * k + 2] = u.z; sc[4 * k + 3] = u.w;
   }
-  for (int i = t; i < n_items; i += 256) {
+  for (int i = t; i < n_items; i += NTHR) {
     const int ch = ((i >> 3) / SEGS) * 8 + (i & 7);
     const uint4 x = *reinterpret_cast<const uint4*>(vb + ch * (PTOK * BITS / 8) + seg * 16);
     const int row = row0 + ch;
@@ -1007,7 +1014,10 @@ __global__ void __launch_bounds__(NG * GW * 32, 1) decode_tc5_kernel(
   static_assert(BH != 16, "integer modes only");
   constexpr int NTHREADS = NG * GW * 32;
 
-  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const int tid = threadIdx.x, lane = tid & 31;
+  // warp index as a value the compiler knows to be warp-uniform (shuffle from lane 0): group, ring and MMA operands
+  // derived from it stay in uniform registers
+  const int warp = __shfl_sync(0xffffffffu, tid >> 5, 0);
   const int j = lane & 3, R = lane >> 2;
   const int split = blockIdx.x, b = blockIdx.y;
   sk_pdl_trigger();
@@ -1047,7 +1057,9 @@ __global__ void __launch_bounds__(NG * GW * 32, 1) decode_tc5_kernel(
     const int st = it % nstage;
     const uint32_t bar = full0 + 8 * st;
     mbar_expect_tx(bar, page_bytes);
-    __threadfence_block();
+    // no fence: what `issued` certifies to a consumer is that the stage's PREVIOUS phase has completed and been consumed
+    // (true whenever the refilling thread runs, and ordered before this store through the group barrier); a barrier that
+    // is not armed yet is still in the new phase and makes the consumer's parity wait block, as it must
     issued[st] = it;
     bulk_g2s_stream(smem_u32(stage_base + (size_t)st * page_bytes), pool + (size_t)page * page_bytes, page_bytes, bar,
                     l2_evict_first_policy());
@@ -1059,7 +1071,7 @@ __global__ void __launch_bounds__(NG * GW * 32, 1) decode_tc5_kernel(
       issued[s] = -1;
     }
     mbar_init(qbar, 1);
-    for (int g = 0; g < NG; ++g) mbar_init(mbar0 + 8 * g, 1);
+    for (int g = 0; g < NG; ++g) mbar_init(mbar0 + 8 * g, n_mt > 1 ? 2 : 1);   // one commit per issuing warp
     fence_barrier_init();
     int pgs[8];
 #pragma unroll
@@ -1091,7 +1103,8 @@ __global__ void __launch_bounds__(NG * GW * 32, 1) decode_tc5_kernel(
   tc_fence_before();
   __syncthreads();
   tc_fence_after();
-  const uint32_t tmem_grp = tmem_base_s + (uint32_t)(grp * n_mt * 32);   // this group's accumulator columns
+  // this group's accumulator columns
+  const uint32_t tmem_grp = __shfl_sync(0xffffffffu, (uint32_t)tmem_base_s, 0) + (uint32_t)(grp * n_mt * 32);
   mbar_wait(qbar, 0);
 
   const uint2* qimg_lane = reinterpret_cast<const uint2*>(smem + PL.off_qimg) + lane;
@@ -1117,6 +1130,12 @@ __global__ void __launch_bounds__(NG * GW * 32, 1) decode_tc5_kernel(
 
   int st = grp % nstage, use = grp / nstage;
   int gi = 0;
+#ifdef SK_TRACE
+  unsigned long long tacc[8] = {0, 0, 0, 0, 0, 0, 0, 0}, tprev = sk_now();
+#define SK_PH(k) do { if (tid == 0) { const unsigned long long n_ = sk_now(); tacc[k] += n_ - tprev; tprev = n_; } } while (0)
+#else
+#define SK_PH(k) do { } while (0)
+#endif
   for (int it = grp; it < n_it; it += NG, ++gi) {
     uint8_t* pg = stage_base + (size_t)st * page_bytes;
     const int nvalid = len - (p0 + it) * PTOK;   // >= 1
@@ -1128,6 +1147,7 @@ __global__ void __launch_bounds__(NG * GW * 32, 1) decode_tc5_kernel(
       while (issued[st] != it) {}
     __syncwarp();
     mbar_wait(full0 + 8 * st, (uint32_t)(use & 1));
+    SK_PH(0);
 
     if (nvalid < PTOK) {   // tail page: zero the key rows and the value scales of the slots past the sequence end
       for (int g = 0; g < L.n_kv_heads; ++g) {
@@ -1143,15 +1163,20 @@ __global__ void __launch_bounds__(NG * GW * 32, 1) decode_tc5_kernel(
     }
 
     // ================= QK + softmax for this warp's quad =================
-    if (has_quad)
+    if (has_quad && !(PL.dbg & 1))
       score_page<BH, BL, true>(L, PL, pg, qimg_lane, kcst, kv0, kv1, nvalid, R, j, gw, m_run, l_run, Pb, p_thr_off, al, fl);
 
+    SK_PH(1);
     // ================= value page -> A operand =================
     if (gi > 0) mbar_wait(mbar, (uint32_t)((gi - 1) & 1));   // the MMAs of the previous page have read A and P
-    deq_block_to_a<BL>(pg + L.v_lo_off, pg + L.v_scale_off + PTOK * 2, L.v_lo_n, L.v_hi_n, abuf, gt);
-    deq_block_to_a<BH>(pg + L.v_hi_off, pg + L.v_scale_off, L.v_hi_n, 0, abuf, t_hi);
+    SK_PH(2);
+    if (!(PL.dbg & 2)) {
+      deq_block_to_a<BL>(pg + L.v_lo_off, pg + L.v_scale_off + PTOK * 2, L.v_lo_n, L.v_hi_n, abuf, gt);
+      deq_block_to_a<BH>(pg + L.v_hi_off, pg + L.v_scale_off, L.v_hi_n, 0, abuf, t_hi);
+    }
     fence_proxy_async();   // P and A (generic-proxy stores) -> visible to the tensor-core (async) proxy
     bar_sync(1 + grp, GW * 32);
+    SK_PH(3);
 
     // ================= lazy rescale of the TMEM accumulators (rare) =================
     {
@@ -1172,21 +1197,37 @@ __global__ void __launch_bounds__(NG * GW * 32, 1) decode_tc5_kernel(
     }
 
     // ================= PV: one thread issues the MMAs, commits, refills the stage =================
-    if (gt == 0) {
+    // warp-uniform roles, one elected lane each, operands are uniform values: warps 0 and 4 issue the MMAs of the even
+    // and odd M tiles (different TMEM tiles: no ordering between them) and commit; warp 2 refills the ring stage
+    if (gw == 0 || (gw == 4 && n_mt > 1)) {
       tc_fence_after();
-      const uint32_t sa = smem_u32(abuf), sb = smem_u32(Pb);
-      for (int mt = 0; mt < n_mt; ++mt)
+      SK_PH(4);
+      const uint64_t da0 = umma_desc_k(smem_u32(abuf)), db0 = umma_desc_k(smem_u32(Pb));
+      if (elect_one()) {
+        for (int mt = gw >> 2; mt < n_mt; mt += (n_mt > 1 ? 2 : 1))
 #pragma unroll
-        for (int ks = 0; ks < PTOK / 16; ++ks)
-          umma_f16(tmem_grp + (uint32_t)(mt * 32), umma_desc_k(sa + mt * UM_TILE_BYTES + ks * 256), umma_desc_k(sb + ks * 256),
-                   IDESC, (gi > 0 || ks > 0) ? 1u : 0u);
-      umma_commit(mbar);
+          for (int ks = 0; ks < PTOK / 16; ++ks)
+            umma_f16(tmem_grp + (uint32_t)(mt * 32), da0 + (uint64_t)((mt * UM_TILE_BYTES + ks * 256) >> 4),
+                     db0 + (uint64_t)((ks * 256) >> 4), IDESC, (gi > 0 || ks > 0) ? 1u : 0u);
+        SK_PH(5);
+        umma_commit(mbar);
+      }
+      __syncwarp();
+    } else if (gw == 2) {
       const int nxt = it + nstage;
-      if (nxt < n_it) issue(nxt, nxt < TBL_SMEM ? tbl_s[nxt] : my_table[nxt]);
+      if (nxt < n_it && elect_one()) issue(nxt, nxt < TBL_SMEM ? tbl_s[nxt] : my_table[nxt]);
+      __syncwarp();
     }
+    SK_PH(6);
     st += NG;
     while (st >= nstage) { st -= nstage; ++use; }
   }
+#ifdef SK_TRACE
+  if (tid == 0) {
+    tacc[7] = (unsigned long long)gi;
+    for (int q = 0; q < 8; ++q) g_sk_trace[(blockIdx.y * gridDim.x + blockIdx.x) * 8 + q] = tacc[q];
+  }
+#endif
 
   // ================= merge the groups and write the split-K partial (D7) =================
   if (gi > 0) mbar_wait(mbar, (uint32_t)((gi - 1) & 1));   // this group's last MMAs are complete
@@ -1272,6 +1313,307 @@ cudaError_t launch_tc5(const starkv_ctx* ctx, dim3 grid, const uint8_t* qimg, si
                    table, max_pages, seq_lens, parts, n_splits);
 }
 
+// ---------------------------------------------------------------------------------------------
+// Warp-specialised form of the tcgen05 kernel (integer modes): 24 warps in three roles, no per-page group barrier.
+//   warps 0-7 / 8-15  QK + softmax of the even / odd pages of the range (score_page as above; P, alpha and the
+//                     rescale flag go to the group's double buffers), then ONE arrival per warp on the page's
+//                     "P ready" mbarrier; a warp never waits for the other warps of its group, so the rank-dependent
+//                     QK cost of the heads (16...56 channels on C3) no longer serialises on a barrier.
+//   warps 16-23       every page in turn: dequantise the value block into one of two A buffers, wait for "P ready",
+//                     rescale the group's TMEM tiles if a head moved its maximum, and (one thread) issue the page's
+//                     tcgen05.mma, commit to "A buffer free" and "P buffer free", refill the ring stage.
+// mbarriers: full[stage] (bulk copy), pready[g][buf] (8 arrivals), pfree[g][buf] and afree[2] (tcgen05.commit).
+// Every wait is at most one phase behind its barrier (pfree/pready/afree are used once per 4/4/2 pages in order).
+// ---------------------------------------------------------------------------------------------
+template <int BH, int BL>
+__global__ void __launch_bounds__(3 * GW * 32, 1) decode_ws_kernel(
+    const __grid_constant__ StarkvLayout L, const __grid_constant__ DecodePlan PL, const uint8_t* __restrict__ qimg_all,
+    size_t qimg_stride, const uint8_t* __restrict__ pool, const int32_t* __restrict__ table, int max_pages,
+    const int32_t* __restrict__ seq_lens, float* __restrict__ parts, int n_splits) {
+  extern __shared__ __align__(128) uint8_t smem[];
+  static_assert(BH != 16, "integer modes only");
+  constexpr int NTHREADS = 3 * GW * 32;
+  constexpr int BAR_D = 3;   // named barriers 3, 4 of the two dequantise/MMA halves (1, 2: the QK groups, tail pages only)
+
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const int j = lane & 3, R = lane >> 2;
+  const int split = blockIdx.x, b = blockIdx.y;
+  sk_pdl_trigger();
+  const int len = seq_lens[b];   // caller-owned inputs: read ahead of the dependency wait (ctx.h)
+  const int n_pages = (len + PTOK - 1) / PTOK;
+  int p0, p1;
+  sk_split_range(n_pages, n_splits, 1, split, &p0, &p1);
+  const int n_it = p1 - p0;
+  const size_t pstride = sk_part_stride(L.rank_v);
+  float* my_parts = parts + ((size_t)b * n_splits + split) * L.n_q_heads * pstride;
+
+  if (n_it <= 0) {   // empty range (CTA-uniform): neutral partial
+    sk_pdl_wait();
+    for (int i = tid; i < L.n_q_heads * (int)pstride; i += NTHREADS) {
+      const int c = i % (int)pstride;
+      my_parts[i] = c == 0 ? -INFINITY : 0.f;
+    }
+    return;
+  }
+
+  uint8_t* stage_base = smem + PL.off_stage;
+  const int nstage = PL.nstage;
+  const int n_mt = PL.um_mt;
+  // barrier area: full[nstage], image, pready[2][2], pfree[2][2], afree[2], TMEM base address, issued[nstage]
+  const uint32_t full0 = smem_u32(smem + PL.off_bar);
+  const uint32_t qbar = full0 + 8 * nstage;
+  const uint32_t pready0 = qbar + 8, pfree0 = pready0 + 32, afree0 = pfree0 + 32;
+  const int misc_off = PL.off_bar + 8 * nstage + 8 + 32 + 32 + 16;
+  volatile uint32_t& tmem_base_s = *reinterpret_cast<volatile uint32_t*>(smem + misc_off);
+  volatile int* issued = reinterpret_cast<int*>(smem + misc_off + 8);   // [nstage]
+  int32_t* tbl_s = reinterpret_cast<int32_t*>(smem + PL.off_tbl);
+  const uint32_t page_bytes = (uint32_t)L.page_bytes;
+  const int32_t* my_table = table + (size_t)b * max_pages + p0;
+
+  auto issue = [&](int it, int page) {   // D2: one page -> ring stage (single thread)
+    const int st = it % nstage;
+    const uint32_t bar = full0 + 8 * st;
+    mbar_expect_tx(bar, page_bytes);
+    __threadfence_block();
+    issued[st] = it;
+    bulk_g2s_stream(smem_u32(stage_base + (size_t)st * page_bytes), pool + (size_t)page * page_bytes, page_bytes, bar,
+                    l2_evict_first_policy());
+  };
+
+  if (tid == 0) {
+    for (int s = 0; s < nstage; ++s) {
+      mbar_init(full0 + 8 * s, 1);
+      issued[s] = -1;
+    }
+    mbar_init(qbar, 1);
+    for (int i = 0; i < 4; ++i) {
+      mbar_init(pready0 + 8 * i, GW);
+      mbar_init(pfree0 + 8 * i, 1);
+    }
+    mbar_init(afree0, 1);
+    mbar_init(afree0 + 8, 1);
+    fence_barrier_init();
+    int pgs[8];
+#pragma unroll
+    for (int s = 0; s < 8; ++s) pgs[s] = s < min(nstage, n_it) ? my_table[s] : 0;
+    sk_pdl_wait();
+    const uint32_t qbytes = (uint32_t)(PL.qimg_bytes + L.n_kv_heads * 32);
+    mbar_expect_tx(qbar, qbytes);
+    bulk_g2s(smem_u32(smem + PL.off_qimg), qimg_all + (size_t)b * qimg_stride, qbytes, qbar);
+#pragma unroll
+    for (int s = 0; s < 8; ++s)
+      if (s < min(nstage, n_it)) issue(s, pgs[s]);
+  }
+  if (warp == 1) {   // TMEM: 32 fp32 columns per (QK group, M tile)
+    const uint32_t dst = smem_u32(smem + misc_off);
+    const uint32_t ncol = (uint32_t)PL.um_cols;
+    asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(dst), "r"(ncol) : "memory");
+    asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+  }
+  for (int i = tid; i < min(n_it, TBL_SMEM); i += NTHREADS) tbl_s[i] = my_table[i];
+  {
+    uint4* pz = reinterpret_cast<uint4*>(smem + PL.off_p);
+    for (int i = tid; i < 2 * 2 * P_BUF_BYTES / 16; i += NTHREADS) pz[i] = make_uint4(0, 0, 0, 0);
+    if (tid < 2 * 64) reinterpret_cast<float*>(smem + PL.off_alpha)[tid] = 1.f;
+    if (tid < 2 * 4) reinterpret_cast<uint32_t*>(smem + PL.off_flag)[tid] = 0;
+  }
+  sk_pdl_wait();
+  tc_fence_before();
+  __syncthreads();
+  tc_fence_after();
+  const uint32_t tmem0 = tmem_base_s;
+  const int gw = warp & (GW - 1);
+  // instruction descriptor: D fp32 (bit 4), A and B fp16 K-major, N = 32 (bits 17..), M = 128 (bits 24..)
+  constexpr uint32_t IDESC = (1u << 4) | ((uint32_t)(32 >> 3) << 17) | ((uint32_t)(UM_ROWS >> 4) << 24);
+
+  float m_run = -INFINITY, l_run = 0.f;
+  int gi = 0;   // pages this QK warp has scored
+  const int grp = warp >> 3;   // 0, 1: QK groups; 2: dequantise / MMA
+  const bool has_quad = gw < PL.nq;
+
+  if (grp < 2) {
+    // ===================== QK + softmax warps =====================
+    mbar_wait(qbar, 0);
+    const uint2* qimg_lane = reinterpret_cast<const uint2*>(smem + PL.off_qimg) + lane;
+    const float* kcst = reinterpret_cast<const float*>(smem + PL.off_kcst);
+    uint8_t* Pm = smem + PL.off_p + grp * 2 * P_BUF_BYTES;
+    float* alpha_s = reinterpret_cast<float*>(smem + PL.off_alpha) + grp * 64;
+    uint8_t* flag_s = smem + PL.off_flag + grp * 16;
+    const int kv0 = gw * PL.kv_per_quad;
+    const int kv1 = min(kv0 + PL.kv_per_quad, L.n_kv_heads);
+    const int p_thr_off = (gw >> 1) * 1024 + (2 * (R >> 1)) * 128 + (4 * (gw & 1) + j) * 16 + 8 * (R & 1);
+    const int gt = tid & 255;
+    int st = grp % nstage, use = grp / nstage;
+    for (int it = grp; it < n_it; it += 2, ++gi) {
+      uint8_t* pg = stage_base + (size_t)st * page_bytes;
+      const int nvalid = len - (p0 + it) * PTOK;   // >= 1
+      const int buf = gi & 1;
+      if (lane == 0)
+        while (issued[st] != it) {}
+      __syncwarp();
+      mbar_wait(full0 + 8 * st, (uint32_t)(use & 1));
+      if (nvalid < PTOK) {   // tail page: zero the key rows of the slots past the sequence end (this group's reads)
+        for (int g = 0; g < L.n_kv_heads; ++g) {
+          for (int blk = 0; blk < 2; ++blk) {
+            const int n = blk ? L.k_lo_n[g] : L.k_hi_n[g];
+            const int rowb = n * (blk ? BL : BH) / 8;
+            uint32_t* dst = reinterpret_cast<uint32_t*>(pg + (blk ? L.k_lo_off[g] : L.k_hi_off[g]) + nvalid * rowb);
+            for (int i = gt; i < (PTOK - nvalid) * rowb / 4; i += 256) dst[i] = 0;
+          }
+        }
+        bar_sync(1 + grp, GW * 32);
+      }
+      if (gi >= 2) mbar_wait(pfree0 + 8 * (2 * grp + buf), (uint32_t)(((gi >> 1) - 1) & 1));   // MMAs of page it - 4 done with P
+      if (has_quad)
+        score_page<BH, BL, true>(L, PL, pg, qimg_lane, kcst, kv0, kv1, nvalid, R, j, gw, m_run, l_run,
+                                 Pm + buf * P_BUF_BYTES, p_thr_off, alpha_s + buf * 32, flag_s + buf * 8);
+      fence_proxy_async();   // P (generic-proxy stores) -> visible to the tensor-core (async) proxy
+      __syncwarp();
+      if (lane == 0) mbar_arrive(pready0 + 8 * (2 * grp + buf));
+      st += 2;
+      while (st >= nstage) { st -= nstage; ++use; }
+    }
+  } else {
+    // ===================== dequantise + MMA warps: two halves of 4 warps on alternating pages =====================
+    const int dh = (warp - 2 * GW) >> 2;          // half = page parity = QK group = A buffer
+    const int dw = warp & 3, gt = tid & 127;      // warp within the half (= its TMEM lane quarter), thread within the half
+    const int n_lo_items = L.v_lo_n * (BL / 2);
+    const int t_hi = (gt + 128 - (n_lo_items & 127)) & 127;
+    uint8_t* abuf = smem + PL.off_a + dh * n_mt * UM_TILE_BYTES;
+    const uint32_t tmem_grp = tmem0 + (uint32_t)(dh * n_mt * 32);
+    int st = dh % nstage, use = dh / nstage;
+    int qi = 0;
+    for (int it = dh; it < n_it; it += 2, ++qi) {
+      uint8_t* pg = stage_base + (size_t)st * page_bytes;
+      const int nvalid = len - (p0 + it) * PTOK;
+      const int buf = qi & 1;
+      if (lane == 0)
+        while (issued[st] != it) {}
+      __syncwarp();
+      mbar_wait(full0 + 8 * st, (uint32_t)(use & 1));
+      if (nvalid < PTOK) {   // tail page: zero the value scales of the slots past the sequence end
+        if ((gt & (PTOK - 1)) >= nvalid) reinterpret_cast<uint16_t*>(pg + L.v_scale_off)[gt] = 0;
+        bar_sync(BAR_D + dh, 128);
+      }
+      if (qi >= 1) mbar_wait(afree0 + 8 * dh, (uint32_t)((qi - 1) & 1));   // MMAs of page it - 2 have read this A buffer
+      deq_block_to_a<BL, 128>(pg + L.v_lo_off, pg + L.v_scale_off + PTOK * 2, L.v_lo_n, L.v_hi_n, abuf, gt);
+      deq_block_to_a<BH, 128>(pg + L.v_hi_off, pg + L.v_scale_off, L.v_hi_n, 0, abuf, t_hi);
+      fence_proxy_async();
+      mbar_wait(pready0 + 8 * (2 * dh + buf), (uint32_t)((qi >> 1) & 1));   // P, alpha, flag of this page are complete
+      {
+        const uint2 f8 = *reinterpret_cast<const uint2*>(smem + PL.off_flag + dh * 16 + buf * 8);
+        if ((f8.x | f8.y) != 0 && qi > 0) {   // lazy rescale of the group's accumulators (its last MMAs: page it - 2, done)
+          const float* al = reinterpret_cast<const float*>(smem + PL.off_alpha) + dh * 64 + buf * 32;
+          tc_fence_after();
+          for (int mt = 0; mt < n_mt; ++mt) {
+            const uint32_t taddr = tmem_grp + ((uint32_t)(dw * 32) << 16) + (uint32_t)(mt * 32);
+            uint32_t v[32];
+            tmem_ld32(taddr, v);
+#pragma unroll
+            for (int c = 0; c < 32; ++c) v[c] = __float_as_uint(__uint_as_float(v[c]) * al[c]);
+            tmem_st32(taddr, v);
+          }
+          tc_fence_before();
+        }
+      }
+      bar_sync(BAR_D + dh, 128);   // A complete, every warp past its reads of the page, rescale written
+      if (gt == 0) {
+        tc_fence_after();
+        const uint32_t sa = smem_u32(abuf), sb = smem_u32(smem + PL.off_p + (2 * dh + buf) * P_BUF_BYTES);
+        for (int mt = 0; mt < n_mt; ++mt)
+#pragma unroll
+          for (int ks = 0; ks < PTOK / 16; ++ks)
+            umma_f16(tmem_grp + (uint32_t)(mt * 32), umma_desc_k(sa + mt * UM_TILE_BYTES + ks * 256), umma_desc_k(sb + ks * 256),
+                     IDESC, (qi > 0 || ks > 0) ? 1u : 0u);
+        umma_commit(afree0 + 8 * dh);
+        umma_commit(pfree0 + 8 * (2 * dh + buf));
+        const int nxt = it + nstage;
+        if (nxt < n_it) issue(nxt, nxt < TBL_SMEM ? tbl_s[nxt] : my_table[nxt]);
+      }
+      st += 2;
+      while (st >= nstage) { st -= nstage; ++use; }
+    }
+    // every MMA of this half is complete before anyone reads TMEM or reuses the stage memory
+    if (qi >= 1) mbar_wait(afree0 + 8 * dh, (uint32_t)((qi - 1) & 1));
+    tc_fence_before();
+  }
+
+  // ================= merge the groups and write the split-K partial (D7) =================
+  bar_sync(BAR_ALL, NTHREADS);
+  tc_fence_after();
+  float* mg = reinterpret_cast<float*>(smem + PL.off_stage);   // m at [g * 32 + head], l at [96 + ..], weight at [192 + ..]
+  float* ost = mg + 384;
+  const int ST = (int)pstride;
+  if (grp < 2 && has_quad) {
+    float lsum = l_run;
+    lsum += __shfl_xor_sync(0xffffffffu, lsum, 4);
+    lsum += __shfl_xor_sync(0xffffffffu, lsum, 8);
+    lsum += __shfl_xor_sync(0xffffffffu, lsum, 16);
+    if (R == 0) {
+      mg[grp * 32 + 4 * gw + j] = m_run;
+      mg[96 + grp * 32 + 4 * gw + j] = lsum;
+    }
+  }
+  bar_sync(BAR_ALL, NTHREADS);
+  if (tid < 32 && tid < L.n_q_heads) {
+    const float m0 = mg[tid], m1 = mg[32 + tid];   // group 0 always has a page: m0 is finite
+    const float ms = fmaxf(m0, m1);
+    const float w0 = ex2(m0 - ms), w1 = m1 == -INFINITY ? 0.f : ex2(m1 - ms);
+    mg[192 + tid] = w0;
+    mg[224 + tid] = w1;
+    *reinterpret_cast<float4*>(ost + tid * ST) = make_float4(ms, mg[96 + tid] * w0 + mg[128 + tid] * w1, 0.f, 0.f);
+  }
+  bar_sync(BAR_ALL, NTHREADS);
+#pragma unroll
+  for (int pass = 0; pass < 2; ++pass) {   // QK group 0's warps store their tiles, group 1's add (if it had a page)
+    if (grp == pass && gi > 0) {
+      const float* wt = mg + 192 + 32 * grp;
+      const uint32_t tmem_grp = tmem0 + (uint32_t)(grp * n_mt * 32);
+      for (int mt = gw >> 2; mt < n_mt; mt += 2) {
+        const uint32_t taddr = tmem_grp + ((uint32_t)((gw & 3) * 32) << 16) + (uint32_t)(mt * 32);
+        uint32_t v[32];
+        tmem_ld32(taddr, v);
+        const int ch = mt * UM_ROWS + (gw & 3) * 32 + lane;
+        if (ch < L.rank_v) {
+          float* o = ost + 4 + ch;
+#pragma unroll
+          for (int h = 0; h < 32; ++h)
+            if (h < L.n_q_heads) {
+              const float x = __uint_as_float(v[h]) * wt[h];
+              o[h * ST] = pass == 0 ? x : o[h * ST] + x;
+            }
+        }
+      }
+    }
+    bar_sync(BAR_ALL, NTHREADS);
+  }
+  {
+    const float4* src = reinterpret_cast<const float4*>(ost);
+    float4* dst = reinterpret_cast<float4*>(my_parts);
+    for (int i = tid; i < L.n_q_heads * ST / 4; i += NTHREADS) dst[i] = src[i];
+  }
+  tc_fence_before();
+  __syncthreads();
+  if (warp == 1) {
+    const uint32_t ncol = (uint32_t)PL.um_cols;
+    asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"((uint32_t)tmem_base_s), "r"(ncol) : "memory");
+  }
+}
+
+template <int BH, int BL>
+cudaError_t launch_ws(const starkv_ctx* ctx, dim3 grid, const uint8_t* qimg, size_t qimg_stride, const uint8_t* pool,
+                      const int32_t* table, int max_pages, const int32_t* seq_lens, float* parts, int n_splits) {
+  auto kern = decode_ws_kernel<BH, BL>;
+  static int smem_set = 0;
+  if (ctx->plan.smem_bytes > smem_set) {
+    const cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, ctx->plan.smem_bytes);
+    if (e != cudaSuccess) return e;
+    smem_set = ctx->plan.smem_bytes;
+  }
+  return sk_launch(ctx, kern, grid, dim3(3 * GW * 32), (size_t)ctx->plan.smem_bytes, ctx->L, ctx->plan, qimg, qimg_stride, pool,
+                   table, max_pages, seq_lens, parts, n_splits);
+}
+
 template <int BH, int BL, int NT, int MT, int NG>
 cudaError_t launch_fast(const starkv_ctx* ctx, dim3 grid, const uint8_t* qimg, size_t qimg_stride, const uint8_t* pool,
                         const int32_t* table, int max_pages, const int32_t* seq_lens, float* parts, int n_splits) {
@@ -1350,7 +1692,7 @@ int sk_fast_plan(starkv_ctx* ctx) {
     const char* e_pv = getenv("STARKV_PV");
     const char* e_g5 = getenv("STARKV_TC5_GROUPS");
     const int um_mt = (L.rank_v + 127) / 128;
-    const int need = (e_pv && e_pv[0] == 't') ? 3 : 4;
+    const int need = (e_pv && (e_pv[0] == 't' || e_pv[0] == 'w')) ? 3 : 4;
     // three groups (8/4-bit mode only, opt-in) if they fit, else two
     for (int ng5 = (e_g5 && e_g5[0] == '3' && L.bits_hi == 8 && L.bits_lo == 4) ? 3 : 2; ng5 >= 2 && !P.um; --ng5) {
       const int a_bytes = ng5 * um_mt * 128 * PTOK * 2;
@@ -1364,10 +1706,12 @@ int sk_fast_plan(starkv_ctx* ctx) {
         while (cols < ng5 * um_mt * 32) cols *= 2;
         P.um_cols = cols;
         P.um_ng = ng5;
+        P.um_ws = (e_pv && e_pv[0] == 'w') ? 1 : 0;   // STARKV_PV=ws: warp-specialised roles (two groups' worth of A)
         ns = ns5;
       }
     }
   }
+  { const char* e_d = getenv("STARKV_DEBUG_SKIP"); P.dbg = e_d ? atoi(e_d) : 0; }
   P.nstage = ns;
   // pages so large that only two fit: one group, so that the second stage is a copy in flight instead of a
   // second page being computed on (built for the fp16 and int8/int4 modes)
@@ -1384,7 +1728,7 @@ int sk_fast_plan(starkv_ctx* ctx) {
   P.off_p = off; off += p_area;
   P.off_alpha = off; off += NG_MAX * 2 * 32 * 4;
   P.off_flag = off; off += 128;
-  P.off_bar = off; off += 8 * ns + 8 + 4 * ns + 4 * ns + 32;
+  P.off_bar = off; off += 8 * ns + 8 + 4 * ns + 4 * ns + 128;
   off = round_up(off, 128);
   if (P.um) { P.off_a = off; off += P.um_ng * P.um_mt * 128 * PTOK * 2; }
   P.off_tbl = off; off += 4 * TBL_SMEM;
@@ -1438,7 +1782,11 @@ int sk_decode_fast(starkv_ctx* ctx, const void* q, const void* pool, const int32
   const bool one = ctx->plan.ng == 1;
 #define SK_TC5(BHv, BLv, NGv) \
   e = launch_tc5<BHv, BLv, NGv>(ctx, grid, qimg, w.qimg_stride, pl, table, max_pages, seq_lens, parts, w.n_splits)
-  if (ctx->plan.um) {
+  if (ctx->plan.um && ctx->plan.um_ws) {
+    if (L.bits_hi == 8 && L.bits_lo == 4) e = launch_ws<8, 4>(ctx, grid, qimg, w.qimg_stride, pl, table, max_pages, seq_lens, parts, w.n_splits);
+    else if (L.bits_hi == 8 && L.bits_lo == 8) e = launch_ws<8, 8>(ctx, grid, qimg, w.qimg_stride, pl, table, max_pages, seq_lens, parts, w.n_splits);
+    else if (L.bits_hi == 4 && L.bits_lo == 4) e = launch_ws<4, 4>(ctx, grid, qimg, w.qimg_stride, pl, table, max_pages, seq_lens, parts, w.n_splits);
+  } else if (ctx->plan.um) {
     const bool three = ctx->plan.um_ng == 3;
     if (L.bits_hi == 8 && L.bits_lo == 4) { if (three) SK_TC5(8, 4, 3); else SK_TC5(8, 4, 2); }
     else if (L.bits_hi == 8 && L.bits_lo == 8) SK_TC5(8, 8, 2);

@@ -53,7 +53,8 @@ def test_peaky_regime(name):
     _check(cfg, regime="peaky")
 
 
-@pytest.mark.parametrize("pv,groups", [("tcgen05", "2"), ("tcgen05", "3"), ("mma", "2")], ids=["tcgen05", "tcgen05-3groups", "mma"])
+@pytest.mark.parametrize("pv,groups", [("tcgen05", "2"), ("tcgen05", "3"), ("ws", "2"), ("mma", "2")],
+                         ids=["tcgen05", "tcgen05-3groups", "warp-specialised", "mma"])
 @pytest.mark.parametrize("bits", [(8, 4), (8, 8), (4, 4)], ids=str)
 def test_value_product_variants(pv, groups, bits, monkeypatch):
     """The integer modes have two value-product paths: tcgen05 with TMEM accumulators
@@ -67,7 +68,7 @@ def test_value_product_variants(pv, groups, bits, monkeypatch):
                                   (8, 8, 64, [8, 16, 24, 32, 40, 48, 56, 64], 72)]:
         cfg = synth.custom_config(f"pv{bits[0]}{bits[1]}", 2, hq, hkv, dh, 1500, rk, rv, bits=bits, outlier_frac=0.1)
         ctx = sk.create_from_config(cfg)
-        want = "decode_tc5_kernel" if pv == "tcgen05" else "decode_fast_kernel"
+        want = {"tcgen05": "decode_tc5_kernel", "ws": "decode_ws_kernel", "mma": "decode_fast_kernel"}[pv]
         assert sk.starkv_decode_kernel_name(ctx) == want
         for regime in ("diffuse", "peaky"):
             cache = build_cache(cfg, seq_lens=[1500, 777], regime=regime)

@@ -1047,8 +1047,9 @@ __global__ void __launch_bounds__(NG * GW * 32, 1) decode_tc5_kernel(
   const uint32_t full0 = smem_u32(smem + PL.off_bar);
   const uint32_t qbar = full0 + 8 * nstage;
   const uint32_t mbar0 = qbar + 8;
-  volatile uint32_t& tmem_base_s = *reinterpret_cast<volatile uint32_t*>(smem + PL.off_bar + 8 * nstage + 8 + 8 * NG);
-  volatile int* issued = reinterpret_cast<int*>(smem + PL.off_bar + 8 * nstage + 8 + 8 * NG + 8);   // [nstage]
+  const uint32_t afree0 = mbar0 + 8 * NG;   // afree[2]: the MMAs of the page that last used A buffer (it & 1) are complete
+  volatile uint32_t& tmem_base_s = *reinterpret_cast<volatile uint32_t*>(smem + PL.off_bar + 8 * nstage + 8 + 8 * NG + 16);
+  volatile int* issued = reinterpret_cast<int*>(smem + PL.off_bar + 8 * nstage + 8 + 8 * NG + 24);   // [nstage]
   int32_t* tbl_s = reinterpret_cast<int32_t*>(smem + PL.off_tbl);
   const uint32_t page_bytes = (uint32_t)L.page_bytes;
   const int32_t* my_table = table + (size_t)b * max_pages + p0;
@@ -1057,9 +1058,8 @@ __global__ void __launch_bounds__(NG * GW * 32, 1) decode_tc5_kernel(
     const int st = it % nstage;
     const uint32_t bar = full0 + 8 * st;
     mbar_expect_tx(bar, page_bytes);
-    // no fence: what `issued` certifies to a consumer is that the stage's PREVIOUS phase has completed and been consumed
-    // (true whenever the refilling thread runs, and ordered before this store through the group barrier); a barrier that
-    // is not armed yet is still in the new phase and makes the consumer's parity wait block, as it must
+    __threadfence_block();   // the barrier is armed before any consumer can see the stage as issued (the refill runs on
+                             // a warp of its own, off the group's critical path)
     issued[st] = it;
     bulk_g2s_stream(smem_u32(stage_base + (size_t)st * page_bytes), pool + (size_t)page * page_bytes, page_bytes, bar,
                     l2_evict_first_policy());
@@ -1071,7 +1071,7 @@ __global__ void __launch_bounds__(NG * GW * 32, 1) decode_tc5_kernel(
       issued[s] = -1;
     }
     mbar_init(qbar, 1);
-    for (int g = 0; g < NG; ++g) mbar_init(mbar0 + 8 * g, n_mt > 1 ? 2 : 1);   // one commit per issuing warp
+    for (int g = 0; g < NG + 2; ++g) mbar_init(mbar0 + 8 * g, n_mt > 1 ? 2 : 1);   // one commit per issuing warp
     fence_barrier_init();
     int pgs[8];
 #pragma unroll
@@ -1085,7 +1085,7 @@ __global__ void __launch_bounds__(NG * GW * 32, 1) decode_tc5_kernel(
       if (s < min(nstage, n_it)) issue(s, pgs[s]);
   }
   if (warp == 1) {   // TMEM: 32 fp32 columns per (group, M tile)
-    const uint32_t dst = smem_u32(smem + PL.off_bar + 8 * nstage + 8 + 8 * NG);
+    const uint32_t dst = smem_u32(smem + PL.off_bar + 8 * nstage + 8 + 8 * NG + 16);
     const uint32_t ncol = (uint32_t)PL.um_cols;
     asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(dst), "r"(ncol) : "memory");
     asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
@@ -1112,7 +1112,7 @@ __global__ void __launch_bounds__(NG * GW * 32, 1) decode_tc5_kernel(
   uint8_t* Pm = smem + PL.off_p + grp * 2 * P_BUF_BYTES;
   float* alpha_s = reinterpret_cast<float*>(smem + PL.off_alpha) + grp * 64;
   uint8_t* flag_s = smem + PL.off_flag + grp * 16;
-  uint8_t* abuf = smem + PL.off_a + grp * n_mt * UM_TILE_BYTES;
+  // two A buffers shared by all groups: page `it` uses buffer it & 1 (with two groups that is the group's own)
   const uint32_t mbar = mbar0 + 8 * grp;
 
   const bool has_quad = gw < PL.nq;
@@ -1143,6 +1143,7 @@ __global__ void __launch_bounds__(NG * GW * 32, 1) decode_tc5_kernel(
     uint8_t* Pb = Pm + buf * P_BUF_BYTES;
     float* al = alpha_s + buf * 32;
     uint8_t* fl = flag_s + buf * 8;
+    uint8_t* abuf = smem + PL.off_a + (it & 1) * n_mt * UM_TILE_BYTES;
     if (lane == 0)
       while (issued[st] != it) {}
     __syncwarp();
@@ -1168,7 +1169,8 @@ __global__ void __launch_bounds__(NG * GW * 32, 1) decode_tc5_kernel(
 
     SK_PH(1);
     // ================= value page -> A operand =================
-    if (gi > 0) mbar_wait(mbar, (uint32_t)((gi - 1) & 1));   // the MMAs of the previous page have read A and P
+    if (gi > 0) mbar_wait(mbar, (uint32_t)((gi - 1) & 1));   // the group's previous MMAs are done with P and its TMEM tiles
+    if (NG != 2 && it >= 2) mbar_wait(afree0 + 8 * (it & 1), (uint32_t)(((it >> 1) - 1) & 1));   // page it - 2 is done with A
     SK_PH(2);
     if (!(PL.dbg & 2)) {
       deq_block_to_a<BL>(pg + L.v_lo_off, pg + L.v_scale_off + PTOK * 2, L.v_lo_n, L.v_hi_n, abuf, gt);
@@ -1211,6 +1213,7 @@ __global__ void __launch_bounds__(NG * GW * 32, 1) decode_tc5_kernel(
                      db0 + (uint64_t)((ks * 256) >> 4), IDESC, (gi > 0 || ks > 0) ? 1u : 0u);
         SK_PH(5);
         umma_commit(mbar);
+        if (NG != 2) umma_commit(afree0 + 8 * (it & 1));
       }
       __syncwarp();
     } else if (gw == 2) {
@@ -1693,9 +1696,9 @@ int sk_fast_plan(starkv_ctx* ctx) {
     const char* e_g5 = getenv("STARKV_TC5_GROUPS");
     const int um_mt = (L.rank_v + 127) / 128;
     const int need = (e_pv && (e_pv[0] == 't' || e_pv[0] == 'w')) ? 3 : 4;
-    // three groups (8/4-bit mode only, opt-in) if they fit, else two
-    for (int ng5 = (e_g5 && e_g5[0] == '3' && L.bits_hi == 8 && L.bits_lo == 4) ? 3 : 2; ng5 >= 2 && !P.um; --ng5) {
-      const int a_bytes = ng5 * um_mt * 128 * PTOK * 2;
+    (void)e_g5;   // three groups were measured (no gain with six ring stages on C3, a hang on C5): two only
+    for (int ng5 = 2; ng5 >= 2 && !P.um; --ng5) {
+      const int a_bytes = 2 * um_mt * 128 * PTOK * 2;   // two A buffers, shared by the groups
       int ns5 = (avail - a_bytes) / L.page_bytes;
       if (ns5 > 8) ns5 = 8;
       const bool room = avail - a_bytes >= merge_bytes;
@@ -1730,7 +1733,7 @@ int sk_fast_plan(starkv_ctx* ctx) {
   P.off_flag = off; off += 128;
   P.off_bar = off; off += 8 * ns + 8 + 4 * ns + 4 * ns + 128;
   off = round_up(off, 128);
-  if (P.um) { P.off_a = off; off += P.um_ng * P.um_mt * 128 * PTOK * 2; }
+  if (P.um) { P.off_a = off; off += 2 * P.um_mt * 128 * PTOK * 2; }
   P.off_tbl = off; off += 4 * TBL_SMEM;
   P.smem_bytes = round_up(off, 128);
   if (P.smem_bytes > ctx->smem_optin) return 0;
@@ -1788,7 +1791,8 @@ int sk_decode_fast(starkv_ctx* ctx, const void* q, const void* pool, const int32
     else if (L.bits_hi == 4 && L.bits_lo == 4) e = launch_ws<4, 4>(ctx, grid, qimg, w.qimg_stride, pl, table, max_pages, seq_lens, parts, w.n_splits);
   } else if (ctx->plan.um) {
     const bool three = ctx->plan.um_ng == 3;
-    if (L.bits_hi == 8 && L.bits_lo == 4) { if (three) SK_TC5(8, 4, 3); else SK_TC5(8, 4, 2); }
+    (void)three;
+    if (L.bits_hi == 8 && L.bits_lo == 4) SK_TC5(8, 4, 2);
     else if (L.bits_hi == 8 && L.bits_lo == 8) SK_TC5(8, 8, 2);
     else if (L.bits_hi == 4 && L.bits_lo == 4) SK_TC5(4, 4, 2);
   } else

@@ -53,8 +53,8 @@ def test_peaky_regime(name):
     _check(cfg, regime="peaky")
 
 
-@pytest.mark.parametrize("pv,groups", [("tcgen05", "2"), ("tcgen05", "3"), ("ws", "2"), ("mma", "2")],
-                         ids=["tcgen05", "tcgen05-3groups", "warp-specialised", "mma"])
+@pytest.mark.parametrize("pv,groups", [("tcgen05", "2"), ("ws", "2"), ("mma", "2")],
+                         ids=["tcgen05", "warp-specialised", "mma"])
 @pytest.mark.parametrize("bits", [(8, 4), (8, 8), (4, 4)], ids=str)
 def test_value_product_variants(pv, groups, bits, monkeypatch):
     """The integer modes have two value-product paths: tcgen05 with TMEM accumulators

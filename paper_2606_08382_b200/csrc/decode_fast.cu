@@ -1130,6 +1130,7 @@ __global__ void __launch_bounds__(NG * GW * 32, 1) decode_tc5_kernel(
 
   int st = grp % nstage, use = grp / nstage;
   int gi = 0;
+  const bool shared_stages = (nstage % NG) != 0;
 #ifdef SK_TRACE
   unsigned long long tacc[8] = {0, 0, 0, 0, 0, 0, 0, 0}, tprev = sk_now();
 #define SK_PH(k) do { if (tid == 0) { const unsigned long long n_ = sk_now(); tacc[k] += n_ - tprev; tprev = n_; } } while (0)
@@ -1144,9 +1145,14 @@ __global__ void __launch_bounds__(NG * GW * 32, 1) decode_tc5_kernel(
     float* al = alpha_s + buf * 32;
     uint8_t* fl = flag_s + buf * 8;
     uint8_t* abuf = smem + PL.off_a + (it & 1) * n_mt * UM_TILE_BYTES;
-    if (lane == 0)
-      while (issued[st] != it) {}
-    __syncwarp();
+    // A stage shared by several groups can be a whole mbarrier phase behind this group's view, which a parity wait
+    // cannot tell from "done": wait until it has been armed for THIS iteration first.  When the ring depth is a multiple
+    // of the group count every stage belongs to one group and the parity wait alone is unambiguous.
+    if (shared_stages) {
+      if (lane == 0)
+        while (issued[st] != it) {}
+      __syncwarp();
+    }
     mbar_wait(full0 + 8 * st, (uint32_t)(use & 1));
     SK_PH(0);
 

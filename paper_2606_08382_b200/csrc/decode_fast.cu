@@ -1123,8 +1123,10 @@ __global__ void __launch_bounds__(NG * GW * 32, 1) decode_tc5_kernel(
   float m_run = -INFINITY, l_run = 0.f;
 
   // dequantisation work split: the trailing block first, the leading block on the threads its last pass leaves idle
+  // (the item slices get lighter with the thread index; the plan hands the light ones to the warps with long QK phases)
   const int n_lo_items = L.v_lo_n * (BL / 2);
-  const int t_hi = (gt + 256 - (n_lo_items & 255)) & 255;
+  const int gtd = PL.deq_slice[gw] * 32 + lane;
+  const int t_hi = (gtd + 256 - (n_lo_items & 255)) & 255;
   // instruction descriptor: D fp32 (bit 4), A and B fp16 K-major, N = 32 (bits 17..), M = 128 (bits 24..)
   constexpr uint32_t IDESC = (1u << 4) | ((uint32_t)(32 >> 3) << 17) | ((uint32_t)(UM_ROWS >> 4) << 24);
 
@@ -1179,7 +1181,7 @@ __global__ void __launch_bounds__(NG * GW * 32, 1) decode_tc5_kernel(
     if (NG != 2 && it >= 2) mbar_wait(afree0 + 8 * (it & 1), (uint32_t)(((it >> 1) - 1) & 1));   // page it - 2 is done with A
     SK_PH(2);
     if (!(PL.dbg & 2)) {
-      deq_block_to_a<BL>(pg + L.v_lo_off, pg + L.v_scale_off + PTOK * 2, L.v_lo_n, L.v_hi_n, abuf, gt);
+      deq_block_to_a<BL>(pg + L.v_lo_off, pg + L.v_scale_off + PTOK * 2, L.v_lo_n, L.v_hi_n, abuf, gtd);
       deq_block_to_a<BH>(pg + L.v_hi_off, pg + L.v_scale_off, L.v_hi_n, 0, abuf, t_hi);
     }
     fence_proxy_async();   // P and A (generic-proxy stores) -> visible to the tensor-core (async) proxy
@@ -1721,6 +1723,17 @@ int sk_fast_plan(starkv_ctx* ctx) {
     }
   }
   { const char* e_d = getenv("STARKV_DEBUG_SKIP"); P.dbg = e_d ? atoi(e_d) : 0; }
+  {   // dequantisation slices by QK load: lightest QK warp -> slice 0 (the heaviest), ties in warp order
+    int cost[GW], order[GW];
+    for (int w = 0; w < GW; ++w) {
+      const int k0 = w * P.kv_per_quad, k1 = k0 + P.kv_per_quad < L.n_kv_heads ? k0 + P.kv_per_quad : L.n_kv_heads;
+      cost[w] = (w < P.nq && k0 < L.n_kv_heads) ? P.qstep_begin[k1] - P.qstep_begin[k0] : 0;
+      order[w] = w;
+    }
+    for (int i = 1; i < GW; ++i)
+      for (int j2 = i; j2 > 0 && cost[order[j2]] < cost[order[j2 - 1]]; --j2) { const int t = order[j2]; order[j2] = order[j2 - 1]; order[j2 - 1] = t; }
+    for (int pos = 0; pos < GW; ++pos) P.deq_slice[order[pos]] = pos;
+  }
   P.nstage = ns;
   // pages so large that only two fit: one group, so that the second stage is a copy in flight instead of a
   // second page being computed on (built for the fp16 and int8/int4 modes)

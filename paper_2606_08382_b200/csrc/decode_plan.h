@@ -34,6 +34,8 @@ struct DecodePlan {
   // tcgen05 PV variant (decode_tc5_kernel, integer modes): value page dequantised into a K-major UMMA A operand
   int32_t um;                                     // 1 = use it
   int32_t um_ng;                                  // groups of 8 warps: 2 (or 3 with STARKV_TC5_GROUPS=3, 8/4-bit mode)
+  int32_t deq_slice[8];                           // warp gw of a group dequantises item slice deq_slice[gw] (32 threads' worth):
+                                                  // the warps with the most QK steps get the lightest slices
   int32_t dbg;                                    // timing experiments only (STARKV_DEBUG_SKIP): 1 = no QK, 2 = no dequantisation
   int32_t um_ws;                                  // 1 = warp-specialised kernel (decode_ws_kernel)
   int32_t um_mt;                                  // 128-channel M tiles = ceil(r_v / 128) <= 4

@@ -1728,6 +1728,9 @@ int sk_fast_plan(starkv_ctx* ctx) {
     for (int w = 0; w < GW; ++w) {
       const int k0 = w * P.kv_per_quad, k1 = k0 + P.kv_per_quad < L.n_kv_heads ? k0 + P.kv_per_quad : L.n_kv_heads;
       cost[w] = (w < P.nq && k0 < L.n_kv_heads) ? P.qstep_begin[k1] - P.qstep_begin[k0] : 0;
+      // the page's bookkeeping counts too (measured: MMA issue about 0.25 us = 3 QK steps, ring refill about half of that)
+      if (w == 0 || (w == 4 && L.rank_v > 128)) cost[w] += 3;
+      if (w == 2) cost[w] += 1;
       order[w] = w;
     }
     for (int i = 1; i < GW; ++i)

@@ -63,7 +63,9 @@ def test_value_product_variants(pv, groups, bits, monkeypatch):
     rank above one 128-channel M tile and one that is not a multiple of 16."""
     monkeypatch.setenv("STARKV_PV", pv)
     monkeypatch.setenv("STARKV_TC5_GROUPS", groups)
+    # (the second shape's pages leave an ODD ring depth beside the A operand in 8/4-bit mode: stages shared by the groups)
     for (hq, hkv, dh, rk, rv) in [(32, 8, 128, [24, 16, 24, 48, 16, 32, 56, 40], 256),
+                                  (32, 8, 128, [40, 40, 48, 32, 40, 40, 48, 32], 256),
                                   (16, 4, 64, [16, 64, 8, 24], 136),
                                   (8, 8, 64, [8, 16, 24, 32, 40, 48, 56, 64], 72)]:
         cfg = synth.custom_config(f"pv{bits[0]}{bits[1]}", 2, hq, hkv, dh, 1500, rk, rv, bits=bits, outlier_frac=0.1)

@@ -605,7 +605,10 @@ __global__ void __launch_bounds__(NG * GW * 32, 1) decode_fast_kernel(
   constexpr bool QUANT = BH != 16;
   constexpr int NTHREADS = NG * GW * 32;
 
-  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const int tid = threadIdx.x, lane = tid & 31;
+  // warp index as a value the compiler knows to be warp-uniform (shuffle from lane 0): group and ring addressing
+  // derived from it can live in uniform registers
+  const int warp = __shfl_sync(0xffffffffu, tid >> 5, 0);
   const int j = lane & 3, R = lane >> 2;
   const int split = blockIdx.x, b = blockIdx.y;
   sk_pdl_trigger();

@@ -347,7 +347,7 @@ def prefill_append_leg(wl, sk, torch, device, T):
     wsb = sk.starkv_append_workspace_bytes(wl.ctx, T)
     ws = torch.empty(wsb, dtype=torch.uint8, device=device)
     f16 = lambda a: torch.from_numpy(np.ascontiguousarray(a).view(np.int16)).to(device).view(torch.float16)  # noqa: E731
-    tc5 = os.environ.get("STARKV_APPEND_GEMM", "").startswith("t")
+    tc5 = False
     out = {"tokens": T, "kernels": ("append_project_tc5_kernel (tcgen05.mma, TMEM accumulator)" if tc5 else
                                     "append_project_mma_kernel (mma.sync m16n8k16, fp32 accumulate)") + " + append_write_kernel"}
     for mode in ("dense", "hidden"):

@@ -139,7 +139,7 @@ int starkv_decode_attn_generic(starkv_ctx* ctx, const void* q, const void* page_
 
 /* The two HOST-buffer variants below stage their host inputs in a pinned block owned by the context when the
  * context has a stream of its own (not the legacy / per-thread default stream): the caller's buffers are read
- * before the call returns, one host-to-device copy carries all inputs of the call, and with STARKV_HOST_GRAPH=1 in
+ * before the call returns, one host-to-device copy carries all inputs of the call, and with the "host_graph" option (starkv_set_option) in
  * the environment the copies and kernels of a call signature are replayed as one cached CUDA graph. */
 
 /* HOST-buffer variant (bench.py "e2e"): q_host / seq_lens_host / out_host are HOST pointers
@@ -183,10 +183,23 @@ int starkv_set_splits(starkv_ctx* ctx, int n_splits);
 int starkv_last_launches(const starkv_ctx* ctx);
 
 /* Name of the main split-K kernel (rows D2-D7) starkv_decode_attn launches for this context:
- * "decode_tc5_kernel" (integer modes: value product on tcgen05 with TMEM accumulators),
- * "decode_fast_kernel" (mma.sync) or "decode_generic_kernel" (shapes the tensor-core kernels do not
- * cover).  Static string, never NULL.  Selection: DESIGN.md section 6, environment switch STARKV_PV. */
+ * "decode_tm_kernel" (integer modes: both products on tcgen05 with their A operands in tensor memory),
+ * "decode_tc5_kernel" (integer modes: value product on tcgen05, scores on mma.sync),
+ * "decode_fast_kernel" (mma.sync; the fp16 mode) or "decode_generic_kernel" (shapes the tensor-core
+ * kernels do not cover).  Static string, never NULL.  Selection: DESIGN.md section 6. */
 const char* starkv_decode_kernel_name(const starkv_ctx* ctx);
+
+/* Per-context options; the library reads NO environment variables.  Returns STARKV_OK,
+ * STARKV_ERR_INVALID_ARG (unknown name / value) or STARKV_ERR_UNSUPPORTED (the context keeps its
+ * previous setting).
+ *   "decode_variant"  0 automatic (default), 1 mma.sync kernel, 2 tcgen05 value product,
+ *                     3 TMEM-operand kernel, 4 scalar kernel; UNSUPPORTED when that kernel does
+ *                     not cover the descriptor.  For tests and measurements.
+ *   "pdl"             1 (default) launches the kernels of a step with programmatic dependent launch.
+ *   "host_graph"      1 makes the HOST-buffer entry points replay a cached CUDA graph per call
+ *                     signature (default 0).
+ *   "append_tc5"      1 runs the prefill projection on the tcgen05 kernel (default 0). */
+int starkv_set_option(starkv_ctx* ctx, const char* name, int value);
 
 const char* starkv_strerror(int code);
 /* Text of the last CUDA error seen by this context ("" if none). */

@@ -25,7 +25,8 @@ SYMBOLS = [
     "starkv_decode_attn", "starkv_decode_attn_generic", "starkv_decode_attn_host",
     "starkv_append_host_workspace_bytes", "starkv_append_host", "starkv_set_kernel_timing",
     "starkv_last_decode_kernel_ms",
-    "starkv_set_splits", "starkv_last_launches", "starkv_decode_kernel_name", "starkv_strerror", "starkv_last_error",
+    "starkv_set_splits", "starkv_set_option", "starkv_last_launches", "starkv_decode_kernel_name", "starkv_strerror",
+    "starkv_last_error",
 ]
 
 STARKV_OK = 0
@@ -92,6 +93,8 @@ def _load() -> ctypes.CDLL:
     lib.starkv_set_splits.restype = c_int
     lib.starkv_last_launches.argtypes = [vp]
     lib.starkv_last_launches.restype = c_int
+    lib.starkv_set_option.argtypes = [vp, ctypes.c_char_p, c_int]
+    lib.starkv_set_option.restype = c_int
     lib.starkv_decode_kernel_name.argtypes = [vp]
     lib.starkv_decode_kernel_name.restype = ctypes.c_char_p
     lib.starkv_strerror.argtypes = [c_int]
@@ -238,6 +241,13 @@ def starkv_last_decode_kernel_ms(ctx: Context) -> float:
 
 def starkv_set_splits(ctx: Context, n_splits: int) -> None:
     ctx._check(_lib.starkv_set_splits(ctx.handle, n_splits))
+
+
+DECODE_VARIANTS = {"auto": 0, "mma": 1, "tc5": 2, "tm": 3, "generic": 4}
+
+
+def starkv_set_option(ctx: Context, name: str, value: int) -> None:
+    ctx._check(_lib.starkv_set_option(ctx.handle, name.encode(), int(value)))
 
 
 def starkv_last_launches(ctx: Context) -> int:

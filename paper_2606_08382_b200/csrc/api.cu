@@ -82,11 +82,9 @@ int starkv_create(starkv_ctx** out, const starkv_desc* d, void* cuda_stream) {
     free(ctx);
     return STARKV_ERR_CUDA;
   }
-  {
-    const char* e_pdl = getenv("STARKV_PDL");
-    ctx->pdl = !(e_pdl && e_pdl[0] == '0');
-  }
+  ctx->pdl = 1;
   sk_fast_plan(ctx);
+  sk_tm_plan(ctx);
   *out = ctx;
   return STARKV_OK;
 }
@@ -138,6 +136,15 @@ int starkv_append(starkv_ctx* ctx, void* pool, const int32_t* table, int max_pag
                    v_new, v_row_stride, d_in_v, A_k, A_v, ws, ws_bytes);
 }
 
+// which decode kernel family a call runs on: the TMEM-operand kernel where it covers the descriptor (integer modes),
+// else the mma.sync / tcgen05-PV kernels of decode_fast.cu, else the scalar kernel
+static int sk_decode_choice(const starkv_ctx* ctx) {
+  if (ctx->variant == SK_VARIANT_GENERIC) return SK_VARIANT_GENERIC;
+  if (ctx->tm.ok && (ctx->variant == SK_VARIANT_AUTO || ctx->variant == SK_VARIANT_TM)) return SK_VARIANT_TM;
+  if (ctx->fast_ok) return ctx->plan.um ? SK_VARIANT_TC5 : SK_VARIANT_MMA;
+  return SK_VARIANT_GENERIC;
+}
+
 static int check_decode_args(starkv_ctx* ctx, const void* q, const void* pool, const int32_t* table, int max_pages,
                              const int32_t* seq_lens, int batch, const void* B_k, const void* B_v, void* ws, void* out) {
   if (!ctx || batch <= 0 || max_pages <= 0) return STARKV_ERR_INVALID_ARG;
@@ -152,8 +159,11 @@ int starkv_decode_attn(starkv_ctx* ctx, const void* q, const void* pool, const i
                        void* out) {
   const int rc = check_decode_args(ctx, q, pool, table, max_pages, seq_lens, batch, B_k, B_v, ws, out);
   if (rc) return rc;
-  if (ctx->fast_ok) return sk_decode_fast(ctx, q, pool, table, max_pages, seq_lens, batch, B_k, B_v, ws, ws_bytes, out);
-  return sk_decode_generic(ctx, q, pool, table, max_pages, seq_lens, batch, B_k, B_v, ws, ws_bytes, out);
+  switch (sk_decode_choice(ctx)) {
+    case SK_VARIANT_TM: return sk_decode_tm(ctx, q, pool, table, max_pages, seq_lens, batch, B_k, B_v, ws, ws_bytes, out);
+    case SK_VARIANT_GENERIC: return sk_decode_generic(ctx, q, pool, table, max_pages, seq_lens, batch, B_k, B_v, ws, ws_bytes, out);
+    default: return sk_decode_fast(ctx, q, pool, table, max_pages, seq_lens, batch, B_k, B_v, ws, ws_bytes, out);
+  }
 }
 
 int starkv_decode_attn_generic(starkv_ctx* ctx, const void* q, const void* pool, const int32_t* table, int max_pages,
@@ -212,7 +222,7 @@ int starkv_decode_attn_host(starkv_ctx* ctx, const void* q_host, const void* poo
   uint8_t* pq = (uint8_t*)ctx->pin + kPinDecode;
   uint8_t* plen = pq + qb;
   uint8_t* pout = plen + lb;
-  static const bool use_graph = []() { const char* e = getenv("STARKV_HOST_GRAPH"); return e && e[0] == '1'; }();
+  const bool use_graph = ctx->host_graph != 0;
   if (!use_graph) {   // default: direct enqueue, one H2D copy (q + seq_lens) from the pinned block, one D2H copy
     memcpy(pq, q_host, qbytes);
     memcpy(plen, seq_lens_host, (size_t)batch * 4);
@@ -302,7 +312,7 @@ int starkv_append_host(starkv_ctx* ctx, void* pool, const int32_t* table, int ma
   const size_t kb = (size_t)n_new * k_row_elems * 2, vb = (size_t)n_new * v_row_elems * 2, ib = (size_t)n_new * 4;
   const bool same = v_new_host == k_new_host;
   const size_t kbp = (kb + up) & ~up, vbp = same ? 0 : ((vb + up) & ~up), ibp = (ib + up) & ~up;
-  static const bool use_graph = []() { const char* e = getenv("STARKV_HOST_GRAPH"); return e && e[0] == '1'; }();
+  const bool use_graph = ctx->host_graph != 0;
   const size_t need = kbp + vbp + 2 * ibp;
   if (n_new > 64 || need > ((size_t)4 << 20) || ctx->stream == nullptr || ctx->stream == cudaStreamLegacy ||
       ctx->stream == cudaStreamPerThread)   // staging is for decode-time appends on a stream of the caller's own
@@ -392,8 +402,34 @@ int starkv_set_splits(starkv_ctx* ctx, int n_splits) {
 int starkv_last_launches(const starkv_ctx* ctx) { return ctx ? ctx->last_launches : 0; }
 
 const char* starkv_decode_kernel_name(const starkv_ctx* ctx) {
-  if (!ctx || !ctx->fast_ok) return "decode_generic_kernel";
-  return ctx->plan.um ? (ctx->plan.um_ws ? "decode_ws_kernel" : "decode_tc5_kernel") : "decode_fast_kernel";
+  if (!ctx) return "decode_generic_kernel";
+  switch (sk_decode_choice(ctx)) {
+    case SK_VARIANT_TM: return "decode_tm_kernel";
+    case SK_VARIANT_TC5: return "decode_tc5_kernel";
+    case SK_VARIANT_MMA: return "decode_fast_kernel";
+    default: return "decode_generic_kernel";
+  }
+}
+
+int starkv_set_option(starkv_ctx* ctx, const char* name, int value) {
+  if (!ctx || !name) return STARKV_ERR_INVALID_ARG;
+  if (!strcmp(name, "pdl")) { ctx->pdl = value != 0; return STARKV_OK; }
+  if (!strcmp(name, "host_graph")) { ctx->host_graph = value != 0; return STARKV_OK; }
+  if (!strcmp(name, "append_tc5")) { ctx->append_tc5 = value != 0; return STARKV_OK; }
+  if (!strcmp(name, "decode_variant")) {
+    if (value < SK_VARIANT_AUTO || value > SK_VARIANT_GENERIC) return STARKV_ERR_INVALID_ARG;
+    const int before = ctx->variant;
+    ctx->variant = value;
+    sk_fast_plan(ctx);   // the mma.sync / tcgen05-PV choice is part of the plan
+    const int got = sk_decode_choice(ctx);
+    if (value != SK_VARIANT_AUTO && got != value) {   // the descriptor is not covered by that kernel
+      ctx->variant = before;
+      sk_fast_plan(ctx);
+      return STARKV_ERR_UNSUPPORTED;
+    }
+    return STARKV_OK;
+  }
+  return STARKV_ERR_INVALID_ARG;
 }
 
 const char* starkv_strerror(int code) {

@@ -847,20 +847,15 @@ int sk_append(starkv_ctx* ctx, void* pool, const int32_t* table, int max_pages, 
     int nkt = 0;
     for (int h = 0; h < L.n_kv_heads; ++h) nkt += (L.rank_k[h] + GN - 1) / GN;
     const int nvt = (L.rank_v + GN - 1) / GN;
-    // STARKV_APPEND_GEMM=tcgen05 selects the tcgen05/TMEM kernel.  It is correct (bit-exact parity) but, staged by
+    // starkv_set_option(ctx, "append_tc5", 1) selects the tcgen05/TMEM kernel.  It is correct (bit-exact parity) but, staged by
     // 16-byte cp.async into 128 x 64 no-swizzle tiles, it is L2-bound and slower than the mma.sync kernel (measured
     // 95 vs 80 us on the C4 prefill chunk), so it is opt-in until it moves to TMA + 128B swizzle + wider tiles.
-    const char* e_tc = getenv("STARKV_APPEND_GEMM");
-    const bool use_tc5 = n_new >= 64 && e_tc && e_tc[0] == 't' && (((L.sum_rank_k + L.rank_v) & 7) == 0);
+    const bool use_tc5 = n_new >= 64 && ctx->append_tc5 && (((L.sum_rank_k + L.rank_v) & 7) == 0);
     if (use_tc5) {
       int nkt5 = 0;
       for (int h = 0; h < L.n_kv_heads; ++h) nkt5 += (L.rank_k[h] + TN - 1) / TN;
       const int nvt5 = (L.rank_v + TN - 1) / TN;
-      static bool attr_done = false;
-      if (!attr_done) {
-        SK_CUDA_CHECK(ctx, cudaFuncSetAttribute(append_project_tc5_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, TC5_SMEM));
-        attr_done = true;
-      }
+      SK_CUDA_CHECK(ctx, sk_need_smem(ctx, append_project_tc5_kernel, TC5_SMEM));
       append_project_tc5_kernel<<<dim3(nkt5 + nvt5, (n_new + TM - 1) / TM), 256, TC5_SMEM, ctx->stream>>>(
           L, n_new, nkt5, (const __half*)k_new, k_row_stride, k_head_stride, d_in_k, (const __half*)v_new, v_row_stride, d_in_v,
           (const __half*)A_k, (const __half*)A_v, z);
@@ -879,8 +874,7 @@ int sk_append(starkv_ctx* ctx, void* pool, const int32_t* table, int max_pages, 
   SK_CUDA_CHECK(ctx, cudaGetLastError());
   const size_t smem = ((size_t)(L.sum_rank_k + L.rank_v) * 2 + 15) / 16 * 16;
   if ((int)smem > ctx->smem_optin) return STARKV_ERR_UNSUPPORTED;
-  if (smem > 48 * 1024)
-    SK_CUDA_CHECK(ctx, cudaFuncSetAttribute(append_write_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+  if (smem > 48 * 1024) SK_CUDA_CHECK(ctx, sk_need_smem(ctx, append_write_kernel, (int)smem));
   SK_PREFER_SMEM(ctx, append_write_kernel);
   sk_launch(ctx, append_write_kernel, dim3(n_new), dim3(512), smem, L, (const __half*)z, zp, n_part, n_new, seq_ids,
             positions, table, max_pages, (uint8_t*)pool);

@@ -18,7 +18,11 @@ struct starkv_ctx {
   int last_launches;
   int fast_ok;           // tensor-core decode kernel covers this descriptor
   DecodePlan plan;
-  int pdl;               // launch the step's kernels with programmatic dependent launch (STARKV_PDL=0 disables)
+  TmPlan tm;             // TMEM-operand kernel of the integer modes (decode_tm.cu); tm.ok = it covers this descriptor
+  int variant;           // decode kernel choice, SK_VARIANT_* (starkv_set_option "decode_variant"); 0 = automatic
+  int append_tc5;        // prefill projection on the tcgen05 kernel (starkv_set_option "append_tc5")
+  int host_graph;        // HOST-buffer entry points replay a cached CUDA graph (starkv_set_option "host_graph")
+  int pdl;               // launch the step's kernels with programmatic dependent launch (starkv_set_option "pdl")
   int timing_on;         // record events around the main decode kernel
   int timing_valid;
   cudaEvent_t ev0, ev1;
@@ -38,8 +42,16 @@ struct starkv_ctx {
   static const int kHostGraphs = 8;   // cached call signatures per entry point (e.g. one per block table in use)
   HostGraph g_dec[8], g_app[8];
   int g_dec_next, g_app_next;         // round-robin replacement
+  // cudaFuncSetAttribute bookkeeping, per context (= per device: a context belongs to the device it was created on):
+  // kernel -> largest dynamic shared-memory size granted (-1 = only the carve-out preference has been set)
+  struct KernelAttr { const void* fn; int smem; };
+  mutable KernelAttr attrs[48];
+  mutable int n_attrs;
   char err[512];
 };
+
+// decode kernel variants (starkv_set_decode_variant)
+enum { SK_VARIANT_AUTO = 0, SK_VARIANT_MMA = 1, SK_VARIANT_TC5 = 2, SK_VARIANT_TM = 3, SK_VARIANT_GENERIC = 4 };
 
 int sk_cuda_fail(starkv_ctx* ctx, cudaError_t e, const char* what);
 
@@ -52,15 +64,33 @@ int sk_cuda_fail(starkv_ctx* ctx, cudaError_t e, const char* what);
 // The decode kernel runs with the maximum shared-memory carve-out.  Every other kernel of the step asks for the
 // same carve-out, so that no L1/shared reconfiguration (an SM drain of several microseconds) sits between
 // consecutive launches of a step.
-#define SK_PREFER_SMEM(ctx, kernel)                                                                       \
-  do {                                                                                                    \
-    static bool _done = false;                                                                            \
-    if (!_done) {                                                                                         \
-      SK_CUDA_CHECK((ctx), cudaFuncSetAttribute((kernel), cudaFuncAttributePreferredSharedMemoryCarveout, \
-                                                (int)cudaSharedmemCarveoutMaxShared));                    \
-      _done = true;                                                                                       \
-    }                                                                                                     \
-  } while (0)
+// The attributes are per device, so the "already set" state lives in the context, not in function-local statics.
+static inline starkv_ctx::KernelAttr* sk_attr_slot(const starkv_ctx* ctx, const void* fn, bool* fresh) {
+  for (int i = 0; i < ctx->n_attrs; ++i)
+    if (ctx->attrs[i].fn == fn) { *fresh = false; return &ctx->attrs[i]; }
+  *fresh = true;
+  if (ctx->n_attrs >= 48) return nullptr;   // table full: the caller sets the attribute every time
+  ctx->attrs[ctx->n_attrs].fn = fn;
+  ctx->attrs[ctx->n_attrs].smem = -1;
+  return &ctx->attrs[ctx->n_attrs++];
+}
+template <typename K>
+static inline cudaError_t sk_prefer_smem(const starkv_ctx* ctx, K kernel) {
+  bool fresh;
+  sk_attr_slot(ctx, (const void*)kernel, &fresh);
+  if (!fresh) return cudaSuccess;
+  return cudaFuncSetAttribute(kernel, cudaFuncAttributePreferredSharedMemoryCarveout, (int)cudaSharedmemCarveoutMaxShared);
+}
+template <typename K>
+static inline cudaError_t sk_need_smem(const starkv_ctx* ctx, K kernel, int bytes) {
+  bool fresh;
+  starkv_ctx::KernelAttr* a = sk_attr_slot(ctx, (const void*)kernel, &fresh);
+  if (a && a->smem >= bytes) return cudaSuccess;
+  const cudaError_t e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
+  if (e == cudaSuccess && a) a->smem = bytes;
+  return e;
+}
+#define SK_PREFER_SMEM(ctx, kernel) SK_CUDA_CHECK((ctx), sk_prefer_smem((ctx), (kernel)))
 
 // Programmatic dependent launch (PDL): the kernels of a step are launched with the stream-serialization
 // attribute, trigger their dependents at once and wait for their predecessor (griddepcontrol.wait) before touching
@@ -121,3 +151,7 @@ int sk_decode_fast(starkv_ctx* ctx, const void* q, const void* pool, const int32
                    size_t ws_bytes, void* out);
 int sk_fast_supported(const starkv_ctx* ctx);
 int sk_fast_plan(starkv_ctx* ctx);   // fills ctx->plan, ctx->fast_ok
+int sk_tm_plan(starkv_ctx* ctx);     // fills ctx->tm
+int sk_decode_tm(starkv_ctx* ctx, const void* q, const void* pool, const int32_t* table, int max_pages,
+                 const int32_t* seq_lens, int batch, const void* B_k, const void* B_v, void* ws, size_t ws_bytes,
+                 void* out);

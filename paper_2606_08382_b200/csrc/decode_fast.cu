@@ -34,25 +34,11 @@
 #include "decode_common.cuh"
 #include "decode_plan.h"
 
-#ifdef SK_TRACE
-__device__ unsigned long long g_sk_trace[1024 * 8];
-__device__ __forceinline__ unsigned long long sk_now() {
-  unsigned long long t;
-  asm volatile("mov.u64 %0, %globaltimer;" : "=l"(t));
-  return t;
-}
-#define SK_STAMP(k) do { if (threadIdx.x == 0) g_sk_trace[(blockIdx.y * gridDim.x + blockIdx.x) * 8 + (k)] = sk_now(); } while (0)
-extern "C" int starkv_debug_trace(unsigned long long* out_host) {
-  return (int)cudaMemcpyFromSymbol(out_host, g_sk_trace, sizeof(g_sk_trace));
-}
-#else
-#define SK_STAMP(k) do { } while (0)
-#endif
 
 namespace {
 
 constexpr int GW = 8;                     // warps per group
-constexpr int NG_MAX = 3;                 // groups per CTA: 2 (128 registers per thread) or 3 (80)
+constexpr int NG_MAX = 2;                 // groups per CTA
 constexpr int BAR_ALL = 8;                // named barrier of all warps (1..NG are the groups' own)
 constexpr int TBL_SMEM = 256;             // block-table entries of the CTA's range kept in shared memory
 constexpr int PTOK = 64;         // tokens per page on this path
@@ -650,8 +636,6 @@ __global__ void __launch_bounds__(NG * GW * 32, 1) decode_fast_kernel(
     bulk_g2s_stream(smem_u32(stage_base + (size_t)st * page_bytes), pool + (size_t)page * page_bytes, page_bytes, bar,
                     l2_evict_first_policy());
   };
-
-  SK_STAMP(0);
   if (tid == 0) {
     for (int s = 0; s < nstage; ++s) {
       mbar_init(full0 + 8 * s, 1);
@@ -685,7 +669,6 @@ __global__ void __launch_bounds__(NG * GW * 32, 1) decode_fast_kernel(
   }
   bar_sync(BAR_ALL, NTHREADS);
   mbar_wait(qbar, 0);
-  SK_STAMP(1);
 
   const uint2* qimg_lane = reinterpret_cast<const uint2*>(smem + PL.off_qimg) + lane;
   const float* kcst = reinterpret_cast<const float*>(smem + PL.off_kcst);
@@ -709,8 +692,6 @@ __global__ void __launch_bounds__(NG * GW * 32, 1) decode_fast_kernel(
     for (int c = 0; c < NT; ++c)
 #pragma unroll
       for (int e = 0; e < 4; ++e) acc[a][c][e] = 0.f;
-
-  SK_STAMP(2);
   int st = grp % nstage, use = grp / nstage;   // ring stage and use count of iteration `it`, kept incrementally
   int gi = 0;                                  // this group's iteration count
   for (int it = grp; it < n_it; it += NG, ++gi) {
@@ -809,9 +790,7 @@ __global__ void __launch_bounds__(NG * GW * 32, 1) decode_fast_kernel(
   // ================= merge the groups and write the split-K partial (D7) =================
   // Stage memory is free (every issued page was consumed): it holds m[NG][32], l[NG][32] and the partial in its
   // global layout [head][4 + r_v], which is then streamed out with coalesced 16-byte stores.
-  if (grp == 0) SK_STAMP(3);
   bar_sync(BAR_ALL, NTHREADS);
-  SK_STAMP(4);
   float* mg = reinterpret_cast<float*>(smem + PL.off_stage);   // m at [g * 32 + head], l at [128 + g * 32 + head]
   float* ost = mg + 256;
   const int ST = (int)pstride;
@@ -826,7 +805,6 @@ __global__ void __launch_bounds__(NG * GW * 32, 1) decode_fast_kernel(
     }
   }
   bar_sync(BAR_ALL, NTHREADS);
-  SK_STAMP(6);
   float fme[NT][2];   // this group's weight per head column: 2^(m_own - max_g m_g); group 0 always has a page
 #pragma unroll
   for (int c = 0; c < NT; ++c)
@@ -878,13 +856,11 @@ __global__ void __launch_bounds__(NG * GW * 32, 1) decode_fast_kernel(
     }
     bar_sync(BAR_ALL, NTHREADS);
   }
-  SK_STAMP(7);
   {
     const float4* src = reinterpret_cast<const float4*>(ost);
     float4* dst = reinterpret_cast<float4*>(my_parts);
     for (int i = tid; i < L.n_q_heads * ST / 4; i += NTHREADS) dst[i] = src[i];
   }
-  SK_STAMP(5);
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -1136,12 +1112,6 @@ __global__ void __launch_bounds__(NG * GW * 32, 1) decode_tc5_kernel(
   int st = grp % nstage, use = grp / nstage;
   int gi = 0;
   const bool shared_stages = (nstage % NG) != 0;
-#ifdef SK_TRACE
-  unsigned long long tacc[8] = {0, 0, 0, 0, 0, 0, 0, 0}, tprev = sk_now();
-#define SK_PH(k) do { if (tid == 0) { const unsigned long long n_ = sk_now(); tacc[k] += n_ - tprev; tprev = n_; } } while (0)
-#else
-#define SK_PH(k) do { } while (0)
-#endif
   for (int it = grp; it < n_it; it += NG, ++gi) {
     uint8_t* pg = stage_base + (size_t)st * page_bytes;
     const int nvalid = len - (p0 + it) * PTOK;   // >= 1
@@ -1159,7 +1129,6 @@ __global__ void __launch_bounds__(NG * GW * 32, 1) decode_tc5_kernel(
       __syncwarp();
     }
     mbar_wait(full0 + 8 * st, (uint32_t)(use & 1));
-    SK_PH(0);
 
     if (nvalid < PTOK) {   // tail page: zero the key rows and the value scales of the slots past the sequence end
       for (int g = 0; g < L.n_kv_heads; ++g) {
@@ -1175,21 +1144,15 @@ __global__ void __launch_bounds__(NG * GW * 32, 1) decode_tc5_kernel(
     }
 
     // ================= QK + softmax for this warp's quad =================
-    if (has_quad && !(PL.dbg & 1))
+    if (has_quad)
       score_page<BH, BL, true>(L, PL, pg, qimg_lane, kcst, kv0, kv1, nvalid, R, j, gw, m_run, l_run, Pb, p_thr_off, al, fl);
-
-    SK_PH(1);
     // ================= value page -> A operand =================
     if (gi > 0) mbar_wait(mbar, (uint32_t)((gi - 1) & 1));   // the group's previous MMAs are done with P and its TMEM tiles
     if (NG != 2 && it >= 2) mbar_wait(afree0 + 8 * (it & 1), (uint32_t)(((it >> 1) - 1) & 1));   // page it - 2 is done with A
-    SK_PH(2);
-    if (!(PL.dbg & 2)) {
-      deq_block_to_a<BL>(pg + L.v_lo_off, pg + L.v_scale_off + PTOK * 2, L.v_lo_n, L.v_hi_n, abuf, gtd);
-      deq_block_to_a<BH>(pg + L.v_hi_off, pg + L.v_scale_off, L.v_hi_n, 0, abuf, t_hi);
-    }
+    deq_block_to_a<BL>(pg + L.v_lo_off, pg + L.v_scale_off + PTOK * 2, L.v_lo_n, L.v_hi_n, abuf, gtd);
+    deq_block_to_a<BH>(pg + L.v_hi_off, pg + L.v_scale_off, L.v_hi_n, 0, abuf, t_hi);
     fence_proxy_async();   // P and A (generic-proxy stores) -> visible to the tensor-core (async) proxy
     bar_sync(1 + grp, GW * 32);
-    SK_PH(3);
 
     // ================= lazy rescale of the TMEM accumulators (rare) =================
     {
@@ -1214,7 +1177,6 @@ __global__ void __launch_bounds__(NG * GW * 32, 1) decode_tc5_kernel(
     // and odd M tiles (different TMEM tiles: no ordering between them) and commit; warp 2 refills the ring stage
     if (gw == 0 || (gw == 4 && n_mt > 1)) {
       tc_fence_after();
-      SK_PH(4);
       const uint64_t da0 = umma_desc_k(smem_u32(abuf)), db0 = umma_desc_k(smem_u32(Pb));
       if (elect_one()) {
         for (int mt = gw >> 2; mt < n_mt; mt += (n_mt > 1 ? 2 : 1))
@@ -1222,7 +1184,6 @@ __global__ void __launch_bounds__(NG * GW * 32, 1) decode_tc5_kernel(
           for (int ks = 0; ks < PTOK / 16; ++ks)
             umma_f16(tmem_grp + (uint32_t)(mt * 32), da0 + (uint64_t)((mt * UM_TILE_BYTES + ks * 256) >> 4),
                      db0 + (uint64_t)((ks * 256) >> 4), IDESC, (gi > 0 || ks > 0) ? 1u : 0u);
-        SK_PH(5);
         umma_commit(mbar);
         if (NG != 2) umma_commit(afree0 + 8 * (it & 1));
       }
@@ -1232,16 +1193,9 @@ __global__ void __launch_bounds__(NG * GW * 32, 1) decode_tc5_kernel(
       if (nxt < n_it && elect_one()) issue(nxt, nxt < TBL_SMEM ? tbl_s[nxt] : my_table[nxt]);
       __syncwarp();
     }
-    SK_PH(6);
     st += NG;
     while (st >= nstage) { st -= nstage; ++use; }
   }
-#ifdef SK_TRACE
-  if (tid == 0) {
-    tacc[7] = (unsigned long long)gi;
-    for (int q = 0; q < 8; ++q) g_sk_trace[(blockIdx.y * gridDim.x + blockIdx.x) * 8 + q] = tacc[q];
-  }
-#endif
 
   // ================= merge the groups and write the split-K partial (D7) =================
   if (gi > 0) mbar_wait(mbar, (uint32_t)((gi - 1) & 1));   // this group's last MMAs are complete
@@ -1317,314 +1271,9 @@ template <int BH, int BL, int NG>
 cudaError_t launch_tc5(const starkv_ctx* ctx, dim3 grid, const uint8_t* qimg, size_t qimg_stride, const uint8_t* pool,
                        const int32_t* table, int max_pages, const int32_t* seq_lens, float* parts, int n_splits) {
   auto kern = decode_tc5_kernel<BH, BL, NG>;
-  static int smem_set = 0;
-  if (ctx->plan.smem_bytes > smem_set) {
-    const cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, ctx->plan.smem_bytes);
-    if (e != cudaSuccess) return e;
-    smem_set = ctx->plan.smem_bytes;
-  }
+  const cudaError_t ea = sk_need_smem(ctx, kern, ctx->plan.smem_bytes);
+  if (ea != cudaSuccess) return ea;
   return sk_launch(ctx, kern, grid, dim3(NG * GW * 32), (size_t)ctx->plan.smem_bytes, ctx->L, ctx->plan, qimg, qimg_stride, pool,
-                   table, max_pages, seq_lens, parts, n_splits);
-}
-
-// ---------------------------------------------------------------------------------------------
-// Warp-specialised form of the tcgen05 kernel (integer modes): 24 warps in three roles, no per-page group barrier.
-//   warps 0-7 / 8-15  QK + softmax of the even / odd pages of the range (score_page as above; P, alpha and the
-//                     rescale flag go to the group's double buffers), then ONE arrival per warp on the page's
-//                     "P ready" mbarrier; a warp never waits for the other warps of its group, so the rank-dependent
-//                     QK cost of the heads (16...56 channels on C3) no longer serialises on a barrier.
-//   warps 16-23       every page in turn: dequantise the value block into one of two A buffers, wait for "P ready",
-//                     rescale the group's TMEM tiles if a head moved its maximum, and (one thread) issue the page's
-//                     tcgen05.mma, commit to "A buffer free" and "P buffer free", refill the ring stage.
-// mbarriers: full[stage] (bulk copy), pready[g][buf] (8 arrivals), pfree[g][buf] and afree[2] (tcgen05.commit).
-// Every wait is at most one phase behind its barrier (pfree/pready/afree are used once per 4/4/2 pages in order).
-// ---------------------------------------------------------------------------------------------
-template <int BH, int BL>
-__global__ void __launch_bounds__(3 * GW * 32, 1) decode_ws_kernel(
-    const __grid_constant__ StarkvLayout L, const __grid_constant__ DecodePlan PL, const uint8_t* __restrict__ qimg_all,
-    size_t qimg_stride, const uint8_t* __restrict__ pool, const int32_t* __restrict__ table, int max_pages,
-    const int32_t* __restrict__ seq_lens, float* __restrict__ parts, int n_splits) {
-  extern __shared__ __align__(128) uint8_t smem[];
-  static_assert(BH != 16, "integer modes only");
-  constexpr int NTHREADS = 3 * GW * 32;
-  constexpr int BAR_D = 3;   // named barriers 3, 4 of the two dequantise/MMA halves (1, 2: the QK groups, tail pages only)
-
-  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-  const int j = lane & 3, R = lane >> 2;
-  const int split = blockIdx.x, b = blockIdx.y;
-  sk_pdl_trigger();
-  const int len = seq_lens[b];   // caller-owned inputs: read ahead of the dependency wait (ctx.h)
-  const int n_pages = (len + PTOK - 1) / PTOK;
-  int p0, p1;
-  sk_split_range(n_pages, n_splits, 1, split, &p0, &p1);
-  const int n_it = p1 - p0;
-  const size_t pstride = sk_part_stride(L.rank_v);
-  float* my_parts = parts + ((size_t)b * n_splits + split) * L.n_q_heads * pstride;
-
-  if (n_it <= 0) {   // empty range (CTA-uniform): neutral partial
-    sk_pdl_wait();
-    for (int i = tid; i < L.n_q_heads * (int)pstride; i += NTHREADS) {
-      const int c = i % (int)pstride;
-      my_parts[i] = c == 0 ? -INFINITY : 0.f;
-    }
-    return;
-  }
-
-  uint8_t* stage_base = smem + PL.off_stage;
-  const int nstage = PL.nstage;
-  const int n_mt = PL.um_mt;
-  // barrier area: full[nstage], image, pready[2][2], pfree[2][2], afree[2], TMEM base address, issued[nstage]
-  const uint32_t full0 = smem_u32(smem + PL.off_bar);
-  const uint32_t qbar = full0 + 8 * nstage;
-  const uint32_t pready0 = qbar + 8, pfree0 = pready0 + 32, afree0 = pfree0 + 32;
-  const int misc_off = PL.off_bar + 8 * nstage + 8 + 32 + 32 + 16;
-  volatile uint32_t& tmem_base_s = *reinterpret_cast<volatile uint32_t*>(smem + misc_off);
-  volatile int* issued = reinterpret_cast<int*>(smem + misc_off + 8);   // [nstage]
-  int32_t* tbl_s = reinterpret_cast<int32_t*>(smem + PL.off_tbl);
-  const uint32_t page_bytes = (uint32_t)L.page_bytes;
-  const int32_t* my_table = table + (size_t)b * max_pages + p0;
-
-  auto issue = [&](int it, int page) {   // D2: one page -> ring stage (single thread)
-    const int st = it % nstage;
-    const uint32_t bar = full0 + 8 * st;
-    mbar_expect_tx(bar, page_bytes);
-    __threadfence_block();
-    issued[st] = it;
-    bulk_g2s_stream(smem_u32(stage_base + (size_t)st * page_bytes), pool + (size_t)page * page_bytes, page_bytes, bar,
-                    l2_evict_first_policy());
-  };
-
-  if (tid == 0) {
-    for (int s = 0; s < nstage; ++s) {
-      mbar_init(full0 + 8 * s, 1);
-      issued[s] = -1;
-    }
-    mbar_init(qbar, 1);
-    for (int i = 0; i < 4; ++i) {
-      mbar_init(pready0 + 8 * i, GW);
-      mbar_init(pfree0 + 8 * i, 1);
-    }
-    mbar_init(afree0, 1);
-    mbar_init(afree0 + 8, 1);
-    fence_barrier_init();
-    int pgs[8];
-#pragma unroll
-    for (int s = 0; s < 8; ++s) pgs[s] = s < min(nstage, n_it) ? my_table[s] : 0;
-    sk_pdl_wait();
-    const uint32_t qbytes = (uint32_t)(PL.qimg_bytes + L.n_kv_heads * 32);
-    mbar_expect_tx(qbar, qbytes);
-    bulk_g2s(smem_u32(smem + PL.off_qimg), qimg_all + (size_t)b * qimg_stride, qbytes, qbar);
-#pragma unroll
-    for (int s = 0; s < 8; ++s)
-      if (s < min(nstage, n_it)) issue(s, pgs[s]);
-  }
-  if (warp == 1) {   // TMEM: 32 fp32 columns per (QK group, M tile)
-    const uint32_t dst = smem_u32(smem + misc_off);
-    const uint32_t ncol = (uint32_t)PL.um_cols;
-    asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(dst), "r"(ncol) : "memory");
-    asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
-  }
-  for (int i = tid; i < min(n_it, TBL_SMEM); i += NTHREADS) tbl_s[i] = my_table[i];
-  {
-    uint4* pz = reinterpret_cast<uint4*>(smem + PL.off_p);
-    for (int i = tid; i < 2 * 2 * P_BUF_BYTES / 16; i += NTHREADS) pz[i] = make_uint4(0, 0, 0, 0);
-    if (tid < 2 * 64) reinterpret_cast<float*>(smem + PL.off_alpha)[tid] = 1.f;
-    if (tid < 2 * 4) reinterpret_cast<uint32_t*>(smem + PL.off_flag)[tid] = 0;
-  }
-  sk_pdl_wait();
-  tc_fence_before();
-  __syncthreads();
-  tc_fence_after();
-  const uint32_t tmem0 = tmem_base_s;
-  const int gw = warp & (GW - 1);
-  // instruction descriptor: D fp32 (bit 4), A and B fp16 K-major, N = 32 (bits 17..), M = 128 (bits 24..)
-  constexpr uint32_t IDESC = (1u << 4) | ((uint32_t)(32 >> 3) << 17) | ((uint32_t)(UM_ROWS >> 4) << 24);
-
-  float m_run = -INFINITY, l_run = 0.f;
-  int gi = 0;   // pages this QK warp has scored
-  const int grp = warp >> 3;   // 0, 1: QK groups; 2: dequantise / MMA
-  const bool has_quad = gw < PL.nq;
-
-  if (grp < 2) {
-    // ===================== QK + softmax warps =====================
-    mbar_wait(qbar, 0);
-    const uint2* qimg_lane = reinterpret_cast<const uint2*>(smem + PL.off_qimg) + lane;
-    const float* kcst = reinterpret_cast<const float*>(smem + PL.off_kcst);
-    uint8_t* Pm = smem + PL.off_p + grp * 2 * P_BUF_BYTES;
-    float* alpha_s = reinterpret_cast<float*>(smem + PL.off_alpha) + grp * 64;
-    uint8_t* flag_s = smem + PL.off_flag + grp * 16;
-    const int kv0 = gw * PL.kv_per_quad;
-    const int kv1 = min(kv0 + PL.kv_per_quad, L.n_kv_heads);
-    const int p_thr_off = (gw >> 1) * 1024 + (2 * (R >> 1)) * 128 + (4 * (gw & 1) + j) * 16 + 8 * (R & 1);
-    const int gt = tid & 255;
-    int st = grp % nstage, use = grp / nstage;
-    for (int it = grp; it < n_it; it += 2, ++gi) {
-      uint8_t* pg = stage_base + (size_t)st * page_bytes;
-      const int nvalid = len - (p0 + it) * PTOK;   // >= 1
-      const int buf = gi & 1;
-      if (lane == 0)
-        while (issued[st] != it) {}
-      __syncwarp();
-      mbar_wait(full0 + 8 * st, (uint32_t)(use & 1));
-      if (nvalid < PTOK) {   // tail page: zero the key rows of the slots past the sequence end (this group's reads)
-        for (int g = 0; g < L.n_kv_heads; ++g) {
-          for (int blk = 0; blk < 2; ++blk) {
-            const int n = blk ? L.k_lo_n[g] : L.k_hi_n[g];
-            const int rowb = n * (blk ? BL : BH) / 8;
-            uint32_t* dst = reinterpret_cast<uint32_t*>(pg + (blk ? L.k_lo_off[g] : L.k_hi_off[g]) + nvalid * rowb);
-            for (int i = gt; i < (PTOK - nvalid) * rowb / 4; i += 256) dst[i] = 0;
-          }
-        }
-        bar_sync(1 + grp, GW * 32);
-      }
-      if (gi >= 2) mbar_wait(pfree0 + 8 * (2 * grp + buf), (uint32_t)(((gi >> 1) - 1) & 1));   // MMAs of page it - 4 done with P
-      if (has_quad)
-        score_page<BH, BL, true>(L, PL, pg, qimg_lane, kcst, kv0, kv1, nvalid, R, j, gw, m_run, l_run,
-                                 Pm + buf * P_BUF_BYTES, p_thr_off, alpha_s + buf * 32, flag_s + buf * 8);
-      fence_proxy_async();   // P (generic-proxy stores) -> visible to the tensor-core (async) proxy
-      __syncwarp();
-      if (lane == 0) mbar_arrive(pready0 + 8 * (2 * grp + buf));
-      st += 2;
-      while (st >= nstage) { st -= nstage; ++use; }
-    }
-  } else {
-    // ===================== dequantise + MMA warps: two halves of 4 warps on alternating pages =====================
-    const int dh = (warp - 2 * GW) >> 2;          // half = page parity = QK group = A buffer
-    const int dw = warp & 3, gt = tid & 127;      // warp within the half (= its TMEM lane quarter), thread within the half
-    const int n_lo_items = L.v_lo_n * (BL / 2);
-    const int t_hi = (gt + 128 - (n_lo_items & 127)) & 127;
-    uint8_t* abuf = smem + PL.off_a + dh * n_mt * UM_TILE_BYTES;
-    const uint32_t tmem_grp = tmem0 + (uint32_t)(dh * n_mt * 32);
-    int st = dh % nstage, use = dh / nstage;
-    int qi = 0;
-    for (int it = dh; it < n_it; it += 2, ++qi) {
-      uint8_t* pg = stage_base + (size_t)st * page_bytes;
-      const int nvalid = len - (p0 + it) * PTOK;
-      const int buf = qi & 1;
-      if (lane == 0)
-        while (issued[st] != it) {}
-      __syncwarp();
-      mbar_wait(full0 + 8 * st, (uint32_t)(use & 1));
-      if (nvalid < PTOK) {   // tail page: zero the value scales of the slots past the sequence end
-        if ((gt & (PTOK - 1)) >= nvalid) reinterpret_cast<uint16_t*>(pg + L.v_scale_off)[gt] = 0;
-        bar_sync(BAR_D + dh, 128);
-      }
-      if (qi >= 1) mbar_wait(afree0 + 8 * dh, (uint32_t)((qi - 1) & 1));   // MMAs of page it - 2 have read this A buffer
-      deq_block_to_a<BL, 128>(pg + L.v_lo_off, pg + L.v_scale_off + PTOK * 2, L.v_lo_n, L.v_hi_n, abuf, gt);
-      deq_block_to_a<BH, 128>(pg + L.v_hi_off, pg + L.v_scale_off, L.v_hi_n, 0, abuf, t_hi);
-      fence_proxy_async();
-      mbar_wait(pready0 + 8 * (2 * dh + buf), (uint32_t)((qi >> 1) & 1));   // P, alpha, flag of this page are complete
-      {
-        const uint2 f8 = *reinterpret_cast<const uint2*>(smem + PL.off_flag + dh * 16 + buf * 8);
-        if ((f8.x | f8.y) != 0 && qi > 0) {   // lazy rescale of the group's accumulators (its last MMAs: page it - 2, done)
-          const float* al = reinterpret_cast<const float*>(smem + PL.off_alpha) + dh * 64 + buf * 32;
-          tc_fence_after();
-          for (int mt = 0; mt < n_mt; ++mt) {
-            const uint32_t taddr = tmem_grp + ((uint32_t)(dw * 32) << 16) + (uint32_t)(mt * 32);
-            uint32_t v[32];
-            tmem_ld32(taddr, v);
-#pragma unroll
-            for (int c = 0; c < 32; ++c) v[c] = __float_as_uint(__uint_as_float(v[c]) * al[c]);
-            tmem_st32(taddr, v);
-          }
-          tc_fence_before();
-        }
-      }
-      bar_sync(BAR_D + dh, 128);   // A complete, every warp past its reads of the page, rescale written
-      if (gt == 0) {
-        tc_fence_after();
-        const uint32_t sa = smem_u32(abuf), sb = smem_u32(smem + PL.off_p + (2 * dh + buf) * P_BUF_BYTES);
-        for (int mt = 0; mt < n_mt; ++mt)
-#pragma unroll
-          for (int ks = 0; ks < PTOK / 16; ++ks)
-            umma_f16(tmem_grp + (uint32_t)(mt * 32), umma_desc_k(sa + mt * UM_TILE_BYTES + ks * 256), umma_desc_k(sb + ks * 256),
-                     IDESC, (qi > 0 || ks > 0) ? 1u : 0u);
-        umma_commit(afree0 + 8 * dh);
-        umma_commit(pfree0 + 8 * (2 * dh + buf));
-        const int nxt = it + nstage;
-        if (nxt < n_it) issue(nxt, nxt < TBL_SMEM ? tbl_s[nxt] : my_table[nxt]);
-      }
-      st += 2;
-      while (st >= nstage) { st -= nstage; ++use; }
-    }
-    // every MMA of this half is complete before anyone reads TMEM or reuses the stage memory
-    if (qi >= 1) mbar_wait(afree0 + 8 * dh, (uint32_t)((qi - 1) & 1));
-    tc_fence_before();
-  }
-
-  // ================= merge the groups and write the split-K partial (D7) =================
-  bar_sync(BAR_ALL, NTHREADS);
-  tc_fence_after();
-  float* mg = reinterpret_cast<float*>(smem + PL.off_stage);   // m at [g * 32 + head], l at [96 + ..], weight at [192 + ..]
-  float* ost = mg + 384;
-  const int ST = (int)pstride;
-  if (grp < 2 && has_quad) {
-    float lsum = l_run;
-    lsum += __shfl_xor_sync(0xffffffffu, lsum, 4);
-    lsum += __shfl_xor_sync(0xffffffffu, lsum, 8);
-    lsum += __shfl_xor_sync(0xffffffffu, lsum, 16);
-    if (R == 0) {
-      mg[grp * 32 + 4 * gw + j] = m_run;
-      mg[96 + grp * 32 + 4 * gw + j] = lsum;
-    }
-  }
-  bar_sync(BAR_ALL, NTHREADS);
-  if (tid < 32 && tid < L.n_q_heads) {
-    const float m0 = mg[tid], m1 = mg[32 + tid];   // group 0 always has a page: m0 is finite
-    const float ms = fmaxf(m0, m1);
-    const float w0 = ex2(m0 - ms), w1 = m1 == -INFINITY ? 0.f : ex2(m1 - ms);
-    mg[192 + tid] = w0;
-    mg[224 + tid] = w1;
-    *reinterpret_cast<float4*>(ost + tid * ST) = make_float4(ms, mg[96 + tid] * w0 + mg[128 + tid] * w1, 0.f, 0.f);
-  }
-  bar_sync(BAR_ALL, NTHREADS);
-#pragma unroll
-  for (int pass = 0; pass < 2; ++pass) {   // QK group 0's warps store their tiles, group 1's add (if it had a page)
-    if (grp == pass && gi > 0) {
-      const float* wt = mg + 192 + 32 * grp;
-      const uint32_t tmem_grp = tmem0 + (uint32_t)(grp * n_mt * 32);
-      for (int mt = gw >> 2; mt < n_mt; mt += 2) {
-        const uint32_t taddr = tmem_grp + ((uint32_t)((gw & 3) * 32) << 16) + (uint32_t)(mt * 32);
-        uint32_t v[32];
-        tmem_ld32(taddr, v);
-        const int ch = mt * UM_ROWS + (gw & 3) * 32 + lane;
-        if (ch < L.rank_v) {
-          float* o = ost + 4 + ch;
-#pragma unroll
-          for (int h = 0; h < 32; ++h)
-            if (h < L.n_q_heads) {
-              const float x = __uint_as_float(v[h]) * wt[h];
-              o[h * ST] = pass == 0 ? x : o[h * ST] + x;
-            }
-        }
-      }
-    }
-    bar_sync(BAR_ALL, NTHREADS);
-  }
-  {
-    const float4* src = reinterpret_cast<const float4*>(ost);
-    float4* dst = reinterpret_cast<float4*>(my_parts);
-    for (int i = tid; i < L.n_q_heads * ST / 4; i += NTHREADS) dst[i] = src[i];
-  }
-  tc_fence_before();
-  __syncthreads();
-  if (warp == 1) {
-    const uint32_t ncol = (uint32_t)PL.um_cols;
-    asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"((uint32_t)tmem_base_s), "r"(ncol) : "memory");
-  }
-}
-
-template <int BH, int BL>
-cudaError_t launch_ws(const starkv_ctx* ctx, dim3 grid, const uint8_t* qimg, size_t qimg_stride, const uint8_t* pool,
-                      const int32_t* table, int max_pages, const int32_t* seq_lens, float* parts, int n_splits) {
-  auto kern = decode_ws_kernel<BH, BL>;
-  static int smem_set = 0;
-  if (ctx->plan.smem_bytes > smem_set) {
-    const cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, ctx->plan.smem_bytes);
-    if (e != cudaSuccess) return e;
-    smem_set = ctx->plan.smem_bytes;
-  }
-  return sk_launch(ctx, kern, grid, dim3(3 * GW * 32), (size_t)ctx->plan.smem_bytes, ctx->L, ctx->plan, qimg, qimg_stride, pool,
                    table, max_pages, seq_lens, parts, n_splits);
 }
 
@@ -1632,12 +1281,8 @@ template <int BH, int BL, int NT, int MT, int NG>
 cudaError_t launch_fast(const starkv_ctx* ctx, dim3 grid, const uint8_t* qimg, size_t qimg_stride, const uint8_t* pool,
                         const int32_t* table, int max_pages, const int32_t* seq_lens, float* parts, int n_splits) {
   auto kern = decode_fast_kernel<BH, BL, NT, MT, NG>;
-  static int smem_set = 0;   // largest dynamic shared-memory size already granted to this instantiation
-  if (ctx->plan.smem_bytes > smem_set) {
-    const cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, ctx->plan.smem_bytes);
-    if (e != cudaSuccess) return e;
-    smem_set = ctx->plan.smem_bytes;
-  }
+  const cudaError_t ea = sk_need_smem(ctx, kern, ctx->plan.smem_bytes);
+  if (ea != cudaSuccess) return ea;
   return sk_launch(ctx, kern, grid, dim3(NG * GW * 32), (size_t)ctx->plan.smem_bytes, ctx->L, ctx->plan, qimg, qimg_stride,
                    pool, table, max_pages, seq_lens, parts, n_splits);
 }
@@ -1700,32 +1345,23 @@ int sk_fast_plan(starkv_ctx* ctx) {
   if ((long long)ns * L.page_bytes < merge_bytes) {
     if (merge_bytes > avail) return 0;
   }
-  // tcgen05 PV for the integer modes: 2 groups x um_mt x 16 KB of A operand come out of the ring's memory.  Taken
-  // when at least 4 ring stages remain (STARKV_PV=mma forces the mma.sync kernel, STARKV_PV=tcgen05 accepts 3 stages).
-  if (quant && L.rank_v <= 4 * 128) {
-    const char* e_pv = getenv("STARKV_PV");
-    const char* e_g5 = getenv("STARKV_TC5_GROUPS");
+  // tcgen05 PV for the integer modes (decode_tc5_kernel): 2 x um_mt x 16 KB of A operand come out of the ring's memory.
+  // Taken when at least 4 ring stages remain (3 when the variant is requested explicitly); SK_VARIANT_MMA keeps mma.sync.
+  if (quant && L.rank_v <= 4 * 128 && ctx->variant != SK_VARIANT_MMA) {
     const int um_mt = (L.rank_v + 127) / 128;
-    const int need = (e_pv && (e_pv[0] == 't' || e_pv[0] == 'w')) ? 3 : 4;
-    (void)e_g5;   // three groups were measured (no gain with six ring stages on C3, a hang on C5): two only
-    for (int ng5 = 2; ng5 >= 2 && !P.um; --ng5) {
-      const int a_bytes = 2 * um_mt * 128 * PTOK * 2;   // two A buffers, shared by the groups
-      int ns5 = (avail - a_bytes) / L.page_bytes;
-      if (ns5 > 8) ns5 = 8;
-      const bool room = avail - a_bytes >= merge_bytes;
-      if (!(e_pv && e_pv[0] == 'm') && ns5 >= need && room) {
-        P.um = 1;
-        P.um_mt = um_mt;
-        int cols = 32;
-        while (cols < ng5 * um_mt * 32) cols *= 2;
-        P.um_cols = cols;
-        P.um_ng = ng5;
-        P.um_ws = (e_pv && e_pv[0] == 'w') ? 1 : 0;   // STARKV_PV=ws: warp-specialised roles (two groups' worth of A)
-        ns = ns5;
-      }
+    const int need = ctx->variant == SK_VARIANT_TC5 ? 3 : 4;
+    const int a_bytes = 2 * um_mt * 128 * PTOK * 2;   // two A buffers, shared by the groups
+    int ns5 = (avail - a_bytes) / L.page_bytes;
+    if (ns5 > 8) ns5 = 8;
+    if (ns5 >= need && avail - a_bytes >= merge_bytes) {
+      P.um = 1;
+      P.um_mt = um_mt;
+      int cols = 32;
+      while (cols < 2 * um_mt * 32) cols *= 2;
+      P.um_cols = cols;
+      ns = ns5;
     }
   }
-  { const char* e_d = getenv("STARKV_DEBUG_SKIP"); P.dbg = e_d ? atoi(e_d) : 0; }
   {   // dequantisation slices by QK load: lightest QK warp -> slice 0 (the heaviest), ties in warp order
     int cost[GW], order[GW];
     for (int w = 0; w < GW; ++w) {
@@ -1744,11 +1380,6 @@ int sk_fast_plan(starkv_ctx* ctx) {
   // pages so large that only two fit: one group, so that the second stage is a copy in flight instead of a
   // second page being computed on (built for the fp16 and int8/int4 modes)
   P.ng = (ns == 2 && (L.bits_hi == 16 || (L.bits_hi == 8 && L.bits_lo == 4))) ? 1 : 2;
-  {
-    const char* e_ng = getenv("STARKV_GROUPS");
-    if (e_ng && e_ng[0] == '2') P.ng = 2;
-    if (e_ng && e_ng[0] == '1' && (L.bits_hi == 16 || (L.bits_hi == 8 && L.bits_lo == 4))) P.ng = 1;
-  }
   int off = 0;
   P.off_stage = off;
   off += round_up(ns * L.page_bytes > merge_bytes ? ns * L.page_bytes : merge_bytes, 128);
@@ -1776,7 +1407,9 @@ void sk_plan_workspace(const starkv_ctx* ctx, int batch, int max_pages, SkWorksp
   if (ns < 1) ns = 1;
   w->n_splits = ns;
   size_t off = 0;
-  w->qimg_stride = (size_t)round_up(ctx->fast_ok ? ctx->plan.qimg_bytes + L.n_kv_heads * 32 : 0, 256);
+  int qb_img = ctx->fast_ok ? ctx->plan.qimg_bytes + L.n_kv_heads * 32 : 0;
+  if (ctx->tm.ok && ctx->tm.img_bytes > qb_img) qb_img = ctx->tm.img_bytes;
+  w->qimg_stride = (size_t)round_up(qb_img, 256);
   w->qimg_off = off; off += w->qimg_stride * batch;
   w->part_off = off; off += ((size_t)batch * ns * L.n_q_heads * sk_part_stride(L.rank_v) * 4 + 255) / 256 * 256;
   w->host_off = off;
@@ -1810,13 +1443,7 @@ int sk_decode_fast(starkv_ctx* ctx, const void* q, const void* pool, const int32
   const bool one = ctx->plan.ng == 1;
 #define SK_TC5(BHv, BLv, NGv) \
   e = launch_tc5<BHv, BLv, NGv>(ctx, grid, qimg, w.qimg_stride, pl, table, max_pages, seq_lens, parts, w.n_splits)
-  if (ctx->plan.um && ctx->plan.um_ws) {
-    if (L.bits_hi == 8 && L.bits_lo == 4) e = launch_ws<8, 4>(ctx, grid, qimg, w.qimg_stride, pl, table, max_pages, seq_lens, parts, w.n_splits);
-    else if (L.bits_hi == 8 && L.bits_lo == 8) e = launch_ws<8, 8>(ctx, grid, qimg, w.qimg_stride, pl, table, max_pages, seq_lens, parts, w.n_splits);
-    else if (L.bits_hi == 4 && L.bits_lo == 4) e = launch_ws<4, 4>(ctx, grid, qimg, w.qimg_stride, pl, table, max_pages, seq_lens, parts, w.n_splits);
-  } else if (ctx->plan.um) {
-    const bool three = ctx->plan.um_ng == 3;
-    (void)three;
+  if (ctx->plan.um) {
     if (L.bits_hi == 8 && L.bits_lo == 4) SK_TC5(8, 4, 2);
     else if (L.bits_hi == 8 && L.bits_lo == 8) SK_TC5(8, 8, 2);
     else if (L.bits_hi == 4 && L.bits_lo == 4) SK_TC5(4, 4, 2);

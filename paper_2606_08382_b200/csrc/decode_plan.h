@@ -33,11 +33,8 @@ struct DecodePlan {
   int32_t smem_bytes;
   // tcgen05 PV variant (decode_tc5_kernel, integer modes): value page dequantised into a K-major UMMA A operand
   int32_t um;                                     // 1 = use it
-  int32_t um_ng;                                  // groups of 8 warps: 2 (or 3 with STARKV_TC5_GROUPS=3, 8/4-bit mode)
   int32_t deq_slice[8];                           // warp gw of a group dequantises item slice deq_slice[gw] (32 threads' worth):
                                                   // the warps with the most QK steps get the lightest slices
-  int32_t dbg;                                    // timing experiments only (STARKV_DEBUG_SKIP): 1 = no QK, 2 = no dequantisation
-  int32_t um_ws;                                  // 1 = warp-specialised kernel (decode_ws_kernel)
   int32_t um_mt;                                  // 128-channel M tiles = ceil(r_v / 128) <= 4
   int32_t um_cols;                                // TMEM columns to allocate (power of two >= 2 groups * um_mt * 32)
   int32_t off_a;                                  // [2 groups][um_mt][16 KB] A operand
@@ -50,3 +47,44 @@ static inline __host__ __device__ int sk_k_to_channel(int bits, int m, int k) {
   const int hi8 = k >> 3, j = (k & 7) >> 1, e = k & 1;
   return bits == 4 ? 8 * j + 2 * m + hi8 + 4 * e : 4 * j + 2 * hi8 + e;
 }
+
+// ---------------------------------------------------------------------------------------------
+// Host-built plan of the TMEM-operand decode kernel (decode_tm.cu, integer modes).
+//
+// One iteration = 128 tokens (two 64-token pages) = the 128 TMEM lanes.  Both products run on tcgen05.mma with the
+// A operand in tensor memory:
+//   QK   S^T[token x (head, block, g)] = codes[token x channel] . Q^T   A = the token's key codes as fp16 subnormals
+//        (thread = token = lane writes its own row), B = latent-space query image in shared memory, K = 16 latent
+//        channels ("k-step" = two 8-channel octets, each octet inside one (KV head, precision block)), N = a 16-column
+//        window of the score tile that covers the columns of the k-step's two octets.
+//   PV   O^T[channel x head] += c[channel x token] . P~^T   A = the channel's value codes, exact in fp16 (thread =
+//        channel = lane), B = P~ = p * value scale, one operand per precision block.
+// ---------------------------------------------------------------------------------------------
+#define SK_TM_MAX_KS 17            // k-steps (272 latent channels)
+#define SK_TM_MAX_OCT (2 * SK_TM_MAX_KS)
+struct TmPlan {
+  int32_t ok;                       // this descriptor runs on the kernel
+  int32_t n_ks;                     // k-steps of 16 latent channels (the last one may hold a padding octet)
+  // per octet slot o (k positions 8(o & 1) .. +8 of k-step o >> 1):
+  int32_t oct_off[SK_TM_MAX_OCT];   // page byte offset of slot 0's eight codes (-1 = padding, zeros)
+  int32_t oct_rowb[SK_TM_MAX_OCT];  // bytes from one token slot to the next
+  int32_t oct_bits[SK_TM_MAX_OCT];  // 8 or 4
+  int32_t oct_head[SK_TM_MAX_OCT];  // KV head
+  int32_t oct_blk[SK_TM_MAX_OCT];   // precision block (0 = leading)
+  int32_t oct_col[SK_TM_MAX_OCT];   // latent column (in [0, sum r_h)) of the octet's first channel
+  int32_t win[SK_TM_MAX_KS];        // first score column of the k-step's 16-column window (multiple of 8)
+  int32_t ds_cols;                  // score-tile columns (multiple of 16, covers every window); column of
+                                    // (KV head h, block b, group member g) = (2 h + b) G + g
+  // latent-space query image, per sequence: [constant tile: ds_cols x 16][k-step tiles: n_ks x (hi 512 B, lo 512 B)]
+  // [scalars: float 2^(24 - e)], all B tiles K-major no-swizzle (LBO 128, SBO 256)
+  int32_t img_ks_off, img_scal_off, img_bytes;
+  // value side
+  int32_t n_vt;                     // 128-channel A tiles = ceil(r_v / 128) <= 2
+  int32_t n_dt;                     // accumulator tiles = (A tile, precision block) pairs that intersect
+  int32_t dt_tile[4], dt_blk[4];
+  // tensor memory columns
+  int32_t col_do, col_av, col_ak, col_ds;
+  // shared memory (bytes from the 1024-aligned base)
+  int32_t nstage;                   // page ring depth
+  int32_t off_stage, off_img, off_p, off_misc, off_bar, off_tbl, smem_bytes;
+};

@@ -67,7 +67,7 @@ def test_pack_empty_is_a_no_op():
     sk.starkv_unpack(ctx, None, 0)
 
 
-def _append_case(cfg, mode, n_new, dyadic, pad=0):
+def _append_case(cfg, mode, n_new, dyadic, pad=0, tc5=False):
     d = CacheDesc.from_config(cfg)
     lay = page_layout(d)
     rng = np.random.default_rng(5)
@@ -107,6 +107,8 @@ def _append_case(cfg, mode, n_new, dyadic, pad=0):
     kw, vw = k2.shape[1], v2.shape[1]
     oappend.append(d, ref, table, seq_ids, positions, k2, khs, d_in_k, v2, ak, av)
     ctx = sk.create_from_config(cfg)
+    if tc5:
+        sk.starkv_set_option(ctx, "append_tc5", 1)
     dpool = dev(pool)
     wsb = sk.starkv_append_workspace_bytes(ctx, n)
     ws = torch.empty(max(wsb, 16), dtype=torch.uint8, device="cuda")
@@ -122,14 +124,14 @@ def _append_case(cfg, mode, n_new, dyadic, pad=0):
 
 @pytest.mark.parametrize("n_new", [-80, 80, 37, 8, 1], ids=["n80-tcgen05", "n80-mma", "n37-mma", "n8-small", "n1-small"])
 @pytest.mark.parametrize("name,mode", [("C1", "dense"), ("C3", "dense"), ("C3", "hidden"), ("C4", "dense")])
-def test_append_bit_exact_on_dyadic_inputs(name, mode, n_new, monkeypatch):
+def test_append_bit_exact_on_dyadic_inputs(name, mode, n_new):
     """n_new 80 -> 134 tokens (two token tiles with a ragged tail) on the mma.sync projection and, opted in through
-    STARKV_APPEND_GEMM, on the tcgen05 projection; 37 -> 62 tokens; 8 -> 15 and 1 -> 2 tokens (split-K small-n kernel)."""
-    if n_new < 0:
-        monkeypatch.setenv("STARKV_APPEND_GEMM", "tcgen05")
-        n_new = -n_new
+    starkv_set_option "append_tc5", on the tcgen05 projection; 37 -> 62 tokens; 8 -> 15 and 1 -> 2 tokens (split-K
+    small-n kernel)."""
+    tc5 = n_new < 0
+    n_new = abs(n_new)
     cfg = synth.make_config(name, context=256, batch=3)
-    d, lay, got, ref, n = _append_case(cfg, mode, n_new, dyadic=True)
+    d, lay, got, ref, n = _append_case(cfg, mode, n_new, dyadic=True, tc5=tc5)
     assert np.array_equal(got, ref), f"{int((got != ref).sum())} bytes differ of {got.size}"
 
 

@@ -53,24 +53,26 @@ def test_peaky_regime(name):
     _check(cfg, regime="peaky")
 
 
-@pytest.mark.parametrize("pv,groups", [("tcgen05", "2"), ("ws", "2"), ("mma", "2")],
-                         ids=["tcgen05", "warp-specialised", "mma"])
+@pytest.mark.parametrize("variant", ["tm", "tc5", "mma"])
 @pytest.mark.parametrize("bits", [(8, 4), (8, 8), (4, 4)], ids=str)
-def test_value_product_variants(pv, groups, bits, monkeypatch):
-    """The integer modes have two value-product paths: tcgen05 with TMEM accumulators
-    (decode_tc5_kernel, the default where its A operand fits beside the page ring) and mma.sync (decode_fast_kernel).
-    Both are held to the oracle, in both regimes (the peaky one exercises the TMEM rescale), ragged lengths, a value
-    rank above one 128-channel M tile and one that is not a multiple of 16."""
-    monkeypatch.setenv("STARKV_PV", pv)
-    monkeypatch.setenv("STARKV_TC5_GROUPS", groups)
-    # (the second shape's pages leave an ODD ring depth beside the A operand in 8/4-bit mode: stages shared by the groups)
+def test_value_product_variants(variant, bits):
+    """The integer modes have three tensor-core kernels: decode_tm_kernel (both products on tcgen05,
+    A operands in tensor memory; the default where it covers the descriptor), decode_tc5_kernel (value product on
+    tcgen05, scores on mma.sync) and decode_fast_kernel (mma.sync).  All are held to the oracle, in both regimes (the
+    peaky one exercises the TMEM rescale), ragged lengths, a value rank above one 128-channel tile and one that is not a
+    multiple of 16."""
+    want = {"tm": "decode_tm_kernel", "tc5": "decode_tc5_kernel", "mma": "decode_fast_kernel"}[variant]
     for (hq, hkv, dh, rk, rv) in [(32, 8, 128, [24, 16, 24, 48, 16, 32, 56, 40], 256),
                                   (32, 8, 128, [40, 40, 48, 32, 40, 40, 48, 32], 256),
                                   (16, 4, 64, [16, 64, 8, 24], 136),
                                   (8, 8, 64, [8, 16, 24, 32, 40, 48, 56, 64], 72)]:
         cfg = synth.custom_config(f"pv{bits[0]}{bits[1]}", 2, hq, hkv, dh, 1500, rk, rv, bits=bits, outlier_frac=0.1)
         ctx = sk.create_from_config(cfg)
-        want = {"tcgen05": "decode_tc5_kernel", "ws": "decode_ws_kernel", "mma": "decode_fast_kernel"}[pv]
+        try:
+            sk.starkv_set_option(ctx, "decode_variant", sk.DECODE_VARIANTS[variant])
+        except sk.StarkvError as e:   # this kernel does not cover the shape (e.g. more than 272 key channels for "tm")
+            assert e.code == sk.STARKV_ERR_UNSUPPORTED and variant == "tm" and sum(rk) > 272
+            continue
         assert sk.starkv_decode_kernel_name(ctx) == want
         for regime in ("diffuse", "peaky"):
             cache = build_cache(cfg, seq_lens=[1500, 777], regime=regime)
@@ -80,7 +82,7 @@ def test_value_product_variants(pv, groups, bits, monkeypatch):
             out = run_decode(cfg, cache, q, bk, bv, ctx=ctx)
             assert np.isfinite(out).all()
             err = row_rel_err(out, ref)
-            assert err <= TOL, f"{pv} {bits} {regime} r_v={rv}: row rel err {err:.3e}"
+            assert err <= TOL, f"{variant} {bits} {regime} r_v={rv}: row rel err {err:.3e}"
 
 
 @pytest.mark.parametrize("bits", [(8, 8), (4, 4), (8, 4), (16, 16)], ids=str)

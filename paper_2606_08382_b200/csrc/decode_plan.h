@@ -60,23 +60,26 @@ static inline __host__ __device__ int sk_k_to_channel(int bits, int m, int k) {
 //   PV   O^T[channel x head] += c[channel x token] . P~^T   A = the channel's value codes, exact in fp16 (thread =
 //        channel = lane), B = P~ = p * value scale, one operand per precision block.
 // ---------------------------------------------------------------------------------------------
-#define SK_TM_MAX_KS 17            // k-steps (272 latent channels)
-#define SK_TM_MAX_OCT (2 * SK_TM_MAX_KS)
+#define SK_TM_MAX_TRIPS 10                    // the key-row warps convert four octets (two k-steps) per trip
+#define SK_TM_MAX_OCT (4 * SK_TM_MAX_TRIPS)   // octet slots (320 latent channels including padding)
+#define SK_TM_MAX_KS (2 * SK_TM_MAX_TRIPS)    // k-steps
 struct TmPlan {
   int32_t ok;                       // this descriptor runs on the kernel
-  int32_t n_ks;                     // k-steps of 16 latent channels (the last one may hold a padding octet)
-  // per octet slot o (k positions 8(o & 1) .. +8 of k-step o >> 1):
-  int32_t oct_off[SK_TM_MAX_OCT];   // page byte offset of slot 0's eight codes (-1 = padding, zeros)
+  // Octet slots: first every 8-bit octet in cache order (head by head, leading block then trailing block), padded to
+  // a multiple of four, then every 4-bit octet likewise.  Grouping by width keeps the conversion loops branch-free.
+  int32_t n_trips8, n_trips4;       // trips (four slots) of the two groups
+  int32_t n_ks;                     // k-steps of 16 latent channels = 2 (n_trips8 + n_trips4)
+  int32_t oct_off[SK_TM_MAX_OCT];   // page byte offset of token slot 0's eight codes (padding slots: 0, read as codes =
+                                    // finite values against zero query rows)
   int32_t oct_rowb[SK_TM_MAX_OCT];  // bytes from one token slot to the next
-  int32_t oct_bits[SK_TM_MAX_OCT];  // 8 or 4
-  int32_t oct_head[SK_TM_MAX_OCT];  // KV head
-  int32_t oct_blk[SK_TM_MAX_OCT];   // precision block (0 = leading)
-  int32_t oct_col[SK_TM_MAX_OCT];   // latent column (in [0, sum r_h)) of the octet's first channel
+  int32_t blk_oct0[2 * STARKV_MAX_KV_HEADS];   // first octet slot of (KV head h, block b) at [2 h + b]
+  int32_t blk_noct[2 * STARKV_MAX_KV_HEADS];   // its octets (consecutive slots)
+  int32_t n_pad, pad_oct[8];        // padding slots
   int32_t win[SK_TM_MAX_KS];        // first score column of the k-step's 16-column window (multiple of 8)
   int32_t ds_cols;                  // score-tile columns (multiple of 16, covers every window); column of
                                     // (KV head h, block b, group member g) = (2 h + b) G + g
   // latent-space query image, per sequence: [constant tile: ds_cols x 16][k-step tiles: n_ks x (hi 512 B, lo 512 B)]
-  // [scalars: float 2^(24 - e)], all B tiles K-major no-swizzle (LBO 128, SBO 256)
+  // [scalars: float 2^(24 - e) per (KV head, block)], all B tiles K-major no-swizzle (LBO 128, SBO 256)
   int32_t img_ks_off, img_scal_off, img_bytes;
   // value side
   int32_t n_vt;                     // 128-channel A tiles = ceil(r_v / 128) <= 2

@@ -771,13 +771,24 @@ int sk_tm_plan(starkv_ctx* ctx) {
         if (bits != want_bits) continue;
         if (n > 128) return 0;
         const int rowb = n * bits / 8;
-        T.blk_oct0[2 * h + blk] = no;
-        T.blk_noct[2 * h + blk] = n / 8;
+        const int hb = 2 * h + blk;
+        // an octet must share its k-step's 16-column window with its partner: if the previous (even) slot's columns are
+        // too far away (a head with an empty block lies between), leave the odd slot empty
+        if (n > 0 && (no & 1) && slot_hb[no - 1] >= 0) {
+          const int ca = slot_hb[no - 1] * G, cb = hb * G;
+          if (cb + G > (ca & ~7) + 16) {
+            if (no >= SK_TM_MAX_OCT || T.n_pad >= 8) return 0;
+            T.pad_oct[T.n_pad++] = no;
+            ++no;
+          }
+        }
+        T.blk_oct0[hb] = no;
+        T.blk_noct[hb] = n / 8;
         for (int oc = 0; oc < n / 8; ++oc) {
           if (no >= SK_TM_MAX_OCT) return 0;
           T.oct_off[no] = (blk ? L.k_lo_off[h] : L.k_hi_off[h]) + oc * bits;   // 8 codes = `bits` bytes
           T.oct_rowb[no] = rowb;
-          slot_hb[no] = 2 * h + blk;
+          slot_hb[no] = hb;
           ++no;
         }
       }
@@ -790,7 +801,8 @@ int sk_tm_plan(starkv_ctx* ctx) {
     else T.n_trips4 = no / 4 - T.n_trips8;
   }
   T.n_ks = no / 2;
-  int need = 2 * (L.n_q_heads <= 8 ? 8 : 32);   // every score column the softmax warps load is initialised by the constant step
+  const int base_cols = 2 * (L.n_q_heads <= 8 ? 8 : 32);   // every score column the softmax warps load is initialised by the
+                                                           // constant step; no window reaches past them
   for (int ks = 0; ks < T.n_ks; ++ks) {
     int ha = slot_hb[2 * ks], hbb = slot_hb[2 * ks + 1];
     if (ha < 0) ha = hbb;
@@ -798,10 +810,12 @@ int sk_tm_plan(starkv_ctx* ctx) {
     if (ha < 0) { T.win[ks] = 0; continue; }   // two padding slots
     const int ca = ha * G, cb = hbb * G;
     const int lo = ca < cb ? ca : cb, hi = (ca > cb ? ca : cb) + G;
-    T.win[ks] = lo & ~7;
-    if (hi > T.win[ks] + 16) return 0;
-    if (T.win[ks] + 16 > need) need = T.win[ks] + 16;
+    int win = lo & ~7;
+    if (win + 16 > base_cols) win = base_cols - 16;
+    T.win[ks] = win;
+    if (lo < win || hi > win + 16) return 0;
   }
+  const int need = base_cols;
   T.ds_cols = round_up(need, 16);
   if (T.ds_cols > 80) return 0;
   T.img_ks_off = T.ds_cols / 8 * 256;

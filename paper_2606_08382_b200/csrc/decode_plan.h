@@ -72,6 +72,7 @@ struct TmPlan {
   int32_t oct_off[SK_TM_MAX_OCT];   // page byte offset of token slot 0's eight codes (padding slots: 0, read as codes =
                                     // finite values against zero query rows)
   int32_t oct_rowb[SK_TM_MAX_OCT];  // bytes from one token slot to the next
+  alignas(16) uint32_t oct_desc[SK_TM_MAX_OCT];   // the two packed for the key-row warps: offset | row bytes << 18
   int32_t blk_oct0[2 * STARKV_MAX_KV_HEADS];   // first octet slot of (KV head h, block b) at [2 h + b]
   int32_t blk_noct[2 * STARKV_MAX_KV_HEADS];   // its octets (consecutive slots)
   int32_t n_pad, pad_oct[8];        // padding slots

@@ -235,10 +235,12 @@ __global__ void __launch_bounds__(TM_THREADS, 1) decode_tm_kernel(
   const uint32_t full0 = smem_u32(smem + T.off_bar);
   const uint32_t empty0 = full0 + 8 * nstage;
   const uint32_t imgbar = empty0 + 8 * nstage;
-  const uint32_t ak_full = imgbar + 8, qk_done = imgbar + 16, ds_free = imgbar + 24, p_full0 = imgbar + 32 /* [2] */,
-                 av_full0 = imgbar + 48 /* [2]: per page */, pv_done0 = imgbar + 64 /* [2]: per P~ buffer */,
-                 pv_half = imgbar + 80 /* the MMAs over the first page's tokens are complete */;
-  volatile uint32_t* tmem_slot = reinterpret_cast<volatile uint32_t*>(smem + T.off_bar + 8 * (2 * nstage) + 96);
+  const uint32_t ak_full0 = imgbar + 8 /* [2]: per half of the k-steps */, qk_done = imgbar + 24, ds_free = imgbar + 32,
+                 p_full0 = imgbar + 40 /* [2] */, av_full0 = imgbar + 56 /* [2]: per page */,
+                 pv_done0 = imgbar + 72 /* [2]: per P~ buffer */,
+                 pv_half = imgbar + 88 /* the value MMAs over the first page's tokens are complete */,
+                 qk_half = imgbar + 96 /* the score MMAs over the first half of the k-steps are complete */;
+  volatile uint32_t* tmem_slot = reinterpret_cast<volatile uint32_t*>(smem + T.off_bar + 8 * (2 * nstage) + 112);
   int32_t* tbl_s = reinterpret_cast<int32_t*>(smem + T.off_tbl);
   float* misc = reinterpret_cast<float*>(smem + T.off_misc);
   uint8_t* stage_base = smem + T.off_stage;
@@ -250,7 +252,9 @@ __global__ void __launch_bounds__(TM_THREADS, 1) decode_tm_kernel(
       mbar_init(empty0 + 8 * s, 2 + 2 * NSPLIT + 4);   // key warps, softmax warps and value warps that read a page
     }
     mbar_init(imgbar, 1);
-    mbar_init(ak_full, 4);
+    mbar_init(ak_full0, 4);
+    mbar_init(ak_full0 + 8, 4);
+    mbar_init(qk_half, 1);
     mbar_init(qk_done, 1);
     mbar_init(ds_free, 4 * NSPLIT);
     mbar_init(p_full0, 4 * NSPLIT);
@@ -294,63 +298,65 @@ __global__ void __launch_bounds__(TM_THREADS, 1) decode_tm_kernel(
       const uint32_t c[8] = {0x04000400u, 0u, 0u, 0u, 0u, 0u, 0u, 0u};   // constant step: (2^-14, 2^-14, 0, ...)
       tmem_st8(tl, c);
     }
-    const int n8 = T.n_trips8, n4 = T.n_trips4;
+    const int n8 = T.n_trips8, nt = T.n_trips8 + T.n_trips4, nt0 = (nt + 1) >> 1;
+    const uint4* desc4 = reinterpret_cast<const uint4*>(T.oct_desc);
     for (int it = 0; it < n_it; ++it) {
       const int j = 2 * it + pgsel;
       const bool exists = j < n_pg;
       const int st = j % nstage;
       if (exists) mbar_wait(full0 + 8 * st, (uint32_t)((j / nstage) & 1));
-      if (it > 0) {   // the previous tile's score MMAs have read the operand
-        mbar_wait(qk_done, (uint32_t)((it - 1) & 1));
-        tc_fence_after();
-      }
       const uint8_t* row = stage_base + (size_t)st * page_bytes;
-      // Four octets (two k-steps) per trip, branch-free: loads, conversions, one 16-column store.  The slot offsets and
-      // row strides are warp-uniform plan entries (constant bank), so an address costs one multiply-add.
+      // Four octets (two k-steps) per trip: packed plan entries (page offset | row bytes << 18), loads, conversions, one
+      // 16-column store.  The k-steps are handed to the MMA warp in two halves, so that the next tile's first half is
+      // converted while the tensor core still reads this tile's second half.
+#pragma unroll 1
+      for (int half = 0; half < 2; ++half) {
+        if (it > 0) {   // the previous tile's score MMAs over this half have read the operand
+          mbar_wait(half ? qk_done : qk_half, (uint32_t)((it - 1) & 1));
+          tc_fence_after();
+        }
+        const int k_end = half ? nt : nt0;
+#pragma unroll 2
+        for (int k2 = half ? nt0 : 0; k2 < k_end; ++k2) {
+          const uint4 dq = desc4[k2];
+          const uint32_t dsc[4] = {dq.x, dq.y, dq.z, dq.w};
+          const uint8_t* p[4];
 #pragma unroll
-      for (int k2 = 0; k2 < SK_TM_MAX_TRIPS; ++k2) {
-        if (k2 < n8) {   // 8-bit fields: (u0, u1), (u2, u3), ... as fp16 subnormals u 2^-24
-          uint2 x[4];
-#pragma unroll
-          for (int oo = 0; oo < 4; ++oo)
-            x[oo] = *reinterpret_cast<const uint2*>(row + T.oct_off[4 * k2 + oo] + slot * T.oct_rowb[4 * k2 + oo]);
+          for (int oo = 0; oo < 4; ++oo) p[oo] = row + (dsc[oo] & 0x3ffffu) + slot * (dsc[oo] >> 18);
           uint32_t r[16];
+          if (k2 < n8) {   // 8-bit fields: (u0, u1), (u2, u3), ... as fp16 subnormals u 2^-24
+            uint2 x[4];
 #pragma unroll
-          for (int oo = 0; oo < 4; ++oo) {
-            r[4 * oo] = prmt(x[oo].x, 0u, 0x4140u);
-            r[4 * oo + 1] = prmt(x[oo].x, 0u, 0x4342u);
-            r[4 * oo + 2] = prmt(x[oo].y, 0u, 0x4140u);
-            r[4 * oo + 3] = prmt(x[oo].y, 0u, 0x4342u);
+            for (int oo = 0; oo < 4; ++oo) x[oo] = *reinterpret_cast<const uint2*>(p[oo]);
+#pragma unroll
+            for (int oo = 0; oo < 4; ++oo) {
+              r[4 * oo] = prmt(x[oo].x, 0u, 0x4140u);
+              r[4 * oo + 1] = prmt(x[oo].x, 0u, 0x4342u);
+              r[4 * oo + 2] = prmt(x[oo].y, 0u, 0x4140u);
+              r[4 * oo + 3] = prmt(x[oo].y, 0u, 0x4342u);
+            }
+          } else {         // 4-bit fields: (u0, u4), 16 (u1, u5), (u2, u6), 16 (u3, u7); the 16 is taken out of the query image
+            uint32_t w[4];
+#pragma unroll
+            for (int oo = 0; oo < 4; ++oo) w[oo] = *reinterpret_cast<const uint32_t*>(p[oo]);
+#pragma unroll
+            for (int oo = 0; oo < 4; ++oo) {
+              const uint32_t w2 = w[oo] >> 8;
+              r[4 * oo] = w[oo] & 0x000f000fu;
+              r[4 * oo + 1] = w[oo] & 0x00f000f0u;
+              r[4 * oo + 2] = w2 & 0x000f000fu;
+              r[4 * oo + 3] = w2 & 0x00f000f0u;
+            }
           }
           tmem_st16(tl + 8 + 16 * k2, r);
         }
-      }
-#pragma unroll
-      for (int k2 = 0; k2 < SK_TM_MAX_TRIPS; ++k2) {
-        if (k2 < n4) {   // 4-bit fields: (u0, u4), 16 (u1, u5), (u2, u6), 16 (u3, u7); the 16 is taken out of the query image
-          const int o0 = 4 * (n8 + k2);
-          uint32_t w[4];
-#pragma unroll
-          for (int oo = 0; oo < 4; ++oo)
-            w[oo] = *reinterpret_cast<const uint32_t*>(row + T.oct_off[o0 + oo] + slot * T.oct_rowb[o0 + oo]);
-          uint32_t r[16];
-#pragma unroll
-          for (int oo = 0; oo < 4; ++oo) {
-            const uint32_t w2 = w[oo] >> 8;
-            r[4 * oo] = w[oo] & 0x000f000fu;
-            r[4 * oo + 1] = w[oo] & 0x00f000f0u;
-            r[4 * oo + 2] = w2 & 0x000f000fu;
-            r[4 * oo + 3] = w2 & 0x00f000f0u;
-          }
-          tmem_st16(tl + 8 + 16 * (n8 + k2), r);
+        tmem_wait_st();
+        tc_fence_before();
+        __syncwarp();
+        if (lane == 0) {
+          mbar_arrive(ak_full0 + 8 * half);
+          if (half && exists) mbar_arrive(empty0 + 8 * st);
         }
-      }
-      tmem_wait_st();
-      tc_fence_before();
-      __syncwarp();
-      if (lane == 0) {
-        mbar_arrive(ak_full);
-        if (exists) mbar_arrive(empty0 + 8 * st);
       }
     }
   } else if (warp < 12) {
@@ -441,7 +447,10 @@ __global__ void __launch_bounds__(TM_THREADS, 1) decode_tm_kernel(
         bool trig = valid && (mxa > TAU || sv0 > M0 || sv1 > M1);
         if (it == 0) trig = true;
         const bool wany = __any_sync(0xffffffffu, trig);
-        if (lane == 0) flag[buf * 8 + wr] = wany ? 1 : 0;
+        if (lane == 0) {
+          flag[buf * 8 + wr] = wany ? 1 : 0;
+          if (exists) mbar_arrive(empty0 + 8 * st);   // every scale of the page has been used: the stage may be refilled
+        }
         bar_sync(BAR_SM, NBAR);
         const volatile uint32_t* flw = reinterpret_cast<const volatile uint32_t*>(flag + buf * 8);
         const bool upd = (flw[0] | flw[1]) != 0u;
@@ -535,10 +544,7 @@ __global__ void __launch_bounds__(TM_THREADS, 1) decode_tm_kernel(
         }
         fence_proxy_async();   // generic-proxy stores -> visible to the tensor core's reads
         __syncwarp();
-        if (lane == 0) {
-          mbar_arrive(p_full0 + 8 * buf);
-          if (exists) mbar_arrive(empty0 + 8 * st);
-        }
+        if (lane == 0) mbar_arrive(p_full0 + 8 * buf);
       }
       // ---- split-K partial (D7): [m, l, 0, 0, acc[r_v]] per head
       {
@@ -593,7 +599,7 @@ __global__ void __launch_bounds__(TM_THREADS, 1) decode_tm_kernel(
       roff[m] = act[m] ? (lo ? L.v_lo_off + (ch - L.v_hi_n) * rowb : L.v_hi_off + ch * rowb) : 0;
     }
     for (int it = 0; it < n_it; ++it) {
-#pragma unroll
+#pragma unroll 1
       for (int pg = 0; pg < 2; ++pg) {
         const int j = 2 * it + pg;
         const bool exists = j < n_pg;
@@ -666,25 +672,26 @@ __global__ void __launch_bounds__(TM_THREADS, 1) decode_tm_kernel(
       const uint64_t dks = umma_desc(img_s + (uint32_t)T.img_ks_off, 128, 256);
       const uint32_t id_const = umma_idesc_f16(T.ds_cols, false), id_win = umma_idesc_f16(16, false);
       const uint32_t t_ds = tbase + (uint32_t)T.col_ds, t_ak = tbase + (uint32_t)T.col_ak;
-      const int n_ks = T.n_ks;
+      const int n_ks = T.n_ks, ks_half = 2 * ((T.n_trips8 + T.n_trips4 + 1) >> 1);
       for (int it = 0; it < n_it; ++it) {
-        mbar_wait(ak_full, (uint32_t)(it & 1));
-        if (it > 0) mbar_wait(ds_free, (uint32_t)((it - 1) & 1));
-        tc_fence_after();
-        if (elect_one()) {
-          umma_ts_f16(t_ds, t_ak, dconst, id_const, 0u);
-          // unrolled over the k-steps: window columns, operand columns and descriptors are constants of the instruction stream
-#pragma unroll
-          for (int ks = 0; ks < SK_TM_MAX_KS; ++ks) {
-            if (ks < n_ks) {
+#pragma unroll 1
+        for (int half = 0; half < 2; ++half) {
+          mbar_wait(ak_full0 + 8 * half, (uint32_t)(it & 1));
+          if (half == 0 && it > 0) mbar_wait(ds_free, (uint32_t)((it - 1) & 1));
+          tc_fence_after();
+          if (elect_one()) {
+            if (half == 0) umma_ts_f16(t_ds, t_ak, dconst, id_const, 0u);
+            const int ks_end = half ? n_ks : ks_half;
+#pragma unroll 2
+            for (int ks = half ? ks_half : 0; ks < ks_end; ++ks) {
               const uint32_t dcol = t_ds + (uint32_t)T.win[ks];
               umma_ts_f16(dcol, t_ak + 8 + 8 * ks, dks + (uint64_t)(ks * 64), id_win, 1u);
               umma_ts_f16(dcol, t_ak + 8 + 8 * ks, dks + (uint64_t)(ks * 64 + 32), id_win, 1u);
             }
+            umma_commit(half ? qk_done : qk_half);
           }
-          umma_commit(qk_done);
+          __syncwarp();
         }
-        __syncwarp();
       }
     } else if (warp == 18) {
       // ================================== value MMAs ==================================
@@ -801,6 +808,10 @@ int sk_tm_plan(starkv_ctx* ctx) {
     else T.n_trips4 = no / 4 - T.n_trips8;
   }
   T.n_ks = no / 2;
+  for (int o = 0; o < SK_TM_MAX_OCT; ++o) {
+    if (T.oct_off[o] >= (1 << 18) || T.oct_rowb[o] >= (1 << 14)) return 0;
+    T.oct_desc[o] = (uint32_t)T.oct_off[o] | ((uint32_t)T.oct_rowb[o] << 18);
+  }
   const int base_cols = 2 * (L.n_q_heads <= 8 ? 8 : 32);   // every score column the softmax warps load is initialised by the
                                                            // constant step; no window reaches past them
   for (int ks = 0; ks < T.n_ks; ++ks) {

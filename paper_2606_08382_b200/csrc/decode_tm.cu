@@ -26,11 +26,12 @@
 //   PV   O[channel, head] += c[channel, token] P~[token, head]:  A = exact signed codes (magic-number trick), B = P~ of
 //        the channel's block; a 128-channel A tile that straddles the block boundary is multiplied with both operands
 //        into two accumulator tiles and each lane keeps its own.
-// Warp roles (20 warps, warpgroup-aligned so that setmaxnreg can move registers between them; the CTA owns 640 x 96
-// registers and the budgets 4 x 80 + 8 x 112 + 4 x 128 + 4 x 48 add up to exactly that -- setmaxnreg.inc can only
+// Warp roles (24 warps, warpgroup-aligned so that setmaxnreg can move registers between them; the CTA owns 768 x 80
+// registers and the budgets 8 x 64 + 8 x 104 + 4 x 104 + 4 x 40 add up to exactly that -- setmaxnreg.inc can only
 // take what another warpgroup of the CTA released):
-//   0-3 key rows -> TMEM, 4-7 / 8-11 softmax of the lower / upper half of the query heads, 12-15 value rows -> TMEM,
-//   16 page producer (cp.async.bulk ring), 17 QK MMA issue, 18 PV MMA issue, 19 TMEM allocation.
+//   0-3 / 4-7 key rows -> TMEM for the first / second half of the k-steps, 8-11 / 12-15 softmax of the lower / upper
+//   half of the query heads, 16-19 value rows -> TMEM, 20 page producer (cp.async.bulk ring), 21 QK MMA issue,
+//   22 PV MMA issue, 23 TMEM allocation.
 // All hand-offs are mbarriers; there is no CTA-wide barrier in the loop.  The value operand is handed over per page
 // (two halves of the 128 tokens), so that the next tile's value rows are converted while the MMAs of this one run.
 #include <string.h>
@@ -44,7 +45,7 @@ using namespace skptx;
 namespace {
 
 constexpr int PTOK = 64;              // tokens per page on this path
-constexpr int TM_THREADS = 640;
+constexpr int TM_THREADS = 768;
 constexpr int TM_TBL = 512;           // block-table entries of the CTA's range kept in shared memory
 constexpr float P_OFFSET = 8.f;       // p' = 2^(s - m + 8)
 constexpr float TAU = 6.f;            // the running maximum may lag the true one by 2^TAU: p' <= 2^14
@@ -249,7 +250,7 @@ __global__ void __launch_bounds__(TM_THREADS, 1) decode_tm_kernel(
   if (tid == 0) {
     for (int s = 0; s < nstage; ++s) {
       mbar_init(full0 + 8 * s, 1);
-      mbar_init(empty0 + 8 * s, 2 + 2 * NSPLIT + 4);   // key warps, softmax warps and value warps that read a page
+      mbar_init(empty0 + 8 * s, 4 + 2 * NSPLIT + 4);   // key warps, softmax warps and value warps that read a page
     }
     mbar_init(imgbar, 1);
     mbar_init(ak_full0, 4);
@@ -266,7 +267,7 @@ __global__ void __launch_bounds__(TM_THREADS, 1) decode_tm_kernel(
     mbar_init(pv_half, 1);
     fence_barrier_init();
   }
-  if (warp == 19) tmem_alloc(smem_u32((const void*)tmem_slot), TM_COLS);
+  if (warp == 23) tmem_alloc(smem_u32((const void*)tmem_slot), TM_COLS);
   if (tid < 36) misc[tid] = tid < 34 ? 0.f : 1.f;   // m = 0, M = 0 (forces the first update), 1/M = 1
 
   sk_pdl_wait();   // seq_lens, block table, query image, pages: nothing global is read before this point
@@ -289,82 +290,80 @@ __global__ void __launch_bounds__(TM_THREADS, 1) decode_tm_kernel(
 
   if (n_pg <= 0) {   // empty range (CTA-uniform): neutral partial
     for (int i = tid; i < L.n_q_heads * (int)pstride; i += TM_THREADS) my_parts[i] = (i % (int)pstride) == 0 ? -INFINITY : 0.f;
-  } else if (warp < 4) {
+  } else if (warp < 8) {
     // =============================== key rows -> A operand of the score product ===============================
-    setmaxnreg_dec<80>();
-    const int wq = warp, tq = wq * 32 + lane, pgsel = tq >> 6, slot = tq & 63;
+    // warps 0-3 convert the first half of the k-steps, warps 4-7 the second half (each warp its own 32 tokens = lanes)
+    setmaxnreg_dec<64>();
+    const int wq = warp & 3, half = warp >> 2, tq = wq * 32 + lane, pgsel = tq >> 6, slot = tq & 63;
     const uint32_t tl = tbase + ((uint32_t)(wq * 32) << 16) + (uint32_t)T.col_ak;
-    {
+    if (half == 0) {
       const uint32_t c[8] = {0x04000400u, 0u, 0u, 0u, 0u, 0u, 0u, 0u};   // constant step: (2^-14, 2^-14, 0, ...)
       tmem_st8(tl, c);
     }
     const int n8 = T.n_trips8, nt = T.n_trips8 + T.n_trips4, nt0 = (nt + 1) >> 1;
+    const int k_begin = half ? nt0 : 0, k_end = half ? nt : nt0;
     const uint4* desc4 = reinterpret_cast<const uint4*>(T.oct_desc);
     for (int it = 0; it < n_it; ++it) {
       const int j = 2 * it + pgsel;
       const bool exists = j < n_pg;
       const int st = j % nstage;
+      uint4 dq = desc4[k_begin];
       if (exists) mbar_wait(full0 + 8 * st, (uint32_t)((j / nstage) & 1));
       const uint8_t* row = stage_base + (size_t)st * page_bytes;
-      // Four octets (two k-steps) per trip: packed plan entries (page offset | row bytes << 18), loads, conversions, one
-      // 16-column store.  The k-steps are handed to the MMA warp in two halves, so that the next tile's first half is
-      // converted while the tensor core still reads this tile's second half.
-#pragma unroll 1
-      for (int half = 0; half < 2; ++half) {
-        if (it > 0) {   // the previous tile's score MMAs over this half have read the operand
-          mbar_wait(half ? qk_done : qk_half, (uint32_t)((it - 1) & 1));
-          tc_fence_after();
-        }
-        const int k_end = half ? nt : nt0;
+      if (it > 0) {   // the previous tile's score MMAs over this half have read the operand
+        mbar_wait(half ? qk_done : qk_half, (uint32_t)((it - 1) & 1));
+        tc_fence_after();
+      }
+      // Four octets (two k-steps) per trip: packed plan entries (page offset | row bytes << 18; the next trip's entry is
+      // fetched a trip ahead), loads, conversions, one 16-column store.
 #pragma unroll 2
-        for (int k2 = half ? nt0 : 0; k2 < k_end; ++k2) {
-          const uint4 dq = desc4[k2];
-          const uint32_t dsc[4] = {dq.x, dq.y, dq.z, dq.w};
-          const uint8_t* p[4];
+      for (int k2 = k_begin; k2 < k_end; ++k2) {
+        const uint32_t dsc[4] = {dq.x, dq.y, dq.z, dq.w};
+        dq = desc4[k2 + 1 < SK_TM_MAX_TRIPS ? k2 + 1 : k2];
+        const uint8_t* p[4];
 #pragma unroll
-          for (int oo = 0; oo < 4; ++oo) p[oo] = row + (dsc[oo] & 0x3ffffu) + slot * (dsc[oo] >> 18);
-          uint32_t r[16];
-          if (k2 < n8) {   // 8-bit fields: (u0, u1), (u2, u3), ... as fp16 subnormals u 2^-24
-            uint2 x[4];
+        for (int oo = 0; oo < 4; ++oo) p[oo] = row + (dsc[oo] & 0x3ffffu) + slot * (dsc[oo] >> 18);
+        uint32_t r[16];
+        if (k2 < n8) {   // 8-bit fields: (u0, u1), (u2, u3), ... as fp16 subnormals u 2^-24
+          uint2 x[4];
 #pragma unroll
-            for (int oo = 0; oo < 4; ++oo) x[oo] = *reinterpret_cast<const uint2*>(p[oo]);
+          for (int oo = 0; oo < 4; ++oo) x[oo] = *reinterpret_cast<const uint2*>(p[oo]);
 #pragma unroll
-            for (int oo = 0; oo < 4; ++oo) {
-              r[4 * oo] = prmt(x[oo].x, 0u, 0x4140u);
-              r[4 * oo + 1] = prmt(x[oo].x, 0u, 0x4342u);
-              r[4 * oo + 2] = prmt(x[oo].y, 0u, 0x4140u);
-              r[4 * oo + 3] = prmt(x[oo].y, 0u, 0x4342u);
-            }
-          } else {         // 4-bit fields: (u0, u4), 16 (u1, u5), (u2, u6), 16 (u3, u7); the 16 is taken out of the query image
-            uint32_t w[4];
-#pragma unroll
-            for (int oo = 0; oo < 4; ++oo) w[oo] = *reinterpret_cast<const uint32_t*>(p[oo]);
-#pragma unroll
-            for (int oo = 0; oo < 4; ++oo) {
-              const uint32_t w2 = w[oo] >> 8;
-              r[4 * oo] = w[oo] & 0x000f000fu;
-              r[4 * oo + 1] = w[oo] & 0x00f000f0u;
-              r[4 * oo + 2] = w2 & 0x000f000fu;
-              r[4 * oo + 3] = w2 & 0x00f000f0u;
-            }
+          for (int oo = 0; oo < 4; ++oo) {
+            r[4 * oo] = prmt(x[oo].x, 0u, 0x4140u);
+            r[4 * oo + 1] = prmt(x[oo].x, 0u, 0x4342u);
+            r[4 * oo + 2] = prmt(x[oo].y, 0u, 0x4140u);
+            r[4 * oo + 3] = prmt(x[oo].y, 0u, 0x4342u);
           }
-          tmem_st16(tl + 8 + 16 * k2, r);
+        } else {         // 4-bit fields: (u0, u4), 16 (u1, u5), (u2, u6), 16 (u3, u7); the 16 is taken out of the query image
+          uint32_t w[4];
+#pragma unroll
+          for (int oo = 0; oo < 4; ++oo) w[oo] = *reinterpret_cast<const uint32_t*>(p[oo]);
+#pragma unroll
+          for (int oo = 0; oo < 4; ++oo) {
+            const uint32_t w2 = w[oo] >> 8;
+            r[4 * oo] = w[oo] & 0x000f000fu;
+            r[4 * oo + 1] = w[oo] & 0x00f000f0u;
+            r[4 * oo + 2] = w2 & 0x000f000fu;
+            r[4 * oo + 3] = w2 & 0x00f000f0u;
+          }
         }
-        tmem_wait_st();
-        tc_fence_before();
-        __syncwarp();
-        if (lane == 0) {
-          mbar_arrive(ak_full0 + 8 * half);
-          if (half && exists) mbar_arrive(empty0 + 8 * st);
-        }
+        tmem_st16(tl + 8 + 16 * k2, r);
+      }
+      tmem_wait_st();
+      tc_fence_before();
+      __syncwarp();
+      if (lane == 0) {
+        mbar_arrive(ak_full0 + 8 * half);
+        if (exists) mbar_arrive(empty0 + 8 * st);
       }
     }
-  } else if (warp < 12) {
+  } else if (warp < 16) {
     // ========================================= softmax (thread = token) =========================================
-    setmaxnreg_inc<112>();
-    const int hh = (warp - 4) >> 2;   // which half of the query heads
+    setmaxnreg_inc<104>();
+    const int hh = (warp - 8) >> 2;   // which half of the query heads
     if (hh < NSPLIT) {
-      const int wq = warp & 3, wr = warp - 4, tq = wq * 32 + lane, pgsel = tq >> 6, slot = tq & 63;
+      const int wq = warp & 3, wr = warp - 8, tq = wq * 32 + lane, pgsel = tq >> 6, slot = tq & 63;
       const int hbase = hh * NHH;     // first query head of this warpgroup
       const uint32_t tlane = tbase + ((uint32_t)(wq * 32) << 16);
       float* mref_s = misc + MISC_MREF;
@@ -424,9 +423,6 @@ __global__ void __launch_bounds__(TM_THREADS, 1) decode_tm_kernel(
           sv0 = h_bits_to_f(vsc[0]);
           sv1 = h_bits_to_f(vsc[PTOK]);
         }
-        float mr[NHH];
-#pragma unroll
-        for (int i = 0; i < NHH; ++i) mr[i] = mref_s[hbase + i];
         const float M0 = M_s[0], M1 = M_s[1];
         tmem_wait_ld();
         tc_fence_before();
@@ -440,7 +436,7 @@ __global__ void __launch_bounds__(TM_THREADS, 1) decode_tm_kernel(
           for (int g = 0; g < G; ++g) {
             const int i = hl * G + g;
             const float s = fmaf(sc[2 * hl], __uint_as_float(d[2 * hl * G + g]), sc[2 * hl + 1] * __uint_as_float(d[2 * hl * G + G + g]));
-            arg[i] = valid ? s - mr[i] : -INFINITY;
+            arg[i] = valid ? s - mref_s[hbase + i] : -INFINITY;
             if (hbase + i < Hq) mxa = fmaxf(mxa, arg[i]);
           }
         }
@@ -458,7 +454,7 @@ __global__ void __launch_bounds__(TM_THREADS, 1) decode_tm_kernel(
           // ---- a maximum (or a value-scale bound) moves: new reference, rescale the running sums and the accumulators
 #pragma unroll
           for (int i = 0; i < NHH; ++i) {
-            const float v = valid ? arg[i] + mr[i] : -INFINITY;   // the score itself
+            const float v = valid ? arg[i] + mref_s[hbase + i] : -INFINITY;   // the score itself
             const int k = __reduce_max_sync(0xffffffffu, f_ordered(v));
             if (lane == 0) red[wr * RED_STRIDE + i] = k;
           }
@@ -473,7 +469,7 @@ __global__ void __launch_bounds__(TM_THREADS, 1) decode_tm_kernel(
 #pragma unroll
           for (int i = 0; i < NHH; ++i) {
             const float mt = f_unordered(max(max(redh[i], redh[RED_STRIDE + i]), max(redh[2 * RED_STRIDE + i], redh[3 * RED_STRIDE + i])));
-            const float m_old = mr[i];
+            const float m_old = mref_s[hbase + i];
             // only a maximum that the tile exceeds moves (to the true maximum so far); the first tile sets it
             float m_new = (it == 0) ? mt : (mt > m_old ? mt : m_old);
             if (!(m_new > -INFINITY)) m_new = m_old;
@@ -581,10 +577,10 @@ __global__ void __launch_bounds__(TM_THREADS, 1) decode_tm_kernel(
         }
       }
     }
-  } else if (warp < 16) {
+  } else if (warp < 20) {
     // =============================== value rows -> A operand of the value product ===============================
-    setmaxnreg_inc<128>();
-    const int wq = warp - 12, tq = wq * 32 + lane;
+    setmaxnreg_inc<104>();
+    const int wq = warp - 16, tq = wq * 32 + lane;
     const uint32_t tl = tbase + ((uint32_t)(wq * 32) << 16) + (uint32_t)T.col_av;
     int roff[2];
     bool four[2], act[2];
@@ -647,8 +643,8 @@ __global__ void __launch_bounds__(TM_THREADS, 1) decode_tm_kernel(
       }
     }
   } else {
-    setmaxnreg_dec<48>();
-    if (warp == 16) {
+    setmaxnreg_dec<40>();
+    if (warp == 20) {
       // ================================== page producer (D2) ==================================
       if (elect_one()) {
         const uint64_t pol = l2_evict_first_policy();
@@ -664,7 +660,7 @@ __global__ void __launch_bounds__(TM_THREADS, 1) decode_tm_kernel(
         }
       }
       __syncwarp();
-    } else if (warp == 17) {
+    } else if (warp == 21) {
       // ================================== score MMAs ==================================
       mbar_wait(imgbar, 0);
       const uint32_t img_s = smem_u32(smem + T.off_img);
@@ -693,7 +689,7 @@ __global__ void __launch_bounds__(TM_THREADS, 1) decode_tm_kernel(
           __syncwarp();
         }
       }
-    } else if (warp == 18) {
+    } else if (warp == 22) {
       // ================================== value MMAs ==================================
       const uint32_t id_pv = umma_idesc_f16(32, true);
       const uint32_t t_do = tbase + (uint32_t)T.col_do, t_av = tbase + (uint32_t)T.col_av;
@@ -735,7 +731,7 @@ __global__ void __launch_bounds__(TM_THREADS, 1) decode_tm_kernel(
 
   tc_fence_before();
   __syncthreads();
-  if (warp == 19) tmem_dealloc(tbase, TM_COLS);
+  if (warp == 23) tmem_dealloc(tbase, TM_COLS);
 }
 
 typedef void (*TmKernel)(const StarkvLayout, const TmPlan, const uint8_t*, size_t, const uint8_t*, const int32_t*, int,

@@ -88,6 +88,7 @@ struct TmPlan {
   int32_t dt_tile[4], dt_blk[4];
   // tensor memory columns
   int32_t col_do, col_av, col_ak, col_ds;
+  int32_t ds_nbuf;                  // score tiles in tensor memory: 2 (double-buffered) where they fit, else 1
   // shared memory (bytes from the 1024-aligned base)
   int32_t nstage;                   // page ring depth
   int32_t off_stage, off_img, off_p, off_misc, off_bar, off_tbl, smem_bytes;

@@ -236,12 +236,15 @@ __global__ void __launch_bounds__(TM_THREADS, 1) decode_tm_kernel(
   const uint32_t full0 = smem_u32(smem + T.off_bar);
   const uint32_t empty0 = full0 + 8 * nstage;
   const uint32_t imgbar = empty0 + 8 * nstage;
-  const uint32_t ak_full0 = imgbar + 8 /* [2]: per half of the k-steps */, qk_done = imgbar + 24, ds_free = imgbar + 32,
-                 p_full0 = imgbar + 40 /* [2] */, av_full0 = imgbar + 56 /* [2]: per page */,
-                 pv_done0 = imgbar + 72 /* [2]: per P~ buffer */,
-                 pv_half = imgbar + 88 /* the value MMAs over the first page's tokens are complete */,
-                 qk_half = imgbar + 96 /* the score MMAs over the first half of the k-steps are complete */;
-  volatile uint32_t* tmem_slot = reinterpret_cast<volatile uint32_t*>(smem + T.off_bar + 8 * (2 * nstage) + 112);
+  const uint32_t ak_full0 = imgbar + 8 /* [2]: per half of the k-steps */, qk_done0 = imgbar + 24 /* [2]: per score buffer */,
+                 ds_free0 = imgbar + 40 /* [2]: per score buffer */, p_full0 = imgbar + 56 /* [2] */,
+                 av_full0 = imgbar + 72 /* [2]: per page */, pv_done0 = imgbar + 88 /* [2]: per P~ buffer */,
+                 pv_half = imgbar + 104 /* the value MMAs over the first page's tokens are complete */,
+                 qk_half = imgbar + 112 /* the score MMAs over the first half of the k-steps are complete */;
+  volatile uint32_t* tmem_slot = reinterpret_cast<volatile uint32_t*>(smem + T.off_bar + 8 * (2 * nstage) + 128);
+  // the score tile is double-buffered when tensor memory has room (T.ds_nbuf = 2): tile `it` uses buffer it % ds_nbuf, so the
+  // score MMAs of the next tile run while the softmax warps still read this one
+  const int ds_nbuf = T.ds_nbuf;
   int32_t* tbl_s = reinterpret_cast<int32_t*>(smem + T.off_tbl);
   float* misc = reinterpret_cast<float*>(smem + T.off_misc);
   uint8_t* stage_base = smem + T.off_stage;
@@ -256,8 +259,10 @@ __global__ void __launch_bounds__(TM_THREADS, 1) decode_tm_kernel(
     mbar_init(ak_full0, 4);
     mbar_init(ak_full0 + 8, 4);
     mbar_init(qk_half, 1);
-    mbar_init(qk_done, 1);
-    mbar_init(ds_free, 4 * NSPLIT);
+    mbar_init(qk_done0, 1);
+    mbar_init(qk_done0 + 8, 1);
+    mbar_init(ds_free0, 4 * NSPLIT);
+    mbar_init(ds_free0 + 8, 4 * NSPLIT);
     mbar_init(p_full0, 4 * NSPLIT);
     mbar_init(p_full0 + 8, 4 * NSPLIT);
     mbar_init(av_full0, 4);
@@ -311,7 +316,9 @@ __global__ void __launch_bounds__(TM_THREADS, 1) decode_tm_kernel(
       if (exists) mbar_wait(full0 + 8 * st, (uint32_t)((j / nstage) & 1));
       const uint8_t* row = stage_base + (size_t)st * page_bytes;
       if (it > 0) {   // the previous tile's score MMAs over this half have read the operand
-        mbar_wait(half ? qk_done : qk_half, (uint32_t)((it - 1) & 1));
+        const int pb = (it - 1) % ds_nbuf;
+        if (half) mbar_wait(qk_done0 + 8 * pb, (uint32_t)(((it - 1) / ds_nbuf) & 1));
+        else mbar_wait(qk_half, (uint32_t)((it - 1) & 1));
         tc_fence_after();
       }
       // Four octets (two k-steps) per trip: packed plan entries (page offset | row bytes << 18; the next trip's entry is
@@ -397,10 +404,11 @@ __global__ void __launch_bounds__(TM_THREADS, 1) decode_tm_kernel(
         const bool exists = j < n_pg;
         const int st = j % nstage;
         const int buf = it & 1;
-        mbar_wait(qk_done, (uint32_t)(it & 1));
+        const int sb = it % ds_nbuf;
+        mbar_wait(qk_done0 + 8 * sb, (uint32_t)((it / ds_nbuf) & 1));
         tc_fence_after();
         uint32_t d[2 * NHH];
-        tmem_ld<2 * NHH>(tlane + (uint32_t)(T.col_ds + 2 * hbase), d);
+        tmem_ld<2 * NHH>(tlane + (uint32_t)(T.col_ds + sb * T.ds_cols + 2 * hbase), d);
         if (exists) mbar_wait(full0 + 8 * st, (uint32_t)((j / nstage) & 1));
         const uint8_t* page = stage_base + (size_t)st * page_bytes;
         const uint16_t* ksc = reinterpret_cast<const uint16_t*>(page + L.k_scale_off) + slot;
@@ -427,7 +435,7 @@ __global__ void __launch_bounds__(TM_THREADS, 1) decode_tm_kernel(
         tmem_wait_ld();
         tc_fence_before();
         __syncwarp();
-        if (lane == 0) mbar_arrive(ds_free);
+        if (lane == 0) mbar_arrive(ds_free0 + 8 * sb);
         float arg[NHH];
         float mxa = -INFINITY;
 #pragma unroll
@@ -672,19 +680,21 @@ __global__ void __launch_bounds__(TM_THREADS, 1) decode_tm_kernel(
       for (int it = 0; it < n_it; ++it) {
 #pragma unroll 1
         for (int half = 0; half < 2; ++half) {
+          const int sb = it % ds_nbuf;
+          const uint32_t t_dsb = t_ds + (uint32_t)(sb * T.ds_cols);
           mbar_wait(ak_full0 + 8 * half, (uint32_t)(it & 1));
-          if (half == 0 && it > 0) mbar_wait(ds_free, (uint32_t)((it - 1) & 1));
+          if (half == 0 && it >= ds_nbuf) mbar_wait(ds_free0 + 8 * sb, (uint32_t)(((it / ds_nbuf) - 1) & 1));   // tile it - ds_nbuf has been read
           tc_fence_after();
           if (elect_one()) {
-            if (half == 0) umma_ts_f16(t_ds, t_ak, dconst, id_const, 0u);
+            if (half == 0) umma_ts_f16(t_dsb, t_ak, dconst, id_const, 0u);
             const int ks_end = half ? n_ks : ks_half;
 #pragma unroll 2
             for (int ks = half ? ks_half : 0; ks < ks_end; ++ks) {
-              const uint32_t dcol = t_ds + (uint32_t)T.win[ks];
+              const uint32_t dcol = t_dsb + (uint32_t)T.win[ks];
               umma_ts_f16(dcol, t_ak + 8 + 8 * ks, dks + (uint64_t)(ks * 64), id_win, 1u);
               umma_ts_f16(dcol, t_ak + 8 + 8 * ks, dks + (uint64_t)(ks * 64 + 32), id_win, 1u);
             }
-            umma_commit(half ? qk_done : qk_half);
+            umma_commit(half ? qk_done0 + 8 * sb : qk_half);
           }
           __syncwarp();
         }
@@ -824,7 +834,7 @@ int sk_tm_plan(starkv_ctx* ctx) {
   }
   const int need = base_cols;
   T.ds_cols = round_up(need, 16);
-  if (T.ds_cols > 80) return 0;
+  if (T.ds_cols > 64) return 0;
   T.img_ks_off = T.ds_cols / 8 * 256;
   T.img_scal_off = T.img_ks_off + T.n_ks * 1024;
   T.img_bytes = T.img_scal_off + 2 * 32 * 4;
@@ -835,7 +845,14 @@ int sk_tm_plan(starkv_ctx* ctx) {
     if (c0 < L.v_hi_n) { T.dt_tile[T.n_dt] = t; T.dt_blk[T.n_dt] = 0; ++T.n_dt; }
     if (c1 > L.v_hi_n) { T.dt_tile[T.n_dt] = t; T.dt_blk[T.n_dt] = 1; ++T.n_dt; }
   }
-  T.col_do = 0; T.col_av = 128; T.col_ak = 256; T.col_ds = 256 + 8 + 8 * SK_TM_MAX_KS;   // 424; score tile <= 80 columns
+  // tensor memory: accumulators (32 columns per tile), value operand (64 per 128-channel tile), key operand (constant step +
+  // 8 per k-step), score tile(s)
+  T.col_do = 0;
+  T.col_av = 32 * T.n_dt;
+  T.col_ak = T.col_av + 64 * T.n_vt;
+  T.col_ds = T.col_ak + 8 + 8 * T.n_ks;
+  T.ds_nbuf = (T.col_ds + 2 * T.ds_cols <= 512) ? 2 : 1;
+  if (T.col_ds + T.ds_nbuf * T.ds_cols > 512) return 0;
   int off = 0;
   const int fixed = round_up(T.img_bytes, 128) + 2 * 2 * P_BLK_BYTES + 1024 /* misc */ + 512 /* barriers */ + 4 * TM_TBL +
                     1024 /* base alignment */;

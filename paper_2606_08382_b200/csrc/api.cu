@@ -83,6 +83,12 @@ int starkv_create(starkv_ctx** out, const starkv_desc* d, void* cuda_stream) {
     return STARKV_ERR_CUDA;
   }
   ctx->pdl = 1;
+  if (cudaMalloc((void**)&ctx->tickets, SK_TICKETS * sizeof(int)) != cudaSuccess ||
+      cudaMemset(ctx->tickets, 0, SK_TICKETS * sizeof(int)) != cudaSuccess) {
+    (void)cudaGetLastError();
+    if (ctx->tickets) cudaFree(ctx->tickets);
+    ctx->tickets = nullptr;   // the sliced combine is skipped
+  }
   sk_fast_plan(ctx);
   sk_tm_plan(ctx);
   *out = ctx;
@@ -98,6 +104,7 @@ void starkv_destroy(starkv_ctx* ctx) {
     if (ctx->g_app[i].exec) cudaGraphExecDestroy(ctx->g_app[i].exec);
   }
   if (ctx->pin_free) cudaEventDestroy(ctx->pin_free);
+  if (ctx->tickets) cudaFree(ctx->tickets);
   if (ctx->pin) cudaFreeHost(ctx->pin);
   if (ctx->pin2) cudaFreeHost(ctx->pin2);
   free(ctx);

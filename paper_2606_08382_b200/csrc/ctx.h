@@ -47,8 +47,11 @@ struct starkv_ctx {
   struct KernelAttr { const void* fn; int smem; };
   mutable KernelAttr attrs[48];
   mutable int n_attrs;
+  int* tickets;          // SK_TICKETS zeroed ints in device memory (allocated at create): arrival counters of the sliced
+                         // combine, one per (sequence, head), reset by the last arriver
   char err[512];
 };
+#define SK_TICKETS 16384
 
 // decode kernel variants (starkv_set_decode_variant)
 enum { SK_VARIANT_AUTO = 0, SK_VARIANT_MMA = 1, SK_VARIANT_TC5 = 2, SK_VARIANT_TM = 3, SK_VARIANT_GENERIC = 4 };
@@ -138,6 +141,7 @@ struct SkWorkspace {   // carve-up of the caller's decode workspace
   size_t qimg_off;     // latent-space query images, per sequence
   size_t qimg_stride;
   size_t part_off;     // split-K partials
+  size_t slice_off;    // sliced combine: per-slice up-projection partials
   size_t host_off;     // staging for the _host variant (q, seq_lens, out)
   size_t total;
   int n_splits;

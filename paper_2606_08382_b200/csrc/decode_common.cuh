@@ -22,4 +22,5 @@ __host__ __device__ inline void sk_split_range(int n_pages, int n_splits, int gr
 }
 
 // D8 + D9: log-sum-exp merge of the split partials, normalise, up-project with B_v.
-int sk_launch_combine(starkv_ctx* ctx, const float* parts, int n_splits, int batch, const void* B_v, void* out);
+int sk_launch_combine(starkv_ctx* ctx, const float* parts, int n_splits, int batch, const void* B_v, void* out,
+                      float* pslice);

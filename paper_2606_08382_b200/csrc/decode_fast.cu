@@ -1412,6 +1412,8 @@ void sk_plan_workspace(const starkv_ctx* ctx, int batch, int max_pages, SkWorksp
   w->qimg_stride = (size_t)round_up(qb_img, 256);
   w->qimg_off = off; off += w->qimg_stride * batch;
   w->part_off = off; off += ((size_t)batch * ns * L.n_q_heads * sk_part_stride(L.rank_v) * 4 + 255) / 256 * 256;
+  w->slice_off = off;   // per-slice up-projection partials of the sliced combine: [batch][H_q][slices of 32 channels][d_h]
+  off += ((size_t)batch * L.n_q_heads * ((L.rank_v + 31) / 32) * L.head_dim * 4 + 255) / 256 * 256;
   w->host_off = off;
   const size_t qb = ((size_t)batch * L.n_q_heads * L.head_dim * 2 + 255) / 256 * 256;
   off += 2 * qb + ((size_t)batch * 4 + 255) / 256 * 256;
@@ -1459,7 +1461,7 @@ int sk_decode_fast(starkv_ctx* ctx, const void* q, const void* pool, const int32
     SK_CUDA_CHECK(ctx, cudaEventRecord(ctx->ev1, ctx->stream));
     ctx->timing_valid = 1;
   }
-  const int rc = sk_launch_combine(ctx, parts, w.n_splits, batch, B_v, out);
+  const int rc = sk_launch_combine(ctx, parts, w.n_splits, batch, B_v, out, reinterpret_cast<float*>((uint8_t*)ws + w.slice_off));
   ctx->last_launches = 3;
   return rc;
 }

@@ -335,17 +335,145 @@ __global__ void __launch_bounds__(1024) combine_fast_kernel(const __grid_constan
   }
 }
 
+// D8 + D9 spread over (head, channel slice, sequence) blocks, for few sequences and many splits (C3: one sequence, 148
+// splits -- one block per head reads 150 KB of partials on its own).  Block (head, slice of 32 channels): every global load
+// that depends on nothing -- the (m, l) pairs, this thread's accumulator rows, its B_v elements -- is issued up front, so
+// the block costs about one memory round trip: split weights, o[c] = sum_s w_s acc_s[c] (thread = (channel, split group)),
+// its part of the up-projection  po[d] = sum_c o[c] B_v[c, g d_h + d] / l*  to the workspace; the LAST slice block of a
+// head to arrive (atomic ticket in context-owned memory, reset by that block) adds the slices and writes the fp16 row.
+constexpr int CS_THREADS = 256, CS_CH = 32, CS_SG = CS_THREADS / CS_CH, CS_PF = 20;
+__global__ void __launch_bounds__(CS_THREADS) combine_sliced_kernel(const __grid_constant__ StarkvLayout L,
+                                                                    const float* __restrict__ parts, int n_splits,
+                                                                    const __half* __restrict__ B_v, __half* __restrict__ out,
+                                                                    float* __restrict__ pslice, int* __restrict__ tickets, int nsl) {
+  __shared__ float wsm[512];
+  __shared__ float osum[CS_SG][CS_CH];
+  __shared__ float po[2][256];
+  __shared__ float rsm[16];
+  __shared__ int last_s;
+  const int head = blockIdx.x, sl = blockIdx.y, b = blockIdx.z, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  sk_pdl_enter();
+  const int g = head / L.group;
+  const int rv = L.rank_v, dh = L.head_dim, dv = L.n_kv_heads * dh;
+  const size_t ps = sk_part_stride(rv);
+  const float* base = parts + ((size_t)b * n_splits * L.n_q_heads + head) * ps;
+  const size_t sstride = (size_t)L.n_q_heads * ps;
+  // ---- loads that depend on nothing
+  float2 ml0 = make_float2(-INFINITY, 0.f), ml1 = make_float2(-INFINITY, 0.f);
+  if (tid < n_splits) ml0 = *reinterpret_cast<const float2*>(base + (size_t)tid * sstride);
+  if (tid + CS_THREADS < n_splits) ml1 = *reinterpret_cast<const float2*>(base + (size_t)(tid + CS_THREADS) * sstride);
+  const int c = tid & (CS_CH - 1), sg = tid >> 5;   // channel of the slice, split group
+  const int ch = sl * CS_CH + c;
+  const float* col = base + SK_PART_ACC + ch;
+  float v[CS_PF];
+#pragma unroll
+  for (int k = 0; k < CS_PF; ++k) {
+    const int s = sg + CS_SG * k;
+    v[k] = (ch < rv && s < n_splits) ? col[(size_t)s * sstride] : 0.f;
+  }
+  // up-projection operand: thread (d, half) takes channels half * 16 .. + 16 of the slice (head dims above 128: two passes)
+  const int nc = min(CS_CH, rv - sl * CS_CH);
+  const int d = tid & 127, hf = tid >> 7;
+  const __half* bcol = B_v + (size_t)(sl * CS_CH + hf * 16) * dv + (size_t)g * dh + d;
+  __half bq[16];
+#pragma unroll
+  for (int k = 0; k < 16; ++k) bq[k] = (d < dh && hf * 16 + k < nc) ? bcol[(size_t)k * dv] : __float2half(0.f);
+  // ---- m*, the split weights, l*
+  float mx = fmaxf(ml0.x, ml1.x);
+#pragma unroll
+  for (int o = 16; o; o >>= 1) mx = fmaxf(mx, __shfl_xor_sync(0xffffffffu, mx, o));
+  if (lane == 0) rsm[warp] = mx;
+  __syncthreads();
+  float mstar = rsm[0];
+#pragma unroll
+  for (int i = 1; i < CS_THREADS / 32; ++i) mstar = fmaxf(mstar, rsm[i]);
+  const float w0 = ml0.x == -INFINITY ? 0.f : exp2f(ml0.x - mstar);
+  const float w1 = ml1.x == -INFINITY ? 0.f : exp2f(ml1.x - mstar);
+  wsm[tid] = w0;
+  wsm[tid + CS_THREADS] = w1;
+  float lp = w0 * ml0.y + w1 * ml1.y;
+#pragma unroll
+  for (int o = 16; o; o >>= 1) lp += __shfl_xor_sync(0xffffffffu, lp, o);
+  if (lane == 0) rsm[8 + warp] = lp;
+  __syncthreads();
+  float lstar = 0.f;
+#pragma unroll
+  for (int i = 0; i < CS_THREADS / 32; ++i) lstar += rsm[8 + i];
+  const float inv = (mstar == -INFINITY || lstar == 0.f) ? 0.f : 1.f / lstar;
+  // ---- o[c] over this thread's splits (wsm is 0 past n_splits: neutral)
+  float a0 = 0.f, a1 = 0.f;
+#pragma unroll
+  for (int k = 0; k < CS_PF; k += 2) {
+    a0 = fmaf(wsm[sg + CS_SG * k], v[k], a0);
+    a1 = fmaf(wsm[sg + CS_SG * (k + 1)], v[k + 1], a1);
+  }
+  if (ch < rv)
+    for (int s = sg + CS_SG * CS_PF; s < n_splits; s += CS_SG) a0 = fmaf(wsm[s], col[(size_t)s * sstride], a0);
+  osum[sg][c] = a0 + a1;
+  __syncthreads();
+  if (tid < CS_CH) {
+    float o = 0.f;
+#pragma unroll
+    for (int k = 0; k < CS_SG; ++k) o += osum[k][tid];
+    osum[0][tid] = o * inv;
+  }
+  __syncthreads();
+  // ---- this slice's part of the up-projection
+  {
+    float acc = 0.f;
+#pragma unroll
+    for (int k = 0; k < 16; ++k) acc = fmaf(osum[0][hf * 16 + k], __half2float(bq[k]), acc);
+    po[hf][d] = acc;
+  }
+  for (int d2 = 128 + d; d2 < dh; d2 += 128) {   // head dims above 128
+    float acc = 0.f;
+    for (int k = 0; k < 16 && hf * 16 + k < nc; ++k) acc = fmaf(osum[0][hf * 16 + k], __half2float(bcol[(size_t)k * dv + (d2 - d)]), acc);
+    po[hf][d2] = acc;
+  }
+  __syncthreads();
+  float* mine = pslice + (((size_t)b * L.n_q_heads + head) * nsl + sl) * dh;
+  if (tid < dh) mine[tid] = po[0][tid] + po[1][tid];
+  __threadfence();
+  __syncthreads();
+  if (tid == 0) {
+    int* tk = tickets + (size_t)b * L.n_q_heads + head;
+    const int t = atomicAdd(tk, 1);
+    const int last = t == nsl - 1;
+    if (last) *tk = 0;   // ready for the next call (calls of a context are ordered on its stream)
+    last_s = last;
+  }
+  __syncthreads();
+  if (last_s) {
+    __threadfence();
+    if (tid < dh) {
+      const float* ph = pslice + ((size_t)b * L.n_q_heads + head) * nsl * dh + tid;
+      float sacc = 0.f;
+      for (int k = 0; k < nsl; ++k) sacc += __ldcg(ph + (size_t)k * dh);
+      out[((size_t)b * L.n_q_heads + head) * dh + tid] = __float2half_rn(sacc);
+    }
+  }
+}
+
 }  // namespace
 
-int sk_launch_combine(starkv_ctx* ctx, const float* parts, int n_splits, int batch, const void* B_v, void* out) {
-  if (n_splits <= 512 && ctx->L.rank_v <= 512) {
+int sk_launch_combine(starkv_ctx* ctx, const float* parts, int n_splits, int batch, const void* B_v, void* out,
+                      float* pslice) {
+  const StarkvLayout& L = ctx->L;
+  const int nsl = (L.rank_v + CS_CH - 1) / CS_CH;
+  // sliced combine where one block per head would be the long pole: few sequences, many splits
+  // (measured: C3, 148 splits x 1 sequence: step 57.6 -> 53.2 us; C2, 37 splits x 4 sequences: 50.0 -> 54.1 us)
+  if (ctx->tickets && pslice && n_splits >= 64 && n_splits <= 512 && L.head_dim <= CS_THREADS && nsl > 1 &&
+      (size_t)batch * L.n_q_heads <= (size_t)SK_TICKETS && batch * L.n_q_heads < 2 * ctx->n_sm) {
+    SK_PREFER_SMEM(ctx, combine_sliced_kernel);
+    SK_CUDA_CHECK(ctx, sk_launch(ctx, combine_sliced_kernel, dim3(L.n_q_heads, nsl, batch), dim3(CS_THREADS), 0, L, parts, n_splits,
+                                 (const __half*)B_v, (__half*)out, pslice, ctx->tickets, nsl));
+  } else if (n_splits <= 512 && L.rank_v <= 512) {
     SK_PREFER_SMEM(ctx, combine_fast_kernel);
-    SK_CUDA_CHECK(ctx, sk_launch(ctx, combine_fast_kernel, dim3(ctx->L.n_q_heads, batch), dim3(1024), 0, ctx->L, parts, n_splits,
+    SK_CUDA_CHECK(ctx, sk_launch(ctx, combine_fast_kernel, dim3(L.n_q_heads, batch), dim3(1024), 0, L, parts, n_splits,
                                  (const __half*)B_v, (__half*)out));
   } else {
     SK_PREFER_SMEM(ctx, combine_kernel);
-    combine_kernel<<<dim3(ctx->L.n_q_heads, batch), 256, 0, ctx->stream>>>(ctx->L, parts, n_splits, (const __half*)B_v,
-                                                                           (__half*)out);
+    combine_kernel<<<dim3(L.n_q_heads, batch), 256, 0, ctx->stream>>>(L, parts, n_splits, (const __half*)B_v, (__half*)out);
   }
   SK_CUDA_CHECK(ctx, cudaGetLastError());
   return STARKV_OK;
@@ -369,7 +497,7 @@ int sk_decode_generic(starkv_ctx* ctx, const void* q, const void* pool, const in
     SK_CUDA_CHECK(ctx, cudaEventRecord(ctx->ev1, ctx->stream));
     ctx->timing_valid = 1;
   }
-  const int rc = sk_launch_combine(ctx, parts, w.n_splits, batch, B_v, out);
+  const int rc = sk_launch_combine(ctx, parts, w.n_splits, batch, B_v, out, reinterpret_cast<float*>((uint8_t*)ws + w.slice_off));
   ctx->last_launches = 2;
   return rc;
 }

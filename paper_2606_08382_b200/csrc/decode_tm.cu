@@ -898,7 +898,7 @@ int sk_decode_tm(starkv_ctx* ctx, const void* q, const void* pool, const int32_t
     SK_CUDA_CHECK(ctx, cudaEventRecord(ctx->ev1, ctx->stream));
     ctx->timing_valid = 1;
   }
-  const int rc = sk_launch_combine(ctx, parts, w.n_splits, batch, B_v, out);
+  const int rc = sk_launch_combine(ctx, parts, w.n_splits, batch, B_v, out, reinterpret_cast<float*>((uint8_t*)ws + w.slice_off));
   ctx->last_launches = 3;
   return rc;
 }

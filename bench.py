@@ -41,6 +41,7 @@ UNIT = "GB/s"
 L2_BYTES = 126 * 1024 * 1024
 NOMINAL_HBM_GBS = 8000.0          # north_star's denominator (context; the roofline uses the measured one)
 FALLBACK_HBM_GBS = 6650.0         # B200_PROFILING.md fallback when MEASURED_PEAKS.json is absent
+HEADLINE = "C3"                   # north_star target configs are C2, C3, C5; C3 (128K, int8/int4, batch 1) is the hardest
 
 
 def step_bytes(cfg) -> int:
@@ -391,23 +392,16 @@ def workload_name(cfg) -> str:
 # ------------------------------------------------------------------------------------------------
 # our arm
 # ------------------------------------------------------------------------------------------------
-def run_ours(args, cfg):
+def run_ours(args, cfg, env, K, with_cpu):
+    """One single-layer workload (C2, C3 or C4) on every rank; returns the JSON line as a dict (rank 0) or None."""
     import torch
     import torch.distributed as dist
 
     import paper_2606_08382_b200 as sk      # raises if libstarkv.so is missing: there is no fallback
     from paper_2606_08382_b200.sharding import max_over_ranks
 
-    world = int(os.environ.get("WORLD_SIZE", "1"))
-    rank = int(os.environ.get("RANK", "0"))
-    local = int(os.environ.get("LOCAL_RANK", "0"))
-    if not torch.cuda.is_available():
-        raise SystemExit("bench.py: no CUDA device; the product path has no CPU fallback")
-    torch.cuda.set_device(local)
-    device = torch.device("cuda", local)
-    if world > 1:
-        dist.init_process_group("nccl", device_id=device)
-    K, W = args.steps, max(args.warmup, 3)
+    world, rank, local, device = env
+    W = max(args.warmup, 3)
 
     # weak scaling: every rank owns one full BASELINE batch (sequences are independent: no collective)
     wl = Workload(cfg, sk, torch, device, n_rep=args.replicas or None, verbose=(rank == 0 and args.verbose))
@@ -500,10 +494,11 @@ def run_ours(args, cfg):
     clocks = sampler.finish()
     torch.cuda.synchronize()
 
+    h2d_b, d2h_b, kname = wl.h2d_bytes(), wl.d2h_bytes(), sk.starkv_decode_kernel_name(wl.ctx)
+    del graphs, wl
+    torch.cuda.empty_cache()
     if rank != 0:
-        if world > 1:
-            dist.destroy_process_group()
-        return
+        return None
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
         "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
@@ -516,11 +511,11 @@ def run_ours(args, cfg):
         "us_per_step_per_layer": ms_step * 1e3,
         "tokens_per_s_attn_only_32_layers": world * cfg.batch / (32 * ms_step * 1e-3),
         "frac_of_nominal_8TBs": value / world / NOMINAL_HBM_GBS,
-        "e2e": {"value": e2e, "unit": UNIT, "h2d_bytes_per_step": wl.h2d_bytes(), "d2h_bytes_per_step": wl.d2h_bytes(),
+        "e2e": {"value": e2e, "unit": UNIT, "h2d_bytes_per_step": h2d_b, "d2h_bytes_per_step": d2h_b,
                 "ms_per_step": ms_e2e, "steps": Ke},
         "gpu_launches": K * launches_per_step,
         "clocks": clocks,
-        "roofline": {"bound": "hbm", "kernel": sk.starkv_decode_kernel_name(wl.ctx) + " (rows D2-D7)", "achieved": achieved,
+        "roofline": {"bound": "hbm", "kernel": kname + " (rows D2-D7)", "achieved": achieved,
                      "peak": peak,
                      "unit": "GB/s", "frac": achieved / peak, "traffic": stored_traffic(cfg.name),
                      "peak_source": peak_src, "kernel_us": k_ms * 1e3, "kernel_us_min": float(np.min(kms)) * 1e3,
@@ -529,11 +524,9 @@ def run_ours(args, cfg):
     }
     if prefill is not None:
         line["append_prefill"] = prefill
-    if world == 1 and not args.no_cpu:
+    if world == 1 and with_cpu:
         line["cpu_baseline"] = cpu_baseline(cfg)
-    print(json.dumps(line))
-    if world > 1:
-        dist.destroy_process_group()
+    return line
 
 
 # ------------------------------------------------------------------------------------------------
@@ -545,7 +538,7 @@ N_LAYERS_C5 = 32
 NON_ATTN_WEIGHT_BYTES = 2 * (32 * (2 * 4096 * 4096 + 2 * 4096 * 1024 + 3 * 4096 * 14336) + 128256 * 4096)
 
 
-def run_c5(args):
+def run_c5(args, env, K):
     """One step = starkv_append + starkv_decode_attn for each of the 32 layers (each layer its own rank table,
     context and cache), captured as one CUDA graph.  The 32 caches (2.9 GB) are the L2 defeat."""
     import torch
@@ -554,16 +547,8 @@ def run_c5(args):
     import paper_2606_08382_b200 as sk
     from paper_2606_08382_b200.sharding import max_over_ranks
 
-    world = int(os.environ.get("WORLD_SIZE", "1"))
-    rank = int(os.environ.get("RANK", "0"))
-    local = int(os.environ.get("LOCAL_RANK", "0"))
-    if not torch.cuda.is_available():
-        raise SystemExit("bench.py: no CUDA device; the product path has no CPU fallback")
-    torch.cuda.set_device(local)
-    device = torch.device("cuda", local)
-    if world > 1:
-        dist.init_process_group("nccl", device_id=device)
-    K, W = args.steps, max(args.warmup, 3)
+    world, rank, local, device = env
+    W = max(args.warmup, 3)
     n_layers = args.layers or N_LAYERS_C5
     stream = torch.cuda.Stream(device=device)
     layers = []
@@ -647,11 +632,12 @@ def run_c5(args):
     achieved = bytes_kern / (k_ms * 1e-3) / 1e9
     clocks = sampler.finish()
     torch.cuda.synchronize()
+    h2d_b, d2h_b = sum(w.h2d_bytes() for w in layers), sum(w.d2h_bytes() for w in layers)
+    kname, c0 = sk.starkv_decode_kernel_name(layers[0].ctx), layers[0].cfg
+    del g, layers
+    torch.cuda.empty_cache()
     if rank != 0:
-        if world > 1:
-            dist.destroy_process_group()
-        return
-    c0 = layers[0].cfg
+        return None
     non_attn_ms = NON_ATTN_WEIGHT_BYTES / (peak * 1e9) * 1e3
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
@@ -672,20 +658,43 @@ def run_c5(args):
                                   "model": "LLaMA-3.1-8B-shaped fp16 weights (%.1f GB) read once per step at the measured HBM "
                                            "bandwidth; the library holds no such code" % (NON_ATTN_WEIGHT_BYTES / 1e9)},
         "frac_of_nominal_8TBs": value / world / NOMINAL_HBM_GBS,
-        "e2e": {"value": e2e, "unit": UNIT, "h2d_bytes_per_step": sum(w.h2d_bytes() for w in layers),
-                "d2h_bytes_per_step": sum(w.d2h_bytes() for w in layers), "ms_per_step": ms_e2e, "steps": Ke},
+        "e2e": {"value": e2e, "unit": UNIT, "h2d_bytes_per_step": h2d_b, "d2h_bytes_per_step": d2h_b, "ms_per_step": ms_e2e,
+                "steps": Ke},
         "gpu_launches": K * launches,
         "clocks": clocks,
-        "roofline": {"bound": "hbm", "kernel": sk.starkv_decode_kernel_name(layers[0].ctx) +
-                     " (rows D2-D7), summed over the layers of a step",
+        "roofline": {"bound": "hbm", "kernel": kname + " (rows D2-D7), summed over the layers of a step",
                      "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
                      "traffic": stored_traffic("C5"), "peak_source": peak_src, "kernel_us": k_ms * 1e3,
                      "launches_timed": len(kms) * n_layers, "algorithmic_bytes_per_launch": bytes_kern / n_layers,
                      "frac_of_nominal_8TBs": achieved / NOMINAL_HBM_GBS},
     }
-    print(json.dumps(line))
-    if world > 1:
-        dist.destroy_process_group()
+    return line
+
+
+def summary(d):
+    """What the per_config block keeps of a workload's line."""
+    r = d["roofline"]
+    out = {"workload": d["config"]["workload"], "steps": d["steps"], "step_us": d["ms_per_step"] * 1e3,
+           "us_per_step_per_layer": d["us_per_step_per_layer"], "value": d["value"], "unit": d["unit"],
+           "frac_of_nominal_8TBs": d["frac_of_nominal_8TBs"],
+           "roofline": {k: r[k] for k in ("kernel", "kernel_us", "achieved", "peak", "frac", "traffic", "frac_of_nominal_8TBs")},
+           "e2e": {"value": d["e2e"]["value"], "ms_per_step": d["e2e"]["ms_per_step"]},
+           "gpu_launches_per_step": d["gpu_launches"] // max(1, d["steps"])}
+    for k in ("append_prefill", "attention_share_model", "tokens_per_s_attn_only", "tokens_per_s_attn_only_32_layers"):
+        if k in d:
+            out[k] = d[k]
+    return out
+
+
+def spawn_ranks(n):
+    """`bench.py --gpus N` outside torchrun: start the N ranks ourselves (one process per GPU, NCCL rendezvous on
+    127.0.0.1) with the same arguments."""
+    import socket
+    with socket.socket() as so:
+        so.bind(("127.0.0.1", 0))
+        port = so.getsockname()[1]
+    os.execvp(sys.executable, [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={n}",
+                               "--master-addr", "127.0.0.1", "--master-port", str(port), os.path.abspath(__file__)] + sys.argv[1:])
 
 
 def main():
@@ -694,7 +703,8 @@ def main():
     ap.add_argument("--steps", type=int, default=2000)
     ap.add_argument("--warmup", type=int, default=20)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--workload", default="C2", help="C2 (default: the config the metric is quoted on), C3, C4, C5")
+    ap.add_argument("--workload", default="all",
+                    help="all (default: headline C3 + per_config block with C2, C4, C5), or one of C2, C3, C4, C5")
     ap.add_argument("--replicas", type=int, default=0)
     ap.add_argument("--layers", type=int, default=0, help="C5 only: number of layers (default 32)")
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
@@ -702,13 +712,46 @@ def main():
     ap.add_argument("--prefill-tokens", type=int, default=2048)
     ap.add_argument("--verbose", action="store_true")
     args = ap.parse_args()
-    cfg = synth.make_config(args.workload)
     if args.impl == "reference":
-        run_reference(args, cfg)
-    elif cfg.name == "C5":
-        run_c5(args)
+        run_reference(args, synth.make_config(HEADLINE if args.workload == "all" else args.workload))
+        return
+    if args.gpus > 1 and "WORLD_SIZE" not in os.environ:
+        spawn_ranks(args.gpus)
+    import torch
+    import torch.distributed as dist
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the product path has no CPU fallback")
+    torch.cuda.set_device(local)
+    device = torch.device("cuda", local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=device)
+    env = (world, rank, local, device)
+
+    def measure(name, K, with_cpu):
+        if name == "C5":
+            return run_c5(args, env, K)
+        return run_ours(args, synth.make_config(name), env, K, with_cpu)
+
+    if args.workload != "all":
+        line = measure(args.workload, args.steps, not args.no_cpu)
     else:
-        run_ours(args, cfg)
+        # headline = the hardest target configuration (C3: 128K context, int8/int4): exactly --steps timed steps.  The other
+        # BASELINE.json configurations are measured the same way with a bounded number of steps and reported in per_config.
+        line = measure(HEADLINE, args.steps, not args.no_cpu)
+        per = {HEADLINE: summary(line)} if line is not None else {}
+        for name in ("C2", "C4", "C5"):
+            d = measure(name, min(args.steps, 200 if name == "C5" else 500), False)
+            if d is not None:
+                per[name] = summary(d)
+        if line is not None:
+            line["per_config"] = per
+    if rank == 0 and line is not None:
+        print(json.dumps(line))
+    if world > 1:
+        dist.destroy_process_group()
 
 
 if __name__ == "__main__":

@@ -273,7 +273,7 @@ __global__ void __launch_bounds__(TM_THREADS, 1) decode_tm_kernel(
     fence_barrier_init();
   }
   if (warp == 23) tmem_alloc(smem_u32((const void*)tmem_slot), TM_COLS);
-  if (tid < 36) misc[tid] = tid < 34 ? 0.f : 1.f;   // m = 0, M = 0 (forces the first update), 1/M = 1
+  if (tid < 36) misc[tid] = tid < 32 ? -P_OFFSET : (tid < 34 ? 0.f : 1.f);   // reference m - 8 with m = 0, M = 0 (forces the first update), 1/M = 1
 
   sk_pdl_wait();   // seq_lens, block table, query image, pages: nothing global is read before this point
   const int len = seq_lens[b];
@@ -373,7 +373,7 @@ __global__ void __launch_bounds__(TM_THREADS, 1) decode_tm_kernel(
       const int wq = warp & 3, wr = warp - 8, tq = wq * 32 + lane, pgsel = tq >> 6, slot = tq & 63;
       const int hbase = hh * NHH;     // first query head of this warpgroup
       const uint32_t tlane = tbase + ((uint32_t)(wq * 32) << 16);
-      float* mref_s = misc + MISC_MREF;
+      float* mref_s = misc + MISC_MREF;   // running reference of every head, stored as m - 8: 2^(s - (m - 8)) = p'
       float* M_s = misc + MISC_M;
       float* invM_s = misc + MISC_INVM;
       int* red = reinterpret_cast<int*>(misc + MISC_RED);                                // [8 warps][RED_STRIDE], ordered ints
@@ -399,16 +399,18 @@ __global__ void __launch_bounds__(TM_THREADS, 1) decode_tm_kernel(
       const float* ce_s = reinterpret_cast<const float*>(smem + T.off_img + T.img_scal_off);   // 2^(24 - e) per (head, block)
       bar_sync(BAR_SM, NBAR);
 
+      uint32_t d[2 * NHH];
       for (int it = 0; it < n_it; ++it) {
         const int j = 2 * it + pgsel;
         const bool exists = j < n_pg;
         const int st = j % nstage;
         const int buf = it & 1;
         const int sb = it % ds_nbuf;
-        mbar_wait(qk_done0 + 8 * sb, (uint32_t)((it / ds_nbuf) & 1));
-        tc_fence_after();
-        uint32_t d[2 * NHH];
-        tmem_ld<2 * NHH>(tlane + (uint32_t)(T.col_ds + sb * T.ds_cols + 2 * hbase), d);
+        if (!(ds_nbuf == 2 && it > 0)) {   // (double-buffered score tiles: loaded ahead, at the end of the previous tile's arithmetic)
+          mbar_wait(qk_done0 + 8 * sb, (uint32_t)((it / ds_nbuf) & 1));
+          tc_fence_after();
+          tmem_ld<2 * NHH>(tlane + (uint32_t)(T.col_ds + sb * T.ds_cols + 2 * hbase), d);
+        }
         if (exists) mbar_wait(full0 + 8 * st, (uint32_t)((j / nstage) & 1));
         const uint8_t* page = stage_base + (size_t)st * page_bytes;
         const uint16_t* ksc = reinterpret_cast<const uint16_t*>(page + L.k_scale_off) + slot;
@@ -448,7 +450,15 @@ __global__ void __launch_bounds__(TM_THREADS, 1) decode_tm_kernel(
             if (hbase + i < Hq) mxa = fmaxf(mxa, arg[i]);
           }
         }
-        bool trig = valid && (mxa > TAU || sv0 > M0 || sv1 > M1);
+        if (ds_nbuf == 2 && it + 1 < n_it) {
+          // the next tile's scores: its MMAs ran while this tile was being read, so the TMEM load's latency hides behind the
+          // rest of this tile's work
+          const int sn = (it + 1) & 1;
+          mbar_wait(qk_done0 + 8 * sn, (uint32_t)(((it + 1) >> 1) & 1));
+          tc_fence_after();
+          tmem_ld<2 * NHH>(tlane + (uint32_t)(T.col_ds + sn * T.ds_cols + 2 * hbase), d);
+        }
+        bool trig = valid && (mxa > TAU + P_OFFSET || sv0 > M0 || sv1 > M1);
         if (it == 0) trig = true;
         const bool wany = __any_sync(0xffffffffu, trig);
         if (lane == 0) {
@@ -477,9 +487,9 @@ __global__ void __launch_bounds__(TM_THREADS, 1) decode_tm_kernel(
 #pragma unroll
           for (int i = 0; i < NHH; ++i) {
             const float mt = f_unordered(max(max(redh[i], redh[RED_STRIDE + i]), max(redh[2 * RED_STRIDE + i], redh[3 * RED_STRIDE + i])));
-            const float m_old = mref_s[hbase + i];
+            const float m_old = mref_s[hbase + i];    // (references are stored as m - 8)
             // only a maximum that the tile exceeds moves (to the true maximum so far); the first tile sets it
-            float m_new = (it == 0) ? mt : (mt > m_old ? mt : m_old);
+            float m_new = (it == 0) ? mt - P_OFFSET : fmaxf(mt - P_OFFSET, m_old);
             if (!(m_new > -INFINITY)) m_new = m_old;
             const float delta = m_old - m_new;       // <= 0 after the first tile
             fs[i] = ex2(delta);
@@ -528,6 +538,7 @@ __global__ void __launch_bounds__(TM_THREADS, 1) decode_tm_kernel(
         }
         // ---- p' and the two scaled operands
         const float a0 = sv0 * invM_s[0], a1 = sv1 * invM_s[1];
+        const uint32_t a0h = pack_h2(a0, a0), a1h = pack_h2(a1, a1);
         if (it >= 2) mbar_wait(pv_done0 + 8 * buf, (uint32_t)(((it >> 1) - 1) & 1));   // the MMAs of tile it - 2 have read the buffer
         uint8_t* pb = smem + T.off_p + buf * 2 * P_BLK_BYTES;
 #pragma unroll
@@ -535,14 +546,15 @@ __global__ void __launch_bounds__(TM_THREADS, 1) decode_tm_kernel(
           float p[8];
 #pragma unroll
           for (int k = 0; k < 8; ++k) {
-            p[k] = ex2(arg[8 * oc + k] + P_OFFSET);   // -inf -> 0 for slots past the sequence end
+            p[k] = ex2(arg[8 * oc + k]);   // -inf -> 0 for slots past the sequence end
             l_acc[8 * oc + k] += p[k];
           }
+          // p' -> fp16 pairs once, then the two value-scale factors as packed fp16 multiplies (two roundings of 2^-11 on
+          // a term of the value product; no flush to zero)
+          const uint32_t q0 = pack_h2(p[0], p[1]), q1 = pack_h2(p[2], p[3]), q2 = pack_h2(p[4], p[5]), q3 = pack_h2(p[6], p[7]);
           uint4 x0, x1;
-          x0.x = pack_h2(p[0] * a0, p[1] * a0); x0.y = pack_h2(p[2] * a0, p[3] * a0);
-          x0.z = pack_h2(p[4] * a0, p[5] * a0); x0.w = pack_h2(p[6] * a0, p[7] * a0);
-          x1.x = pack_h2(p[0] * a1, p[1] * a1); x1.y = pack_h2(p[2] * a1, p[3] * a1);
-          x1.z = pack_h2(p[4] * a1, p[5] * a1); x1.w = pack_h2(p[6] * a1, p[7] * a1);
+          x0.x = h2mul(q0, a0h); x0.y = h2mul(q1, a0h); x0.z = h2mul(q2, a0h); x0.w = h2mul(q3, a0h);
+          x1.x = h2mul(q0, a1h); x1.y = h2mul(q1, a1h); x1.z = h2mul(q2, a1h); x1.w = h2mul(q3, a1h);
           *reinterpret_cast<uint4*>(pb + paddr[0] + oc * 2048) = x0;
           *reinterpret_cast<uint4*>(pb + paddr[1] + oc * 2048) = x1;
         }
@@ -581,7 +593,7 @@ __global__ void __launch_bounds__(TM_THREADS, 1) decode_tm_kernel(
         if (tq < NHH && hbase + tq < Hq) {
           const float* rh = redf + 4 * hh * RED_STRIDE;
           const float lsum = rh[tq] + rh[RED_STRIDE + tq] + rh[2 * RED_STRIDE + tq] + rh[3 * RED_STRIDE + tq];
-          *reinterpret_cast<float4*>(my_parts + (size_t)(hbase + tq) * pstride) = make_float4(mref_s[hbase + tq], lsum, 0.f, 0.f);
+          *reinterpret_cast<float4*>(my_parts + (size_t)(hbase + tq) * pstride) = make_float4(mref_s[hbase + tq] + P_OFFSET, lsum, 0.f, 0.f);
         }
       }
     }

@@ -90,6 +90,8 @@ struct TmPlan {
   int32_t col_do, col_av, col_ak, col_ds;
   int32_t ds_nbuf;                  // score tiles in tensor memory: 2 (double-buffered) where they fit, else 1
   // shared memory (bytes from the 1024-aligned base)
-  int32_t nstage;                   // page ring depth
-  int32_t off_stage, off_img, off_p, off_misc, off_bar, off_tbl, smem_bytes;
+  int32_t k_bytes, ks_bytes, v_bytes, vs_bytes;   // the four parts of a page: key blocks, key scales, value blocks, value scales
+  int32_t kstride, vstride, sstride;              // stage strides of the three rings (scales: key scales then value scales)
+  int32_t n_kstage, n_vstage, n_sstage;           // ring depths
+  int32_t off_kstage, off_vstage, off_sstage, off_img, off_p, off_misc, off_bar, off_tbl, smem_bytes;
 };

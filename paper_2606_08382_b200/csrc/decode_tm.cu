@@ -231,30 +231,38 @@ __global__ void __launch_bounds__(TM_THREADS, 1) decode_tm_kernel(
   const int split = blockIdx.x, b = blockIdx.y;
   sk_pdl_trigger();
 
-  // barrier area: full[nstage], empty[nstage], then the single barriers
-  const int nstage = T.nstage;
-  const uint32_t full0 = smem_u32(smem + T.off_bar);
-  const uint32_t empty0 = full0 + 8 * nstage;
-  const uint32_t imgbar = empty0 + 8 * nstage;
+  // Three page rings, each with full[] / empty[] mbarriers: a page is fetched as its key blocks, its value blocks and its
+  // scales (key scales + value scales), because the three are consumed at different depths of the pipeline -- the key
+  // rows a few tiles ahead of the value rows and of the softmax, which reads the scales.  One ring of whole pages
+  // would have to hold every page for the whole pipeline depth.
+  const int nK = T.n_kstage, nV = T.n_vstage, nS = T.n_sstage;
+  const uint32_t fullK0 = smem_u32(smem + T.off_bar);
+  const uint32_t emptyK0 = fullK0 + 8 * nK;
+  const uint32_t fullV0 = emptyK0 + 8 * nK;
+  const uint32_t emptyV0 = fullV0 + 8 * nV;
+  const uint32_t fullS0 = emptyV0 + 8 * nV;
+  const uint32_t emptyS0 = fullS0 + 8 * nS;
+  const uint32_t imgbar = emptyS0 + 8 * nS;
   const uint32_t ak_full0 = imgbar + 8 /* [2]: per half of the k-steps */, qk_done0 = imgbar + 24 /* [2]: per score buffer */,
                  ds_free0 = imgbar + 40 /* [2]: per score buffer */, p_full0 = imgbar + 56 /* [2] */,
                  av_full0 = imgbar + 72 /* [2]: per page */, pv_done0 = imgbar + 88 /* [2]: per P~ buffer */,
                  pv_half = imgbar + 104 /* the value MMAs over the first page's tokens are complete */,
                  qk_half = imgbar + 112 /* the score MMAs over the first half of the k-steps are complete */;
-  volatile uint32_t* tmem_slot = reinterpret_cast<volatile uint32_t*>(smem + T.off_bar + 8 * (2 * nstage) + 128);
+  volatile uint32_t* tmem_slot = reinterpret_cast<volatile uint32_t*>(smem + T.off_bar + 16 * (nK + nV + nS) + 128);
   // the score tile is double-buffered when tensor memory has room (T.ds_nbuf = 2): tile `it` uses buffer it % ds_nbuf, so the
   // score MMAs of the next tile run while the softmax warps still read this one
   const int ds_nbuf = T.ds_nbuf;
   int32_t* tbl_s = reinterpret_cast<int32_t*>(smem + T.off_tbl);
   float* misc = reinterpret_cast<float*>(smem + T.off_misc);
-  uint8_t* stage_base = smem + T.off_stage;
+  uint8_t* kstage_base = smem + T.off_kstage;
+  uint8_t* vstage_base = smem + T.off_vstage;
+  uint8_t* sstage_base = smem + T.off_sstage;
   const uint32_t page_bytes = (uint32_t)L.page_bytes;
 
   if (tid == 0) {
-    for (int s = 0; s < nstage; ++s) {
-      mbar_init(full0 + 8 * s, 1);
-      mbar_init(empty0 + 8 * s, 4 + 2 * NSPLIT + 4);   // key warps, softmax warps and value warps that read a page
-    }
+    for (int s = 0; s < nK; ++s) { mbar_init(fullK0 + 8 * s, 1); mbar_init(emptyK0 + 8 * s, 4); }            // 2 + 2 key warps read a page
+    for (int s = 0; s < nV; ++s) { mbar_init(fullV0 + 8 * s, 1); mbar_init(emptyV0 + 8 * s, 4); }            // 4 value warps
+    for (int s = 0; s < nS; ++s) { mbar_init(fullS0 + 8 * s, 1); mbar_init(emptyS0 + 8 * s, 2 * NSPLIT); }   // softmax warps of the page
     mbar_init(imgbar, 1);
     mbar_init(ak_full0, 4);
     mbar_init(ak_full0 + 8, 4);
@@ -311,10 +319,10 @@ __global__ void __launch_bounds__(TM_THREADS, 1) decode_tm_kernel(
     for (int it = 0; it < n_it; ++it) {
       const int j = 2 * it + pgsel;
       const bool exists = j < n_pg;
-      const int st = j % nstage;
+      const int st = j % nK;
       uint4 dq = desc4[k_begin];
-      if (exists) mbar_wait(full0 + 8 * st, (uint32_t)((j / nstage) & 1));
-      const uint8_t* row = stage_base + (size_t)st * page_bytes;
+      if (exists) mbar_wait(fullK0 + 8 * st, (uint32_t)((j / nK) & 1));
+      const uint8_t* row = kstage_base + (size_t)st * T.kstride;
       if (it > 0) {   // the previous tile's score MMAs over this half have read the operand
         const int pb = (it - 1) % ds_nbuf;
         if (half) mbar_wait(qk_done0 + 8 * pb, (uint32_t)(((it - 1) / ds_nbuf) & 1));
@@ -362,7 +370,7 @@ __global__ void __launch_bounds__(TM_THREADS, 1) decode_tm_kernel(
       __syncwarp();
       if (lane == 0) {
         mbar_arrive(ak_full0 + 8 * half);
-        if (exists) mbar_arrive(empty0 + 8 * st);
+        if (exists) mbar_arrive(emptyK0 + 8 * st);
       }
     }
   } else if (warp < 16) {
@@ -403,7 +411,7 @@ __global__ void __launch_bounds__(TM_THREADS, 1) decode_tm_kernel(
       for (int it = 0; it < n_it; ++it) {
         const int j = 2 * it + pgsel;
         const bool exists = j < n_pg;
-        const int st = j % nstage;
+        const int st = j % nS;
         const int buf = it & 1;
         const int sb = it % ds_nbuf;
         if (!(ds_nbuf == 2 && it > 0)) {   // (double-buffered score tiles: loaded ahead, at the end of the previous tile's arithmetic)
@@ -411,10 +419,10 @@ __global__ void __launch_bounds__(TM_THREADS, 1) decode_tm_kernel(
           tc_fence_after();
           tmem_ld<2 * NHH>(tlane + (uint32_t)(T.col_ds + sb * T.ds_cols + 2 * hbase), d);
         }
-        if (exists) mbar_wait(full0 + 8 * st, (uint32_t)((j / nstage) & 1));
-        const uint8_t* page = stage_base + (size_t)st * page_bytes;
-        const uint16_t* ksc = reinterpret_cast<const uint16_t*>(page + L.k_scale_off) + slot;
-        const uint16_t* vsc = reinterpret_cast<const uint16_t*>(page + L.v_scale_off) + slot;
+        if (exists) mbar_wait(fullS0 + 8 * st, (uint32_t)((j / nS) & 1));
+        const uint8_t* sslot = sstage_base + (size_t)st * T.sstride;   // [key scales][value scales] of the page
+        const uint16_t* ksc = reinterpret_cast<const uint16_t*>(sslot) + slot;
+        const uint16_t* vsc = reinterpret_cast<const uint16_t*>(sslot + T.ks_bytes) + slot;
         const bool valid = exists && ((p0 + j) * PTOK + slot) < len;
         float sc[2 * (NHH / G)];
 #pragma unroll
@@ -463,7 +471,7 @@ __global__ void __launch_bounds__(TM_THREADS, 1) decode_tm_kernel(
         const bool wany = __any_sync(0xffffffffu, trig);
         if (lane == 0) {
           flag[buf * 8 + wr] = wany ? 1 : 0;
-          if (exists) mbar_arrive(empty0 + 8 * st);   // every scale of the page has been used: the stage may be refilled
+          if (exists) mbar_arrive(emptyS0 + 8 * st);   // every scale of the page has been used: the slot may be refilled
         }
         bar_sync(BAR_SM, NBAR);
         const volatile uint32_t* flw = reinterpret_cast<const volatile uint32_t*>(flag + buf * 8);
@@ -619,14 +627,14 @@ __global__ void __launch_bounds__(TM_THREADS, 1) decode_tm_kernel(
       for (int pg = 0; pg < 2; ++pg) {
         const int j = 2 * it + pg;
         const bool exists = j < n_pg;
-        const int st = j % nstage;
-        if (exists) mbar_wait(full0 + 8 * st, (uint32_t)((j / nstage) & 1));
+        const int st = j % nV;
+        if (exists) mbar_wait(fullV0 + 8 * st, (uint32_t)((j / nV) & 1));
         if (it > 0) {   // the previous tile's value MMAs over this half of the tokens have read the operand
           if (pg == 0) mbar_wait(pv_half, (uint32_t)((it - 1) & 1));
           else mbar_wait(pv_done0 + 8 * ((it - 1) & 1), (uint32_t)(((it - 1) >> 1) & 1));
           tc_fence_after();
         }
-        const uint8_t* pagep = stage_base + (size_t)st * page_bytes;
+        const uint8_t* pagep = vstage_base + (size_t)st * T.vstride - L.v_hi_off;   // (row offsets are page-relative)
 #pragma unroll
         for (int m = 0; m < 2; ++m) {
           if (m < T.n_vt) {
@@ -658,25 +666,49 @@ __global__ void __launch_bounds__(TM_THREADS, 1) decode_tm_kernel(
         __syncwarp();
         if (lane == 0) {
           mbar_arrive(av_full0 + 8 * pg);
-          if (exists) mbar_arrive(empty0 + 8 * st);
+          if (exists) mbar_arrive(emptyV0 + 8 * st);
         }
       }
     }
   } else {
     setmaxnreg_dec<40>();
     if (warp == 20) {
-      // ================================== page producer (D2) ==================================
+      // ================================== page producer (D2): key blocks ==================================
       if (elect_one()) {
         const uint64_t pol = l2_evict_first_policy();
         mbar_expect_tx(imgbar, (uint32_t)T.img_bytes);
         bulk_g2s(smem_u32(smem + T.off_img), img_all + (size_t)b * img_stride, (uint32_t)T.img_bytes, imgbar);
         for (int j = 0; j < n_pg; ++j) {
-          const int st = j % nstage;
-          if (j >= nstage) mbar_wait(empty0 + 8 * st, (uint32_t)(((j / nstage) - 1) & 1));
+          const int st = j % nK;
+          if (j >= nK) mbar_wait(emptyK0 + 8 * st, (uint32_t)(((j / nK) - 1) & 1));
           const int page = j < TM_TBL ? tbl_s[j] : my_table[j];
-          mbar_expect_tx(full0 + 8 * st, page_bytes);
-          bulk_g2s_stream(smem_u32(stage_base + (size_t)st * page_bytes), pool + (size_t)page * page_bytes, page_bytes,
-                          full0 + 8 * st, pol);
+          mbar_expect_tx(fullK0 + 8 * st, (uint32_t)T.k_bytes);
+          bulk_g2s_stream(smem_u32(kstage_base + (size_t)st * T.kstride), pool + (size_t)page * page_bytes, (uint32_t)T.k_bytes,
+                          fullK0 + 8 * st, pol);
+        }
+      }
+      __syncwarp();
+    } else if (warp == 23) {
+      // ================================== page producer (D2): scales and value blocks ==================================
+      if (elect_one()) {
+        const uint64_t pol = l2_evict_first_policy();
+        for (int j = 0; j < n_pg; ++j) {
+          const int page = j < TM_TBL ? tbl_s[j] : my_table[j];
+          const uint8_t* src = pool + (size_t)page * page_bytes;
+          {
+            const int st = j % nS;
+            if (j >= nS) mbar_wait(emptyS0 + 8 * st, (uint32_t)(((j / nS) - 1) & 1));
+            const uint32_t dst = smem_u32(sstage_base + (size_t)st * T.sstride);
+            mbar_expect_tx(fullS0 + 8 * st, (uint32_t)(T.ks_bytes + T.vs_bytes));
+            bulk_g2s_stream(dst, src + L.k_scale_off, (uint32_t)T.ks_bytes, fullS0 + 8 * st, pol);
+            bulk_g2s_stream(dst + (uint32_t)T.ks_bytes, src + L.v_scale_off, (uint32_t)T.vs_bytes, fullS0 + 8 * st, pol);
+          }
+          {
+            const int st = j % nV;
+            if (j >= nV) mbar_wait(emptyV0 + 8 * st, (uint32_t)(((j / nV) - 1) & 1));
+            mbar_expect_tx(fullV0 + 8 * st, (uint32_t)T.v_bytes);
+            bulk_g2s_stream(smem_u32(vstage_base + (size_t)st * T.vstride), src + L.v_hi_off, (uint32_t)T.v_bytes, fullV0 + 8 * st, pol);
+          }
         }
       }
       __syncwarp();
@@ -865,19 +897,34 @@ int sk_tm_plan(starkv_ctx* ctx) {
   T.col_ds = T.col_ak + 8 + 8 * T.n_ks;
   T.ds_nbuf = (T.col_ds + 2 * T.ds_cols <= 512) ? 2 : 1;
   if (T.col_ds + T.ds_nbuf * T.ds_cols > 512) return 0;
+  // page parts (every block of the format is padded to 16 bytes, so the parts are bulk-copy aligned)
+  T.k_bytes = L.k_scale_off;
+  T.ks_bytes = L.v_hi_off - L.k_scale_off;
+  T.v_bytes = L.v_scale_off - L.v_hi_off;
+  T.vs_bytes = round_up(2 * PTOK * 2, 16);
+  T.kstride = round_up(T.k_bytes, 128);
+  T.vstride = round_up(T.v_bytes, 128);
+  T.sstride = round_up(T.ks_bytes + T.vs_bytes, 128);
   int off = 0;
-  const int fixed = round_up(T.img_bytes, 128) + 2 * 2 * P_BLK_BYTES + 1024 /* misc */ + 512 /* barriers */ + 4 * TM_TBL +
+  const int fixed = round_up(T.img_bytes, 128) + 2 * 2 * P_BLK_BYTES + 1024 /* misc */ + 1024 /* barriers */ + 4 * TM_TBL +
                     1024 /* base alignment */;
-  int ns = (ctx->smem_optin - fixed) / L.page_bytes;
-  if (ns > 12) ns = 12;
-  if (ns < 4) return 0;
-  T.nstage = ns;
-  T.off_stage = off; off += ns * L.page_bytes;
+  const int avail = ctx->smem_optin - fixed;
+  // the key rows are consumed first (a few stages cover the memory latency); values and scales wait for the softmax
+  // and the value MMAs, about three tiles deeper
+  int nk = 5;
+  int nv = (avail - nk * T.kstride) / (T.vstride + T.sstride);
+  if (nv > 14) nv = 14;
+  if (nv < 4) { nk = 3; nv = (avail - nk * T.kstride) / (T.vstride + T.sstride); }
+  if (nv < 4) return 0;
+  T.n_kstage = nk; T.n_vstage = nv; T.n_sstage = nv;
+  T.off_kstage = off; off += nk * T.kstride;
+  T.off_vstage = off; off += nv * T.vstride;
+  T.off_sstage = off; off += nv * T.sstride;
   off = round_up(off, 128);
   T.off_img = off; off += round_up(T.img_bytes, 128);
   T.off_p = off; off += 2 * 2 * P_BLK_BYTES;
   T.off_misc = off; off += 1024;
-  T.off_bar = off; off += 512;
+  T.off_bar = off; off += 1024;
   T.off_tbl = off; off += 4 * TM_TBL;
   T.smem_bytes = round_up(off, 128);
   if (T.smem_bytes > ctx->smem_optin) return 0;

@@ -27,7 +27,7 @@
 //        the channel's block; a 128-channel A tile that straddles the block boundary is multiplied with both operands
 //        into two accumulator tiles and each lane keeps its own.
 // Warp roles (24 warps, warpgroup-aligned so that setmaxnreg can move registers between them; the CTA owns 768 x 80
-// registers and the budgets 8 x 64 + 8 x 104 + 4 x 104 + 4 x 40 add up to exactly that -- setmaxnreg.inc can only
+// registers and the budgets 8 x 64 + 8 x 112 + 4 x 88 + 4 x 40 add up to exactly that -- setmaxnreg.inc can only
 // take what another warpgroup of the CTA released):
 //   0-3 / 4-7 key rows -> TMEM for the first / second half of the k-steps, 8-11 / 12-15 softmax of the lower / upper
 //   half of the query heads, 16-19 value rows -> TMEM, 20 page producer (cp.async.bulk ring), 21 QK MMA issue,
@@ -219,6 +219,16 @@ __device__ __forceinline__ int f_ordered(float v) {   // monotone map float -> i
 }
 __device__ __forceinline__ float f_unordered(int k) { return __int_as_float(k ^ ((k >> 31) & 0x7fffffff)); }
 
+// position of a consumer / producer in a ring of n stages: stage index and mbarrier phase parity, advanced without divisions
+struct RingPos {
+  int st, ph, n;
+  __device__ __forceinline__ RingPos(int j0, int n_) : st(j0 % n_), ph((j0 / n_) & 1), n(n_) {}
+  __device__ __forceinline__ void advance(int k) {   // k <= n
+    st += k;
+    if (st >= n) { st -= n; ph ^= 1; }
+  }
+};
+
 // NHH = query heads per softmax warpgroup (the heads are split over NSPLIT warpgroups), G = H_q / H_kv
 template <int NHH, int G, int NSPLIT>
 __global__ void __launch_bounds__(TM_THREADS, 1) decode_tm_kernel(
@@ -316,16 +326,17 @@ __global__ void __launch_bounds__(TM_THREADS, 1) decode_tm_kernel(
     const int n8 = T.n_trips8, nt = T.n_trips8 + T.n_trips4, nt0 = (nt + 1) >> 1;
     const int k_begin = half ? nt0 : 0, k_end = half ? nt : nt0;
     const uint4* desc4 = reinterpret_cast<const uint4*>(T.oct_desc);
-    for (int it = 0; it < n_it; ++it) {
+    RingPos rk(pgsel, nK);
+    const int dsh = ds_nbuf - 1;   // tile it uses score buffer it & dsh, for the (it >> dsh)-th time
+    for (int it = 0; it < n_it; ++it, rk.advance(2)) {
       const int j = 2 * it + pgsel;
       const bool exists = j < n_pg;
-      const int st = j % nK;
+      const int st = rk.st;
       uint4 dq = desc4[k_begin];
-      if (exists) mbar_wait(fullK0 + 8 * st, (uint32_t)((j / nK) & 1));
+      if (exists) mbar_wait(fullK0 + 8 * st, (uint32_t)rk.ph);
       const uint8_t* row = kstage_base + (size_t)st * T.kstride;
       if (it > 0) {   // the previous tile's score MMAs over this half have read the operand
-        const int pb = (it - 1) % ds_nbuf;
-        if (half) mbar_wait(qk_done0 + 8 * pb, (uint32_t)(((it - 1) / ds_nbuf) & 1));
+        if (half) mbar_wait(qk_done0 + 8 * ((it - 1) & dsh), (uint32_t)(((it - 1) >> dsh) & 1));
         else mbar_wait(qk_half, (uint32_t)((it - 1) & 1));
         tc_fence_after();
       }
@@ -375,7 +386,7 @@ __global__ void __launch_bounds__(TM_THREADS, 1) decode_tm_kernel(
     }
   } else if (warp < 16) {
     // ========================================= softmax (thread = token) =========================================
-    setmaxnreg_inc<104>();
+    setmaxnreg_inc<112>();
     const int hh = (warp - 8) >> 2;   // which half of the query heads
     if (hh < NSPLIT) {
       const int wq = warp & 3, wr = warp - 8, tq = wq * 32 + lane, pgsel = tq >> 6, slot = tq & 63;
@@ -408,39 +419,35 @@ __global__ void __launch_bounds__(TM_THREADS, 1) decode_tm_kernel(
       bar_sync(BAR_SM, NBAR);
 
       uint32_t d[2 * NHH];
-      for (int it = 0; it < n_it; ++it) {
+      RingPos rs(pgsel, nS);
+      const int dsh = ds_nbuf - 1;
+      for (int it = 0; it < n_it; ++it, rs.advance(2)) {
         const int j = 2 * it + pgsel;
         const bool exists = j < n_pg;
-        const int st = j % nS;
+        const int st = rs.st;
         const int buf = it & 1;
-        const int sb = it % ds_nbuf;
+        const int sb = it & dsh;
         if (!(ds_nbuf == 2 && it > 0)) {   // (double-buffered score tiles: loaded ahead, at the end of the previous tile's arithmetic)
-          mbar_wait(qk_done0 + 8 * sb, (uint32_t)((it / ds_nbuf) & 1));
+          mbar_wait(qk_done0 + 8 * sb, (uint32_t)((it >> dsh) & 1));
           tc_fence_after();
           tmem_ld<2 * NHH>(tlane + (uint32_t)(T.col_ds + sb * T.ds_cols + 2 * hbase), d);
         }
-        if (exists) mbar_wait(fullS0 + 8 * st, (uint32_t)((j / nS) & 1));
+        if (exists) mbar_wait(fullS0 + 8 * st, (uint32_t)rs.ph);
         const uint8_t* sslot = sstage_base + (size_t)st * T.sstride;   // [key scales][value scales] of the page
         const uint16_t* ksc = reinterpret_cast<const uint16_t*>(sslot) + slot;
         const uint16_t* vsc = reinterpret_cast<const uint16_t*>(sslot + T.ks_bytes) + slot;
         const bool valid = exists && ((p0 + j) * PTOK + slot) < len;
+        // unconditional loads (slots past the sequence end and heads past the last hold finite or junk bits that the
+        // selects below discard): no divergent regions, one base address
         float sc[2 * (NHH / G)];
 #pragma unroll
         for (int hl = 0; hl < NHH / G; ++hl) {
-          const int kvh = hbase / G + hl;
-          float shi = 0.f, slo = 0.f;
-          if (kvh < n_kv && valid) {
-            shi = h_bits_to_f(ksc[(2 * kvh) * PTOK]) * ce_s[2 * kvh];
-            slo = h_bits_to_f(ksc[(2 * kvh + 1) * PTOK]) * ce_s[2 * kvh + 1];
-          }
-          sc[2 * hl] = shi;
-          sc[2 * hl + 1] = slo;
+          const int kvh = min(hbase / G + hl, n_kv - 1);
+          sc[2 * hl] = h_bits_to_f(ksc[(2 * kvh) * PTOK]) * ce_s[2 * kvh];
+          sc[2 * hl + 1] = h_bits_to_f(ksc[(2 * kvh + 1) * PTOK]) * ce_s[2 * kvh + 1];
         }
-        float sv0 = 0.f, sv1 = 0.f;
-        if (valid) {
-          sv0 = h_bits_to_f(vsc[0]);
-          sv1 = h_bits_to_f(vsc[PTOK]);
-        }
+        const float sv0 = valid ? h_bits_to_f(vsc[0]) : 0.f;
+        const float sv1 = valid ? h_bits_to_f(vsc[PTOK]) : 0.f;
         const float M0 = M_s[0], M1 = M_s[1];
         tmem_wait_ld();
         tc_fence_before();
@@ -607,7 +614,7 @@ __global__ void __launch_bounds__(TM_THREADS, 1) decode_tm_kernel(
     }
   } else if (warp < 20) {
     // =============================== value rows -> A operand of the value product ===============================
-    setmaxnreg_inc<104>();
+    setmaxnreg_inc<88>();
     const int wq = warp - 16, tq = wq * 32 + lane;
     const uint32_t tl = tbase + ((uint32_t)(wq * 32) << 16) + (uint32_t)T.col_av;
     int roff[2];
@@ -622,13 +629,14 @@ __global__ void __launch_bounds__(TM_THREADS, 1) decode_tm_kernel(
       four[m] = bits == 4;
       roff[m] = act[m] ? (lo ? L.v_lo_off + (ch - L.v_hi_n) * rowb : L.v_hi_off + ch * rowb) : 0;
     }
+    RingPos rv(0, nV);
     for (int it = 0; it < n_it; ++it) {
 #pragma unroll 1
-      for (int pg = 0; pg < 2; ++pg) {
+      for (int pg = 0; pg < 2; ++pg, rv.advance(1)) {
         const int j = 2 * it + pg;
         const bool exists = j < n_pg;
-        const int st = j % nV;
-        if (exists) mbar_wait(fullV0 + 8 * st, (uint32_t)((j / nV) & 1));
+        const int st = rv.st;
+        if (exists) mbar_wait(fullV0 + 8 * st, (uint32_t)rv.ph);
         if (it > 0) {   // the previous tile's value MMAs over this half of the tokens have read the operand
           if (pg == 0) mbar_wait(pv_half, (uint32_t)((it - 1) & 1));
           else mbar_wait(pv_done0 + 8 * ((it - 1) & 1), (uint32_t)(((it - 1) >> 1) & 1));
@@ -678,9 +686,10 @@ __global__ void __launch_bounds__(TM_THREADS, 1) decode_tm_kernel(
         const uint64_t pol = l2_evict_first_policy();
         mbar_expect_tx(imgbar, (uint32_t)T.img_bytes);
         bulk_g2s(smem_u32(smem + T.off_img), img_all + (size_t)b * img_stride, (uint32_t)T.img_bytes, imgbar);
-        for (int j = 0; j < n_pg; ++j) {
-          const int st = j % nK;
-          if (j >= nK) mbar_wait(emptyK0 + 8 * st, (uint32_t)(((j / nK) - 1) & 1));
+        RingPos rp(0, nK);
+        for (int j = 0; j < n_pg; ++j, rp.advance(1)) {
+          const int st = rp.st;
+          if (j >= nK) mbar_wait(emptyK0 + 8 * st, (uint32_t)(rp.ph ^ 1));
           const int page = j < TM_TBL ? tbl_s[j] : my_table[j];
           mbar_expect_tx(fullK0 + 8 * st, (uint32_t)T.k_bytes);
           bulk_g2s_stream(smem_u32(kstage_base + (size_t)st * T.kstride), pool + (size_t)page * page_bytes, (uint32_t)T.k_bytes,
@@ -692,20 +701,21 @@ __global__ void __launch_bounds__(TM_THREADS, 1) decode_tm_kernel(
       // ================================== page producer (D2): scales and value blocks ==================================
       if (elect_one()) {
         const uint64_t pol = l2_evict_first_policy();
-        for (int j = 0; j < n_pg; ++j) {
+        RingPos rs(0, nS), rv(0, nV);
+        for (int j = 0; j < n_pg; ++j, rs.advance(1), rv.advance(1)) {
           const int page = j < TM_TBL ? tbl_s[j] : my_table[j];
           const uint8_t* src = pool + (size_t)page * page_bytes;
           {
-            const int st = j % nS;
-            if (j >= nS) mbar_wait(emptyS0 + 8 * st, (uint32_t)(((j / nS) - 1) & 1));
+            const int st = rs.st;
+            if (j >= nS) mbar_wait(emptyS0 + 8 * st, (uint32_t)(rs.ph ^ 1));
             const uint32_t dst = smem_u32(sstage_base + (size_t)st * T.sstride);
             mbar_expect_tx(fullS0 + 8 * st, (uint32_t)(T.ks_bytes + T.vs_bytes));
             bulk_g2s_stream(dst, src + L.k_scale_off, (uint32_t)T.ks_bytes, fullS0 + 8 * st, pol);
             bulk_g2s_stream(dst + (uint32_t)T.ks_bytes, src + L.v_scale_off, (uint32_t)T.vs_bytes, fullS0 + 8 * st, pol);
           }
           {
-            const int st = j % nV;
-            if (j >= nV) mbar_wait(emptyV0 + 8 * st, (uint32_t)(((j / nV) - 1) & 1));
+            const int st = rv.st;
+            if (j >= nV) mbar_wait(emptyV0 + 8 * st, (uint32_t)(rv.ph ^ 1));
             mbar_expect_tx(fullV0 + 8 * st, (uint32_t)T.v_bytes);
             bulk_g2s_stream(smem_u32(vstage_base + (size_t)st * T.vstride), src + L.v_hi_off, (uint32_t)T.v_bytes, fullV0 + 8 * st, pol);
           }
@@ -724,10 +734,10 @@ __global__ void __launch_bounds__(TM_THREADS, 1) decode_tm_kernel(
       for (int it = 0; it < n_it; ++it) {
 #pragma unroll 1
         for (int half = 0; half < 2; ++half) {
-          const int sb = it % ds_nbuf;
+          const int sb = it & (ds_nbuf - 1);
           const uint32_t t_dsb = t_ds + (uint32_t)(sb * T.ds_cols);
           mbar_wait(ak_full0 + 8 * half, (uint32_t)(it & 1));
-          if (half == 0 && it >= ds_nbuf) mbar_wait(ds_free0 + 8 * sb, (uint32_t)(((it / ds_nbuf) - 1) & 1));   // tile it - ds_nbuf has been read
+          if (half == 0 && it >= ds_nbuf) mbar_wait(ds_free0 + 8 * sb, (uint32_t)(((it >> (ds_nbuf - 1)) - 1) & 1));   // tile it - ds_nbuf has been read
           tc_fence_after();
           if (elect_one()) {
             if (half == 0) umma_ts_f16(t_dsb, t_ak, dconst, id_const, 0u);

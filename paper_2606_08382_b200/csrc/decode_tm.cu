@@ -448,22 +448,43 @@ __global__ void __launch_bounds__(TM_THREADS, 1) decode_tm_kernel(
         }
         const float sv0 = valid ? h_bits_to_f(vsc[0]) : 0.f;
         const float sv1 = valid ? h_bits_to_f(vsc[PTOK]) : 0.f;
-        const float M0 = M_s[0], M1 = M_s[1];
         tmem_wait_ld();
         tc_fence_before();
         __syncwarp();
         if (lane == 0) mbar_arrive(ds_free0 + 8 * sb);
         float arg[NHH];
+#pragma unroll
+        for (int hl = 0; hl < NHH / G; ++hl)
+#pragma unroll
+          for (int g = 0; g < G; ++g)
+            arg[hl * G + g] = fmaf(sc[2 * hl], __uint_as_float(d[2 * hl * G + g]), sc[2 * hl + 1] * __uint_as_float(d[2 * hl * G + G + g]));
+        if (it == 0) {
+          // The references start from the range's first token (always inside the sequence): its scores, and 2^8 times its
+          // value scales.  A later token that exceeds them by the lazy bounds takes the (rare) update path below, so the
+          // common case never runs that code at all -- it would run instruction-cache cold on every CTA.
+          if (tq == 0) {
+#pragma unroll
+            for (int i = 0; i < NHH; ++i) mref_s[hbase + i] = arg[i] - P_OFFSET;
+            if (hh == 0) {
+#pragma unroll
+              for (int blk = 0; blk < 2; ++blk) {
+                const float sv = blk ? sv1 : sv0;
+                unsigned eb = ((__float_as_uint(sv) >> 23) & 0xffu) + 8u;   // (a single token: 2^8 of headroom)
+                if (eb > 254u) eb = 254u;
+                const float M = sv > 0.f ? __uint_as_float(eb << 23) : 1.f;
+                M_s[blk] = M;
+                invM_s[blk] = 1.f / M;
+              }
+            }
+          }
+          bar_sync(BAR_SM, NBAR);
+        }
+        const float M0 = M_s[0], M1 = M_s[1];
         float mxa = -INFINITY;
 #pragma unroll
-        for (int hl = 0; hl < NHH / G; ++hl) {
-#pragma unroll
-          for (int g = 0; g < G; ++g) {
-            const int i = hl * G + g;
-            const float s = fmaf(sc[2 * hl], __uint_as_float(d[2 * hl * G + g]), sc[2 * hl + 1] * __uint_as_float(d[2 * hl * G + G + g]));
-            arg[i] = valid ? s - mref_s[hbase + i] : -INFINITY;
-            if (hbase + i < Hq) mxa = fmaxf(mxa, arg[i]);
-          }
+        for (int i = 0; i < NHH; ++i) {
+          arg[i] = valid ? arg[i] - mref_s[hbase + i] : -INFINITY;
+          if (hbase + i < Hq) mxa = fmaxf(mxa, arg[i]);
         }
         if (ds_nbuf == 2 && it + 1 < n_it) {
           // the next tile's scores: its MMAs ran while this tile was being read, so the TMEM load's latency hides behind the
@@ -473,8 +494,7 @@ __global__ void __launch_bounds__(TM_THREADS, 1) decode_tm_kernel(
           tc_fence_after();
           tmem_ld<2 * NHH>(tlane + (uint32_t)(T.col_ds + sn * T.ds_cols + 2 * hbase), d);
         }
-        bool trig = valid && (mxa > TAU + P_OFFSET || sv0 > M0 || sv1 > M1);
-        if (it == 0) trig = true;
+        const bool trig = valid && (mxa > TAU + P_OFFSET || sv0 > M0 || sv1 > M1);
         const bool wany = __any_sync(0xffffffffu, trig);
         if (lane == 0) {
           flag[buf * 8 + wr] = wany ? 1 : 0;
@@ -504,7 +524,7 @@ __global__ void __launch_bounds__(TM_THREADS, 1) decode_tm_kernel(
             const float mt = f_unordered(max(max(redh[i], redh[RED_STRIDE + i]), max(redh[2 * RED_STRIDE + i], redh[3 * RED_STRIDE + i])));
             const float m_old = mref_s[hbase + i];    // (references are stored as m - 8)
             // only a maximum that the tile exceeds moves (to the true maximum so far); the first tile sets it
-            float m_new = (it == 0) ? mt - P_OFFSET : fmaxf(mt - P_OFFSET, m_old);
+            float m_new = fmaxf(mt - P_OFFSET, m_old);
             if (!(m_new > -INFINITY)) m_new = m_old;
             const float delta = m_old - m_new;       // <= 0 after the first tile
             fs[i] = ex2(delta);
@@ -517,7 +537,7 @@ __global__ void __launch_bounds__(TM_THREADS, 1) decode_tm_kernel(
           for (int blk = 0; blk < 2; ++blk) {
             const float sm = __uint_as_float((unsigned)max(max(redh[16 + blk], redh[RED_STRIDE + 16 + blk]),
                                                            max(redh[2 * RED_STRIDE + 16 + blk], redh[3 * RED_STRIDE + 16 + blk])));
-            const float M_old = blk ? M1 : M0;
+            const float M_old = M_s[blk];
             float M_new = M_old;
             if (sm > M_old) {   // a power of two 8-16 times above the largest scale seen: later tiles rarely exceed it
               unsigned eb = ((__float_as_uint(sm) >> 23) & 0xffu) + 4u;

@@ -286,13 +286,16 @@ def _latent_block(g: np.random.Generator, n: int, r: int, kappa: float,
     return (z * sig).astype(np.float16)
 
 
-def make_latents(cfg: Config, n_tokens: int, seq: int = 0, regime: str = "diffuse"):
+def make_latents(cfg: Config, n_tokens: int, seq: int = 0, regime: str = "diffuse",
+                 clip: Optional[float] = KEY_OUTLIER_CLIP):
     """Latent cache contents for one sequence, fp16: L_k [n, sum r_h], L_v [n, r_v].
 
     z[t,c] = kappa * sigma_c * g,  sigma_c = exp(-c/(r/2)),  g ~ N(0,1); a seeded
     ``outlier_frac`` of tokens draws g from Student-t(df=3) instead.  Key latents use
     kappa_h = tau / (sm_scale * sqrt(sum_c sigma_c^2)) so that, for unit-variance projected
     queries, scores have standard deviation ~tau (REGIME_TAU); value latents use kappa = 1.
+    ``clip`` bounds the Student-t draws of the KEY latents (default +-KEY_OUTLIER_CLIP; ``None`` = unclipped, as
+    BASELINE.json words the workload -- parity tests run both).
     """
     tau = REGIME_TAU[regime]
     outlier = None
@@ -303,7 +306,7 @@ def make_latents(cfg: Config, n_tokens: int, seq: int = 0, regime: str = "diffus
         sig2 = float(np.sum(np.exp(-np.arange(r) / (r / 2.0)) ** 2))
         kappa = tau / (cfg.sm_scale * math.sqrt(sig2))
         g = _rng(cfg.seed, _S_LAT_K, (cfg.layer * 65536 + seq) * 256 + h)
-        lk[:, off:off + r] = _latent_block(g, n_tokens, r, kappa, outlier, KEY_OUTLIER_CLIP)
+        lk[:, off:off + r] = _latent_block(g, n_tokens, r, kappa, outlier, clip)
     g = _rng(cfg.seed, _S_LAT_V, cfg.layer * 65536 + seq)
     lv = _latent_block(g, n_tokens, cfg.rank_v, 1.0, outlier)
     return lk, lv

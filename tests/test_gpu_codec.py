@@ -148,7 +148,7 @@ def test_append_gaussian_inputs_close(n_new):
     cfg = synth.make_config("C3", context=256, batch=3)
     d, lay, got, ref, n = _append_case(cfg, "dense", n_new, dyadic=False)
     frac = float((got != ref).mean())
-    assert frac < 2e-3, frac
+    assert frac < 1e-3, frac   # SURVEY pin P15: code mismatches on <= 1e-3 of the entries
     # compare decoded values of the touched pages
     n_pages = got.shape[0]
     a = ocodec.unpack_pages(d, got, n_pages * lay.page_tokens)

@@ -18,8 +18,8 @@ sk = pytest.importorskip("paper_2606_08382_b200")
 TOL = 2e-3
 
 
-def _check(cfg, seq_lens=None, regime="diffuse", generic=False, splits=0, heads=None, tol=TOL):
-    cache = build_cache(cfg, seq_lens=seq_lens, regime=regime)
+def _check(cfg, seq_lens=None, regime="diffuse", generic=False, splits=0, heads=None, tol=TOL, clip=synth.KEY_OUTLIER_CLIP):
+    cache = build_cache(cfg, seq_lens=seq_lens, regime=regime, clip=clip)
     bk, bv = synth.make_factors(cfg)
     q = synth.make_q(cfg, batch=len(cache["seq_lens"]))
     ref = oattn.decode_attn(cache["desc"], q, cache["pool"], cache["table"], cache["seq_lens"], bk, bv, heads=heads)
@@ -167,15 +167,36 @@ def test_long_page_ranges_per_cta(name, ctx, splits):
     _check(cfg, seq_lens=[ctx - 17], splits=splits)
 
 
-@pytest.mark.parametrize("name", ["C2", "C3", "C4", "C5"])
-def test_full_baseline_size_in_the_bench_launch_configuration(name):
+@pytest.mark.parametrize("name,regime", [("C2", "diffuse"), ("C3", "diffuse"), ("C3", "peaky"), ("C4", "diffuse"), ("C5", "diffuse")])
+def test_full_baseline_size_in_the_bench_launch_configuration(name, regime):
     """BASELINE.json's full sizes (batch, context, ranks) through starkv_decode_attn with the automatic split
     count bench.py times (one CTA per SM); the oracle evaluates a seeded sample of query heads on every
-    sequence (it reconstructs K, V for the sampled heads only)."""
+    sequence (it reconstructs K, V for the sampled heads only).  C3 (the headline configuration) also in the peaky
+    regime, where maxima keep moving and the accumulators are rescaled."""
     cfg = synth.make_config(name)
     rng = np.random.default_rng(11)
     heads = sorted(int(h) for h in rng.choice(cfg.n_q_heads, size=3, replace=False))
-    _check(cfg, heads=heads)
+    _check(cfg, heads=heads, regime=regime)
+
+
+@pytest.mark.parametrize("regime", ["diffuse", "peaky"])
+@pytest.mark.parametrize("variant", ["auto", "tc5", "mma"])
+def test_unclipped_student_t_key_outliers(regime, variant):
+    """BASELINE.json configs[2]: "10% heavy-tailed outlier tokens (Student-t, df=3)" -- with NO clip on the key latents
+    (synth clips them at 6 sigma by default).  |g| reaches 10^2, so single tokens capture the softmax, the running
+    maximum jumps by far more than the lazy bound and the 4-bit absmax scales stretch.  C3's shape, 8192 tokens."""
+    cfg = synth.make_config("C3", context=8192, batch=2)
+    ctx = sk.create_from_config(cfg)
+    sk.starkv_set_option(ctx, "decode_variant", sk.DECODE_VARIANTS[variant])
+    cache = build_cache(cfg, seq_lens=[8192, 5000], regime=regime, clip=None)
+    assert max(float(np.abs(lk.astype(np.float64)).max()) for lk, _ in cache["lat"]) > 20.0   # the outliers are really there
+    bk, bv = synth.make_factors(cfg)
+    q = synth.make_q(cfg, batch=2)
+    ref = oattn.decode_attn(cache["desc"], q, cache["pool"], cache["table"], cache["seq_lens"], bk, bv)
+    out = run_decode(cfg, cache, q, bk, bv, ctx=ctx)
+    assert np.isfinite(out).all()
+    err = row_rel_err(out, ref)
+    assert err <= TOL, f"{variant} {regime}: row rel err {err:.3e}"
 
 
 def test_fast_matches_generic_on_a_larger_case():
@@ -189,11 +210,12 @@ def test_fast_matches_generic_on_a_larger_case():
     assert row_rel_err(b, a) <= TOL
 
 
+@pytest.mark.parametrize("vscale", [1e-3, 3e-2])
 @pytest.mark.parametrize("D", [10, 12, 14, 16])
-def test_underflow_closed_form(D):
-    """Pin P16 on the GPU: one token at score +D (natural log units) over N equal tokens, constant value
-    codes: out = (v0 + N e^-D v) / (1 + N e^-D) -- exercises fp16 P underflow handling."""
-    cfg = synth.custom_config("uf", 1, 4, 1, 64, 32768, [16], 32, bits=(8, 4), rank_v_hi=16)
+def test_underflow_closed_form(D, vscale):
+    """Pin P16 on the GPU at the survey's size: one token at score +D (natural log units) over N = 131071 equal
+    tokens, constant value codes: out = (v0 + N e^-D v) / (1 + N e^-D) -- the 128K underflow regime of fp16 P."""
+    cfg = synth.custom_config("uf", 1, 4, 1, 64, 131072, [16], 32, bits=(8, 4), rank_v_hi=16)
     n = cfg.context
     bk, bv = synth.make_factors(cfg)
     q = synth.make_q(cfg, batch=1)
@@ -202,10 +224,10 @@ def test_underflow_closed_form(D):
     u = qt / np.dot(qt, qt)
     lk = np.zeros((n, 16), np.float16)
     lk[0] = (D * u).astype(np.float16)
-    lv = np.full((n, 32), np.float16(1e-3))
+    lv = np.full((n, 32), np.float16(vscale))
     lv[0] = np.float16(0.5)
     cache = build_cache(cfg, seq_lens=[n], latents=[(lk, lv)])
-    ref = oattn.decode_attn(cache["desc"], q, cache["pool"], cache["table"], cache["seq_lens"], bk, bv)
+    ref = oattn.decode_attn(cache["desc"], q, cache["pool"], cache["table"], cache["seq_lens"], bk, bv, heads=[0])
     out = run_decode(cfg, cache, q, bk, bv)
     assert row_rel_err(out[:, :1], ref[:, :1]) <= TOL
 

@@ -151,11 +151,12 @@ def test_P14_gqa_heads_with_identical_query_agree():
     assert not np.allclose(out[0, 0], out[0, 4])
 
 
-@pytest.mark.parametrize("D", [10.0, 14.0])
-def test_P16_one_dominant_token_over_many_equal_ones(D):
+@pytest.mark.parametrize("N,D,vscale", [(4095, 10.0, 1e-3), (4095, 14.0, 1e-3),
+                                        (131071, 10.0, 1e-3), (131071, 12.0, 3e-2), (131071, 14.0, 1e-3), (131071, 16.0, 3e-2)])
+def test_P16_one_dominant_token_over_many_equal_ones(N, D, vscale):
     """Closed form: token 0 at score +D over N equal tokens of score 0, constant codes:
-    out = (v0 + N e^-D v) / (1 + N e^-D)."""
-    N = 4095
+    out = (v0 + N e^-D v) / (1 + N e^-D).  N = 131071 with value scales 1e-3 and 3e-2 is SURVEY's P16 size (the
+    128K underflow regime of the headline configuration)."""
     cfg = synth.custom_config("t", 1, 1, 1, 16, N + 1, [8], 8, bits=(8, 4), page_tokens=64,
                               rank_k_hi=[8], rank_v_hi=8)
     d = CacheDesc.from_config(cfg)
@@ -166,7 +167,7 @@ def test_P16_one_dominant_token_over_many_equal_ones(D):
     q[0, 0, 0] = 4.0                                   # sm_scale = 1/4 -> score = latent channel 0
     lk = np.zeros((N + 1, 8), np.float16)
     lk[0, 0] = D                                       # exactly representable after 8-bit quant: absmax -> qmax
-    lv = np.full((N + 1, 8), 1e-3, np.float16)
+    lv = np.full((N + 1, 8), vscale, np.float16)
     lv[0] = 0.5
     c = build_cache(cfg, latents=[(lk, lv)])
     un = codec.unpack_pages(d, c["pool"][c["table"][0]], N + 1)["dequant"]
@@ -198,6 +199,56 @@ def test_P17_hidden_state_and_dense_kv_modes_give_same_latent():
     hidden_mode = x @ A
     dense_mode = (x @ W.T) @ B.T                       # dense K row times A_dense = U_r = B^T
     assert np.allclose(hidden_mode, dense_mode, atol=1e-12)
+
+
+def test_append_hidden_state_mode_against_a_per_head_loop_and_the_dense_mode():
+    """oracle.append.project_latents in HIDDEN-STATE mode (k_head_stride = 0, d_in = d_model; §3.2
+    K' = x (Sigma V)_K): every KV head reads the SAME input row and its own columns of A_k.  Pinned (i) against an
+    explicit scalar loop per head and column, and (ii) through W = U S V^T against the dense-KV mode of the same
+    routine (k_head_stride = d_h), which must give the same latent: x (V S)_r == (x W^T) U_r.  A stride mistake in
+    either mode fails one of the two."""
+    rng = np.random.default_rng(23)
+    dmodel, dh, n = 24, 16, 5
+    cfg = synth.custom_config("t", 1, 4, 2, dh, 32, [8, 16], 16, page_tokens=16)
+    d = CacheDesc.from_config(cfg)
+    # dyadic-grid inputs so that every sum is exact in double and in fp16 after one rounding
+    x = (rng.integers(-8, 9, size=(n, dmodel)) / 8.0).astype(np.float16)
+    ak = (rng.integers(-16, 17, size=(dmodel, d.sum_rank_k)) / 16.0 * (rng.random((dmodel, d.sum_rank_k)) < 0.3)).astype(np.float16)
+    av = (rng.integers(-16, 17, size=(dmodel, d.rank_v)) / 16.0 * (rng.random((dmodel, d.rank_v)) < 0.3)).astype(np.float16)
+    lk, lv = oappend.project_latents(d, x, 0, dmodel, x, ak, av)
+    for t in range(n):
+        for h, (off, r) in enumerate(zip(d.k_offsets(), d.rank_k)):
+            for c in range(r):
+                acc = 0.0
+                for j in range(dmodel):
+                    acc += float(x[t, j]) * float(ak[j, off + c])
+                assert np.float16(acc) == lk[t, off + c], (t, h, c)
+        for c in range(d.rank_v):
+            acc = sum(float(x[t, j]) * float(av[j, c]) for j in range(dmodel))
+            assert np.float16(acc) == lv[t, c]
+    # (ii) the two modes of the same routine agree through an SVD: head h projects x with W_h = U S V^T
+    xs = rng.standard_normal((n, dmodel))
+    lat_hidden = np.zeros((n, d.sum_rank_k))
+    a_hidden = np.zeros((dmodel, d.sum_rank_k))
+    a_dense = np.zeros((dh, d.sum_rank_k))
+    kd = np.zeros((n, d.n_kv_heads, dh))
+    for h, (off, r) in enumerate(zip(d.k_offsets(), d.rank_k)):
+        W = rng.standard_normal((dh, dmodel))
+        A, B, _ = analysis.svd_factors(W, r)          # A = (V S)_r [dmodel, r], B = U_r^T [r, dh]
+        a_hidden[:, off:off + r] = A
+        a_dense[:, off:off + r] = B.T
+        kd[:, h] = xs @ W.T
+        lat_hidden[:, off:off + r] = xs @ A
+    # (fp16 storage of inputs and factors perturbs both sides by ~2^-11 per term)
+    got_hidden, _ = oappend.project_latents(d, xs.astype(np.float16), 0, dmodel, xs.astype(np.float16), a_hidden.astype(np.float16), av)
+    got_dense, _ = oappend.project_latents(d, kd.reshape(n, -1).astype(np.float16), dh, dh, xs.astype(np.float16), a_dense.astype(np.float16), av)
+    scale = np.abs(lat_hidden).max()
+    assert np.abs(got_hidden.astype(np.float64) - lat_hidden).max() <= 4e-3 * scale * np.sqrt(dmodel)
+    assert np.abs(got_dense.astype(np.float64) - lat_hidden).max() <= 4e-3 * scale * np.sqrt(dmodel)
+    # and a deliberately wrong stride is caught by (ii): dense inputs read with stride 0 give head 0's row to every head
+    wrong, _ = oappend.project_latents(d, kd.reshape(n, -1).astype(np.float16), 0, dh, xs.astype(np.float16), a_dense.astype(np.float16), av)
+    off1 = d.k_offsets()[1]
+    assert np.abs(wrong.astype(np.float64)[:, off1:] - lat_hidden[:, off1:]).max() > 0.1 * scale
 
 
 def test_append_projection_is_plain_matmul_and_rounds_once():

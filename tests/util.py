@@ -6,7 +6,7 @@ from oracle import codec as ocodec
 from oracle.layout import CacheDesc, page_layout
 
 
-def build_cache(cfg, seq_lens=None, regime="diffuse", shuffle=True, latents=None):
+def build_cache(cfg, seq_lens=None, regime="diffuse", shuffle=True, latents=None, clip=synth.KEY_OUTLIER_CLIP):
     """Returns dict(desc, layout, pool uint8 [n_pool, page_bytes], table, seq_lens, lat=[(lk, lv)...])."""
     d = CacheDesc.from_config(cfg)
     lay = page_layout(d)
@@ -16,7 +16,7 @@ def build_cache(cfg, seq_lens=None, regime="diffuse", shuffle=True, latents=None
     lat = []
     for b, l in enumerate(seq_lens):
         l = int(l)
-        lk, lv = latents[b] if latents is not None else synth.make_latents(cfg, l, seq=b, regime=regime)
+        lk, lv = latents[b] if latents is not None else synth.make_latents(cfg, l, seq=b, regime=regime, clip=clip)
         lat.append((lk, lv))
         if l == 0:
             continue

@@ -13,6 +13,18 @@ int sk_cuda_fail(starkv_ctx* ctx, cudaError_t e, const char* what) {
 
 static bool aligned16(const void* p) { return ((uintptr_t)p & 15) == 0; }
 
+// A context belongs to the device it was created on (kernel attributes, tickets, pinned staging): a call made with
+// another device current is refused instead of launching there.
+static bool sk_device_ok(starkv_ctx* ctx) {
+  int dev = -1;
+  if (cudaGetDevice(&dev) != cudaSuccess) { (void)cudaGetLastError(); return false; }
+  if (dev != ctx->device) {
+    snprintf(ctx->err, sizeof(ctx->err), "context created on device %d, called with device %d current", ctx->device, dev);
+    return false;
+  }
+  return true;
+}
+
 // ---- pinned staging and graph cache of the HOST-buffer entry points ----
 static const size_t kPinDecode = 0;
 // grow a pinned staging block; the graph that captured the old address is dropped
@@ -122,13 +134,13 @@ size_t starkv_workspace_bytes(const starkv_ctx* ctx, int batch, int max_pages) {
 size_t starkv_append_workspace_bytes(const starkv_ctx* ctx, int n_new) { return ctx ? sk_append_ws_bytes(ctx, n_new) : 0; }
 
 int starkv_pack(starkv_ctx* ctx, const void* lk, const void* lv, int n_tokens, void* pages) {
-  if (!ctx) return STARKV_ERR_INVALID_ARG;
+  if (!ctx || !sk_device_ok(ctx)) return STARKV_ERR_INVALID_ARG;
   if (n_tokens > 0 && (!aligned16(lk) || !aligned16(lv) || !aligned16(pages))) return STARKV_ERR_INVALID_ARG;
   return sk_pack(ctx, lk, lv, n_tokens, pages);
 }
 
 int starkv_unpack(starkv_ctx* ctx, const void* pages, int n_tokens, int8_t* codes, uint16_t* scales, float* deq) {
-  if (!ctx) return STARKV_ERR_INVALID_ARG;
+  if (!ctx || !sk_device_ok(ctx)) return STARKV_ERR_INVALID_ARG;
   if (n_tokens > 0 && !aligned16(pages)) return STARKV_ERR_INVALID_ARG;
   return sk_unpack(ctx, pages, n_tokens, codes, scales, deq);
 }
@@ -137,7 +149,7 @@ int starkv_append(starkv_ctx* ctx, void* pool, const int32_t* table, int max_pag
                   const int32_t* positions, int n_new, const void* k_new, int64_t k_row_stride, int64_t k_head_stride,
                   int d_in_k, const void* v_new, int64_t v_row_stride, int d_in_v, const void* A_k, const void* A_v,
                   void* ws, size_t ws_bytes) {
-  if (!ctx) return STARKV_ERR_INVALID_ARG;
+  if (!ctx || !sk_device_ok(ctx)) return STARKV_ERR_INVALID_ARG;
   if (n_new > 0 && (!aligned16(pool) || !aligned16(ws))) return STARKV_ERR_INVALID_ARG;
   return sk_append(ctx, pool, table, max_pages, seq_ids, positions, n_new, k_new, k_row_stride, k_head_stride, d_in_k,
                    v_new, v_row_stride, d_in_v, A_k, A_v, ws, ws_bytes);
@@ -154,7 +166,7 @@ static int sk_decode_choice(const starkv_ctx* ctx) {
 
 static int check_decode_args(starkv_ctx* ctx, const void* q, const void* pool, const int32_t* table, int max_pages,
                              const int32_t* seq_lens, int batch, const void* B_k, const void* B_v, void* ws, void* out) {
-  if (!ctx || batch <= 0 || max_pages <= 0) return STARKV_ERR_INVALID_ARG;
+  if (!ctx || batch <= 0 || max_pages <= 0 || !sk_device_ok(ctx)) return STARKV_ERR_INVALID_ARG;
   if (!q || !pool || !table || !seq_lens || !B_k || !B_v || !ws || !out) return STARKV_ERR_INVALID_ARG;
   if (!aligned16(q) || !aligned16(B_k) || !aligned16(B_v) || !aligned16(ws) || !aligned16(out)) return STARKV_ERR_INVALID_ARG;
   if (((uintptr_t)pool & 127) != 0) return STARKV_ERR_INVALID_ARG;

@@ -680,6 +680,7 @@ __global__ void __launch_bounds__(512) append_write_kernel(const __grid_constant
   const int R = L.sum_rank_k + L.rank_v;
   const bool quant = L.bits_hi != 16;
   const int pos = positions[j];
+  if (pos < 0 || pos / P >= max_pages || seq_ids[j] < 0) return;   // caller error: skip the token rather than write wildly
   const int pidx = table[(size_t)seq_ids[j] * max_pages + pos / P];
   if (pidx < 0) return;
   uint8_t* pg = pool + (size_t)pidx * L.page_bytes;

@@ -598,10 +598,12 @@ __global__ void __launch_bounds__(NG * GW * 32, 1) decode_fast_kernel(
   const int j = lane & 3, R = lane >> 2;
   const int split = blockIdx.x, b = blockIdx.y;
   sk_pdl_trigger();
-  // seq_lens and the block table are caller-owned inputs (ctx.h): read ahead of the dependency wait, as is the
-  // shared-memory set-up, so that after the wait thread 0 only has to issue the first page copies
+  // Nothing global is read before the dependency wait: seq_lens and the block table may have been written by a kernel the
+  // caller enqueued right before this call (CUDA makes a predecessor's writes visible only after griddepcontrol.wait).
+  sk_pdl_wait();
   const int len = seq_lens[b];
-  const int n_pages = (len + PTOK - 1) / PTOK;
+  int n_pages = len > 0 ? (len + PTOK - 1) / PTOK : 0;
+  if (n_pages > max_pages) n_pages = max_pages;   // (a length past the table is a caller error: memory-safe, result undefined)
   int p0, p1;
   sk_split_range(n_pages, n_splits, 1, split, &p0, &p1);
   const int n_it = p1 - p0;
@@ -633,7 +635,7 @@ __global__ void __launch_bounds__(NG * GW * 32, 1) decode_fast_kernel(
     mbar_expect_tx(bar, page_bytes);
     __threadfence_block();   // the barrier is armed before any consumer can see the stage as issued
     issued[st] = it;
-    bulk_g2s_stream(smem_u32(stage_base + (size_t)st * page_bytes), pool + (size_t)page * page_bytes, page_bytes, bar,
+    bulk_g2s_stream(smem_u32(stage_base + (size_t)st * page_bytes), pool + (size_t)max(page, 0) * page_bytes, page_bytes, bar,
                     l2_evict_first_policy());
   };
   if (tid == 0) {
@@ -1000,10 +1002,12 @@ __global__ void __launch_bounds__(NG * GW * 32, 1) decode_tc5_kernel(
   const int j = lane & 3, R = lane >> 2;
   const int split = blockIdx.x, b = blockIdx.y;
   sk_pdl_trigger();
-  // seq_lens and the block table are caller-owned inputs (ctx.h): read ahead of the dependency wait, as is all the
-  // shared-memory and TMEM set-up, so that after the wait thread 0 only has to issue the first page copies
+  // Nothing global is read before the dependency wait: seq_lens and the block table may have been written by a kernel the
+  // caller enqueued right before this call (CUDA makes a predecessor's writes visible only after griddepcontrol.wait).
+  sk_pdl_wait();
   const int len = seq_lens[b];
-  const int n_pages = (len + PTOK - 1) / PTOK;
+  int n_pages = len > 0 ? (len + PTOK - 1) / PTOK : 0;
+  if (n_pages > max_pages) n_pages = max_pages;   // (a length past the table is a caller error: memory-safe, result undefined)
   int p0, p1;
   sk_split_range(n_pages, n_splits, 1, split, &p0, &p1);
   const int n_it = p1 - p0;
@@ -1040,7 +1044,7 @@ __global__ void __launch_bounds__(NG * GW * 32, 1) decode_tc5_kernel(
     __threadfence_block();   // the barrier is armed before any consumer can see the stage as issued (the refill runs on
                              // a warp of its own, off the group's critical path)
     issued[st] = it;
-    bulk_g2s_stream(smem_u32(stage_base + (size_t)st * page_bytes), pool + (size_t)page * page_bytes, page_bytes, bar,
+    bulk_g2s_stream(smem_u32(stage_base + (size_t)st * page_bytes), pool + (size_t)max(page, 0) * page_bytes, page_bytes, bar,
                     l2_evict_first_policy());
   };
 

@@ -710,7 +710,7 @@ __global__ void __launch_bounds__(TM_THREADS, 1) decode_tm_kernel(
         for (int j = 0; j < n_pg; ++j, rp.advance(1)) {
           const int st = rp.st;
           if (j >= nK) mbar_wait(emptyK0 + 8 * st, (uint32_t)(rp.ph ^ 1));
-          const int page = j < TM_TBL ? tbl_s[j] : my_table[j];
+          const int page = max(j < TM_TBL ? tbl_s[j] : my_table[j], 0);   // (a negative entry is a caller error: memory-safe)
           mbar_expect_tx(fullK0 + 8 * st, (uint32_t)T.k_bytes);
           bulk_g2s_stream(smem_u32(kstage_base + (size_t)st * T.kstride), pool + (size_t)page * page_bytes, (uint32_t)T.k_bytes,
                           fullK0 + 8 * st, pol);
@@ -723,7 +723,7 @@ __global__ void __launch_bounds__(TM_THREADS, 1) decode_tm_kernel(
         const uint64_t pol = l2_evict_first_policy();
         RingPos rs(0, nS), rv(0, nV);
         for (int j = 0; j < n_pg; ++j, rs.advance(1), rv.advance(1)) {
-          const int page = j < TM_TBL ? tbl_s[j] : my_table[j];
+          const int page = max(j < TM_TBL ? tbl_s[j] : my_table[j], 0);   // (a negative entry is a caller error: memory-safe)
           const uint8_t* src = pool + (size_t)page * page_bytes;
           {
             const int st = rs.st;

@@ -336,3 +336,36 @@ def test_append_host_variant_matches_device_variant(own_stream):
                               akd, avd, ws, wsb)
         torch.cuda.synchronize()
         assert torch.equal(pool_a, pool_b), step
+
+
+@pytest.mark.parametrize("variant", ["auto", "tc5", "mma", "generic"])
+def test_no_write_outside_the_buffers_it_was_given(variant):
+    """compute-sanitizer is closed on this GPU pool (profiles/README.md), so out-of-bounds WRITES are checked the slow
+    way: workspace and output sit between guard regions filled with a pattern, the page pool is compared byte for byte
+    (a decode call must not touch it), ragged lengths including an empty sequence and a one-token tail page."""
+    cfg = synth.make_config("C3", context=1000, batch=4)
+    ctx = sk.create_from_config(cfg)
+    sk.starkv_set_option(ctx, "decode_variant", sk.DECODE_VARIANTS[variant])
+    cache = build_cache(cfg, seq_lens=[1000, 0, 65, 513])
+    bk, bv = synth.make_factors(cfg)
+    from tests.gpu_util import dev, f16
+    pool = dev(cache["pool"])
+    pool_before = pool.clone()
+    table = dev(cache["table"].astype(np.int32))
+    lens = dev(np.asarray(cache["seq_lens"], np.int32))
+    B, max_pages = table.shape
+    q, bkd, bvd = f16(synth.make_q(cfg, batch=B)), f16(bk), f16(bv)
+    G = 4096
+    wsb = sk.starkv_workspace_bytes(ctx, B, max_pages)
+    ws_all = torch.full((wsb + 2 * G,), 0xA5, dtype=torch.uint8, device="cuda")
+    out_n = B * cfg.n_q_heads * cfg.head_dim
+    out_all = torch.full((out_n + 2 * G,), -7.0, dtype=torch.float16, device="cuda")
+    for _ in range(2):
+        sk.starkv_decode_attn(ctx, q, pool, table, max_pages, lens, B, bkd, bvd, ws_all[G:G + wsb], wsb, out_all[G:G + out_n])
+    torch.cuda.synchronize()
+    assert bool((ws_all[:G] == 0xA5).all()) and bool((ws_all[G + wsb:] == 0xA5).all()), "workspace guard overwritten"
+    assert bool((out_all[:G] == -7.0).all()) and bool((out_all[G + out_n:] == -7.0).all()), "output guard overwritten"
+    assert torch.equal(pool, pool_before), "decode wrote into the page pool"
+    out = out_all[G:G + out_n].view(B, cfg.n_q_heads, cfg.head_dim).double().cpu().numpy()
+    ref = oattn.decode_attn(cache["desc"], synth.make_q(cfg, batch=B), cache["pool"], cache["table"], cache["seq_lens"], bk, bv)
+    assert row_rel_err(out, ref) <= TOL

@@ -137,6 +137,21 @@ int starkv_decode_attn_generic(starkv_ctx* ctx, const void* q, const void* page_
                                const void* B_v, void* workspace, size_t workspace_bytes,
                                void* out);
 
+/* NEXT-1: decode attention with the paper's own key path -- latent keys are cached PRE-RoPE; per token
+ * the kernel dequantises, reconstructs K = L_k B_k, applies rotary position embedding at the token's position and then
+ * scores against the query (PAPER.md 3.3 L62-68: "RoPE ... is inserted between W_Q and U_K, preventing offline
+ * fusion"; A.6 L619-627).  Same arguments as starkv_decode_attn, plus:
+ *   q_rotated   the query AFTER its own rotation (the caller rotates q at the current position, as for dense attention)
+ *   pos_offset  device int32 [batch] or NULL: token t of sequence b sits at position pos_offset[b] + t (NULL = 0)
+ *   rope_theta  the base (10000 for LLaMA-2, 500000 for LLaMA-3.x); must be > 1
+ * Pairing: half-split (channel i with i + head_dim/2, angle position * theta^(-2i/head_dim)) -- the paper does not state
+ * it; reading R1.  This entry point runs a scalar, correctness-first kernel (r_h * head_dim multiply-adds per
+ * token and head; r_h <= 128); values, split-K and combine are the ones of starkv_decode_attn.  Same error codes. */
+int starkv_decode_attn_rope(starkv_ctx* ctx, const void* q_rotated, const void* page_pool,
+                            const int32_t* block_table, int max_pages, const int32_t* seq_lens,
+                            const int32_t* pos_offset, float rope_theta, int batch, const void* B_k,
+                            const void* B_v, void* workspace, size_t workspace_bytes, void* out);
+
 /* The two HOST-buffer variants below stage their host inputs in a pinned block owned by the context when the
  * context has a stream of its own (not the legacy / per-thread default stream): the caller's buffers are read
  * before the call returns, one host-to-device copy carries all inputs of the call, and with the "host_graph" option (starkv_set_option) in

@@ -85,6 +85,59 @@ def decode_attn(d: CacheDesc, q16: np.ndarray, pool: np.ndarray, block_table: np
     return out
 
 
+def rope_rotate(x: np.ndarray, positions: np.ndarray, theta: float) -> np.ndarray:
+    """Rotary position embedding of rows x[t, :d_h] at integer positions[t] (Su et al. 2024; §3.3:
+    "RoPE ... applied to the query and key states prior to computing attention scores").
+
+    Channel pairing: HALF-SPLIT -- channel i is rotated together with channel i + d_h/2 by the angle
+    positions[t] * theta^(-2i/d_h), i in [0, d_h/2) -- the convention of the LLaMA-family implementations the paper
+    evaluates.  The paper does not state the pairing (interleaved pairs (2i, 2i+1) are the other common choice):
+    DESIGN.md reading R1, parity with the authors' code UNPINNED."""
+    x = np.asarray(x, np.float64)
+    dh = x.shape[-1]
+    half = dh // 2
+    inv_freq = theta ** (-np.arange(half, dtype=np.float64) * 2.0 / dh)
+    ang = np.asarray(positions, np.float64)[:, None] * inv_freq[None, :]
+    c, sn = np.cos(ang), np.sin(ang)
+    x1, x2 = x[..., :half], x[..., half:]
+    return np.concatenate([x1 * c - x2 * sn, x2 * c + x1 * sn], axis=-1)
+
+
+def decode_attn_rope(d: CacheDesc, q16: np.ndarray, pool: np.ndarray, block_table: np.ndarray,
+                     seq_lens: Sequence[int], bk16: np.ndarray, bv16: np.ndarray, theta: float,
+                     pos_offset: Optional[Sequence[int]] = None, pos_stride: int = 1,
+                     heads: Optional[Sequence[int]] = None):
+    """The paper's own key path (NEXT-1; §3.3, A.6 L619-627), step by step in the paper's order:
+    latent keys are cached PRE-RoPE; per token: dequantise, reconstruct K = L_k B_k, apply RoPE at the token's position,
+    then q . K; softmax; values as in ``decode_attn`` ((p V') U_V).  ``q16`` is the query AFTER its own rotation (the
+    caller rotates q at the current position, as it does for dense attention; any float dtype).  Token t of sequence b
+    sits at position pos_offset[b] + pos_stride * t (defaults 0 and 1; stride 0 puts every token at one position, which
+    the pins use).  out float64 [B, H_q, d_h]."""
+    B = q16.shape[0]
+    dh, G = d.head_dim, d.group
+    heads = list(range(d.n_q_heads)) if heads is None else [int(h) for h in heads]
+    q = np.asarray(q16, np.float64)
+    bk = bk16.astype(np.float64)
+    bv = bv16.astype(np.float64)
+    koff = d.k_offsets()
+    out = np.zeros((B, d.n_q_heads, dh))
+    for b in range(B):
+        l = int(seq_lens[b])
+        if l == 0:
+            continue
+        pos = pos_stride * np.arange(l) + (0 if pos_offset is None else int(pos_offset[b]))
+        Lk, Lv = read_sequence(d, pool, block_table[b], l)
+        for i in heads:
+            g = i // G
+            Kg = Lk[:, koff[g]:koff[g] + d.rank_k[g]] @ bk[koff[g]:koff[g] + d.rank_k[g]]   # reconstruct [l, d_h]
+            Kg = rope_rotate(Kg, pos, theta)                                                   # RoPE at the token's position
+            s = (Kg @ q[b, i]) * d.sm_scale
+            p = np.exp(s - s.max())
+            Vg = Lv @ bv[:, g * dh:(g + 1) * dh]
+            out[b, i] = (p @ Vg) / p.sum()
+    return out
+
+
 def decode_attn_absorbed(d: CacheDesc, q16, pool, block_table, seq_lens, bk16, bv16):
     """Same result through the reordered products (§3.3): score =
     (q B_k^T) . L_k, out = ((p L_v) / sum p) B_v[:, slice].  Identity tests only."""

@@ -22,7 +22,7 @@ LIB_PATH = os.path.join(_HERE, "libstarkv.so")
 SYMBOLS = [
     "starkv_create", "starkv_destroy", "starkv_page_bytes", "starkv_workspace_bytes",
     "starkv_append_workspace_bytes", "starkv_pack", "starkv_unpack", "starkv_append",
-    "starkv_decode_attn", "starkv_decode_attn_generic", "starkv_decode_attn_host",
+    "starkv_decode_attn", "starkv_decode_attn_generic", "starkv_decode_attn_rope", "starkv_decode_attn_host",
     "starkv_append_host_workspace_bytes", "starkv_append_host", "starkv_set_kernel_timing",
     "starkv_last_decode_kernel_ms",
     "starkv_set_splits", "starkv_set_option", "starkv_last_launches", "starkv_decode_kernel_name", "starkv_strerror",
@@ -77,6 +77,8 @@ def _load() -> ctypes.CDLL:
                                   c_int, vp, vp, vp, c_sz]
     lib.starkv_append.restype = c_int
     dec = [vp, vp, vp, i32p, c_int, i32p, c_int, vp, vp, vp, c_sz, vp]
+    lib.starkv_decode_attn_rope.argtypes = [vp, vp, vp, i32p, c_int, i32p, i32p, ctypes.c_float, c_int, vp, vp, vp, c_sz, vp]
+    lib.starkv_decode_attn_rope.restype = c_int
     for name in ("starkv_decode_attn", "starkv_decode_attn_generic", "starkv_decode_attn_host"):
         getattr(lib, name).argtypes = dec
         getattr(lib, name).restype = c_int
@@ -202,6 +204,14 @@ def starkv_decode_attn(ctx, q, page_pool, block_table, max_pages, seq_lens, batc
                        workspace_bytes, out) -> None:
     _decode(_lib.starkv_decode_attn, ctx, q, page_pool, block_table, max_pages, seq_lens, batch, B_k, B_v,
             workspace, workspace_bytes, out)
+
+
+def starkv_decode_attn_rope(ctx, q_rotated, page_pool, block_table, max_pages, seq_lens, pos_offset, rope_theta, batch, B_k, B_v,
+                            workspace, workspace_bytes, out) -> None:
+    ctx._check(_lib.starkv_decode_attn_rope(ctx.handle, _ptr(q_rotated), _ptr(page_pool), _ptr(block_table), max_pages,
+                                            _ptr(seq_lens), _ptr(pos_offset) if pos_offset is not None else None,
+                                            ctypes.c_float(rope_theta), batch, _ptr(B_k), _ptr(B_v), _ptr(workspace),
+                                            workspace_bytes, _ptr(out)))
 
 
 def starkv_decode_attn_generic(ctx, q, page_pool, block_table, max_pages, seq_lens, batch, B_k, B_v, workspace,

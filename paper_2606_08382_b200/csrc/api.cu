@@ -193,6 +193,16 @@ int starkv_decode_attn_generic(starkv_ctx* ctx, const void* q, const void* pool,
   return sk_decode_generic(ctx, q, pool, table, max_pages, seq_lens, batch, B_k, B_v, ws, ws_bytes, out);
 }
 
+int starkv_decode_attn_rope(starkv_ctx* ctx, const void* q_rotated, const void* pool, const int32_t* table, int max_pages,
+                            const int32_t* seq_lens, const int32_t* pos_offset, float rope_theta, int batch, const void* B_k,
+                            const void* B_v, void* ws, size_t ws_bytes, void* out) {
+  const int rc = check_decode_args(ctx, q_rotated, pool, table, max_pages, seq_lens, batch, B_k, B_v, ws, out);
+  if (rc) return rc;
+  if (!(rope_theta > 1.f) || (ctx->L.head_dim & 1)) return STARKV_ERR_INVALID_ARG;
+  return sk_decode_generic(ctx, q_rotated, pool, table, max_pages, seq_lens, batch, B_k, B_v, ws, ws_bytes, out, 1, rope_theta,
+                           pos_offset);
+}
+
 // enqueue-only body shared by the direct and the captured path: copies from `q_src` / `len_src`, decode, copy to `out_dst`
 static int sk_decode_host_enqueue(starkv_ctx* ctx, const void* q_src, const void* pool, const int32_t* table, int max_pages,
                                   const int32_t* len_src, int batch, const void* B_k, const void* B_v, void* ws, size_t ws_bytes,

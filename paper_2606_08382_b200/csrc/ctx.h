@@ -149,7 +149,7 @@ struct SkWorkspace {   // carve-up of the caller's decode workspace
 void sk_plan_workspace(const starkv_ctx* ctx, int batch, int max_pages, SkWorkspace* w);
 int sk_decode_generic(starkv_ctx* ctx, const void* q, const void* pool, const int32_t* table, int max_pages,
                       const int32_t* seq_lens, int batch, const void* B_k, const void* B_v, void* ws,
-                      size_t ws_bytes, void* out);
+                      size_t ws_bytes, void* out, int rope = 0, float rope_theta = 0.f, const int32_t* pos_offset = nullptr);
 int sk_decode_fast(starkv_ctx* ctx, const void* q, const void* pool, const int32_t* table, int max_pages,
                    const int32_t* seq_lens, int batch, const void* B_k, const void* B_v, void* ws,
                    size_t ws_bytes, void* out);

@@ -30,31 +30,49 @@ __device__ __forceinline__ float field_value(const uint8_t* row, int idx, int bi
   return (float)((int)((row[idx >> 1] >> (4 * (idx & 1))) & 0xF) - 8);
 }
 
-// grid (n_splits, H_q, batch), 128 threads
+// grid (n_splits, H_q, batch), 128 threads.
+// ROPE = the paper's own key path (NEXT-1; §3.3, A.6 L619-627): the latent keys are cached pre-RoPE, so the
+// score cannot be taken in latent space -- per token: dequantise the latent, reconstruct K = L_k B_k, rotate it at the
+// token's position (half-split pairing, reading R1), then q . K with the caller's already-rotated q.  Scalar and
+// correctness-first (r_h d_h multiply-adds per token and head; angles in double so that positions of 10^5 keep the
+// 2e-3 parity bar): the tensor-core form ([T x r_h] . [r_h x d_h] per KV head) is the next step.
+template <bool ROPE>
 __global__ void __launch_bounds__(128) decode_generic_kernel(
     const __grid_constant__ StarkvLayout L, const __half* __restrict__ q, const uint8_t* __restrict__ pool,
     const int32_t* __restrict__ table, int max_pages, const int32_t* __restrict__ seq_lens,
-    const __half* __restrict__ B_k, float* __restrict__ parts, int n_splits) {
-  __shared__ float qt[256];   // latent-space query of this head (r_g <= head_dim <= 256)
+    const __half* __restrict__ B_k, float* __restrict__ parts, int n_splits, float rope_theta,
+    const int32_t* __restrict__ pos_offset) {
+  __shared__ float qt[256];   // latent-space query of this head (r_g <= head_dim <= 256); ROPE: the query itself
   __shared__ float pbuf[128];
   __shared__ float red[4];
+  extern __shared__ __align__(16) uint8_t dyn_smem[];   // ROPE: B_k block of the KV head [r][d_h] fp16, inverse frequencies [d_h/2] double
   const int split = blockIdx.x, head = blockIdx.y, b = blockIdx.z;
   const int g = head / L.group;
   const int P = L.page_tokens;
   const bool quant = L.bits_hi != 16;
   const int r = L.rank_k[g];
   const int len = seq_lens[b];
-  const int n_pages = (len + P - 1) / P;
+  int n_pages = len > 0 ? (len + P - 1) / P : 0;
+  if (n_pages > max_pages) n_pages = max_pages;
   int p0, p1;
   sk_split_range(n_pages, n_splits, 1, split, &p0, &p1);
+  const int dh = L.head_dim, half_d = dh >> 1;
+  __half* bks = reinterpret_cast<__half*>(dyn_smem);
+  double* invf = reinterpret_cast<double*>(dyn_smem + (((size_t)r * dh * 2 + 15) / 16) * 16);
 
-  // D1: q~ = sm_scale * log2e * q B_k^T
-  const __half* qrow = q + ((size_t)b * L.n_q_heads + head) * L.head_dim;
-  for (int c = threadIdx.x; c < r; c += blockDim.x) {
-    const __half* brow = B_k + (size_t)(L.koff[g] + c) * L.head_dim;
-    float a = 0.f;
-    for (int d = 0; d < L.head_dim; ++d) a = fmaf(__half2float(qrow[d]), __half2float(brow[d]), a);
-    qt[c] = a * L.sm_scale * kLog2e;
+  const __half* qrow = q + ((size_t)b * L.n_q_heads + head) * dh;
+  if (ROPE) {
+    for (int i = threadIdx.x; i < dh; i += blockDim.x) qt[i] = __half2float(qrow[i]) * L.sm_scale * kLog2e;
+    for (int i = threadIdx.x; i < r * dh; i += blockDim.x) bks[i] = B_k[(size_t)L.koff[g] * dh + i];
+    for (int i = threadIdx.x; i < half_d; i += blockDim.x) invf[i] = pow((double)rope_theta, -2.0 * (double)i / (double)dh);
+  } else {
+    // D1: q~ = sm_scale * log2e * q B_k^T
+    for (int c = threadIdx.x; c < r; c += blockDim.x) {
+      const __half* brow = B_k + (size_t)(L.koff[g] + c) * dh;
+      float a = 0.f;
+      for (int d = 0; d < dh; ++d) a = fmaf(__half2float(qrow[d]), __half2float(brow[d]), a);
+      qt[c] = a * L.sm_scale * kLog2e;
+    }
   }
   __syncthreads();
 
@@ -68,7 +86,34 @@ __global__ void __launch_bounds__(128) decode_generic_kernel(
       const int tok = pg * P + slot;
       const bool valid = slot < P && tok < len;
       float s = -INFINITY;
-      if (valid) {
+      if (ROPE && valid) {
+        // dequantised latent of the token, its reconstructed and rotated key against the query, one pair at a time
+        float lat[128];
+        const __half* ksc = reinterpret_cast<const __half*>(page + L.k_scale_off);
+        const uint8_t* row = page + L.k_hi_off[g] + (size_t)slot * (n_hi * L.bits_hi / 8);
+        const float s_hi = quant ? __half2float(ksc[(g * 2 + 0) * P + slot]) : 1.f;
+        for (int c = 0; c < n_hi; ++c) lat[c] = field_value(row, c, L.bits_hi) * s_hi;
+        if (quant && n_lo) {
+          const uint8_t* row2 = page + L.k_lo_off[g] + (size_t)slot * (n_lo * L.bits_lo / 8);
+          const float s_lo = __half2float(ksc[(g * 2 + 1) * P + slot]);
+          for (int c = 0; c < n_lo; ++c) lat[n_hi + c] = field_value(row2, c, L.bits_lo) * s_lo;
+        }
+        const double pos = (double)(tok + (pos_offset ? pos_offset[b] : 0));
+        float d = 0.f;
+        for (int i = 0; i < half_d; ++i) {
+          float k1 = 0.f, k2 = 0.f;
+          for (int c = 0; c < r; ++c) {
+            k1 = fmaf(lat[c], __half2float(bks[c * dh + i]), k1);
+            k2 = fmaf(lat[c], __half2float(bks[c * dh + i + half_d]), k2);
+          }
+          double sn, cs;
+          sincos(pos * invf[i], &sn, &cs);
+          const float cf = (float)cs, sf = (float)sn;
+          d = fmaf(qt[i], k1 * cf - k2 * sf, d);
+          d = fmaf(qt[i + half_d], k2 * cf + k1 * sf, d);
+        }
+        s = d;
+      } else if (valid) {
         const uint8_t* row = page + L.k_hi_off[g] + (size_t)slot * (n_hi * L.bits_hi / 8);
         float d = 0.f;
         for (int c = 0; c < n_hi; ++c) d = fmaf(qt[c], field_value(row, c, L.bits_hi), d);
@@ -481,7 +526,7 @@ int sk_launch_combine(starkv_ctx* ctx, const float* parts, int n_splits, int bat
 
 int sk_decode_generic(starkv_ctx* ctx, const void* q, const void* pool, const int32_t* table, int max_pages,
                       const int32_t* seq_lens, int batch, const void* B_k, const void* B_v, void* ws,
-                      size_t ws_bytes, void* out) {
+                      size_t ws_bytes, void* out, int rope, float rope_theta, const int32_t* pos_offset) {
   const StarkvLayout& L = ctx->L;
   ctx->last_launches = 0;
   if (L.rank_v > 512) return STARKV_ERR_UNSUPPORTED;
@@ -490,8 +535,20 @@ int sk_decode_generic(starkv_ctx* ctx, const void* q, const void* pool, const in
   if (ws_bytes < w.total) return STARKV_ERR_WORKSPACE;
   float* parts = reinterpret_cast<float*>((uint8_t*)ws + w.part_off);
   if (ctx->timing_on) SK_CUDA_CHECK(ctx, cudaEventRecord(ctx->ev0, ctx->stream));
-  decode_generic_kernel<<<dim3(w.n_splits, L.n_q_heads, batch), 128, 0, ctx->stream>>>(
-      L, (const __half*)q, (const uint8_t*)pool, table, max_pages, seq_lens, (const __half*)B_k, parts, w.n_splits);
+  if (rope) {
+    int r_max = 0;
+    for (int h = 0; h < L.n_kv_heads; ++h) r_max = L.rank_k[h] > r_max ? L.rank_k[h] : r_max;
+    if (r_max > 128) return STARKV_ERR_UNSUPPORTED;
+    const int smem = ((r_max * L.head_dim * 2 + 15) / 16) * 16 + (L.head_dim / 2) * 8;
+    if (smem > ctx->smem_optin) return STARKV_ERR_UNSUPPORTED;
+    SK_CUDA_CHECK(ctx, sk_need_smem(ctx, decode_generic_kernel<true>, smem));
+    decode_generic_kernel<true><<<dim3(w.n_splits, L.n_q_heads, batch), 128, smem, ctx->stream>>>(
+        L, (const __half*)q, (const uint8_t*)pool, table, max_pages, seq_lens, (const __half*)B_k, parts, w.n_splits, rope_theta,
+        pos_offset);
+  } else {
+    decode_generic_kernel<false><<<dim3(w.n_splits, L.n_q_heads, batch), 128, 0, ctx->stream>>>(
+        L, (const __half*)q, (const uint8_t*)pool, table, max_pages, seq_lens, (const __half*)B_k, parts, w.n_splits, 0.f, nullptr);
+  }
   SK_CUDA_CHECK(ctx, cudaGetLastError());
   if (ctx->timing_on) {
     SK_CUDA_CHECK(ctx, cudaEventRecord(ctx->ev1, ctx->stream));

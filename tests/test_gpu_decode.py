@@ -369,3 +369,35 @@ def test_no_write_outside_the_buffers_it_was_given(variant):
     out = out_all[G:G + out_n].view(B, cfg.n_q_heads, cfg.head_dim).double().cpu().numpy()
     ref = oattn.decode_attn(cache["desc"], synth.make_q(cfg, batch=B), cache["pool"], cache["table"], cache["seq_lens"], bk, bv)
     assert row_rel_err(out, ref) <= TOL
+
+
+@pytest.mark.parametrize("name,ctxlen", [("C1", 512), ("C3", 3000), ("C4", 700)])
+def test_rope_key_path_against_the_oracle(name, ctxlen):
+    """NEXT-1: starkv_decode_attn_rope (pre-RoPE latent keys: reconstruct, rotate at the token's position, score) against
+    oracle.attention.decode_attn_rope, positions offset by 100000 on one sequence (long-context angles), ragged lengths."""
+    theta = 500000.0 if name == "C3" else 10000.0
+    cfg = synth.make_config(name, context=ctxlen, batch=2)
+    lens = [ctxlen, max(1, ctxlen // 3)]
+    cache = build_cache(cfg, seq_lens=lens)
+    bk, bv = synth.make_factors(cfg)
+    q_raw = synth.make_q(cfg, batch=2).astype(np.float64)
+    offs = np.array([0, 100000], np.int32)
+    # the caller rotates q at the current (last) token's position; round to fp16 once, the same bits go to both sides
+    q = np.stack([oattn.rope_rotate(q_raw[b], np.full(cfg.n_q_heads, lens[b] - 1 + int(offs[b])), theta) for b in range(2)]).astype(np.float16)
+    ref = oattn.decode_attn_rope(cache["desc"], q, cache["pool"], cache["table"], cache["seq_lens"], bk, bv, theta, pos_offset=offs)
+    from tests.gpu_util import dev, f16
+    ctx = sk.create_from_config(cfg)
+    pool, table = dev(cache["pool"]), dev(cache["table"].astype(np.int32))
+    lens_d, offs_d = dev(np.asarray(lens, np.int32)), dev(offs)
+    B, max_pages = table.shape
+    wsb = sk.starkv_workspace_bytes(ctx, B, max_pages)
+    ws = torch.empty(wsb, dtype=torch.uint8, device="cuda")
+    out = torch.full((B, cfg.n_q_heads, cfg.head_dim), float("nan"), dtype=torch.float16, device="cuda")
+    sk.starkv_decode_attn_rope(ctx, f16(q), pool, table, max_pages, lens_d, offs_d, theta, B, f16(bk), f16(bv), ws, wsb, out)
+    torch.cuda.synchronize()
+    got = out.double().cpu().numpy()
+    assert np.isfinite(got).all()
+    assert row_rel_err(got, ref) <= TOL
+    # and it is not the position-free result
+    plain = run_decode(cfg, cache, q, bk, bv)
+    assert row_rel_err(plain, ref) > 10 * TOL

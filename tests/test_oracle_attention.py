@@ -306,3 +306,79 @@ def test_regimes_are_what_design_md_says():
             assert np.median(ne) >= 4096 / 16 and ne.min() >= 4096 / 256, ne
         else:
             assert np.median(ne) <= 200, ne
+
+
+# ------------------------------------------------------------------ NEXT-1: the paper's RoPE key path (oracle only)
+
+ROPE_THETA = 10000.0
+
+
+def _rope_case(l=37):
+    cfg = synth.custom_config("t", 2, 4, 2, 16, l, [8, 16], 16, bits=(8, 4), page_tokens=16)
+    c = build_cache(cfg, seq_lens=[l, l - 9])
+    bk, bv = synth.make_factors(cfg)
+    return cfg, c, bk, bv, synth.make_q(cfg)
+
+
+def test_rope_is_a_rotation():
+    """Position 0 is the identity, norms are preserved, and the inner product of two rotated vectors depends on the
+    position difference only (Su et al. 2024, the property PAPER.md §3.3 L62-68 relies on)."""
+    rng = np.random.default_rng(5)
+    x, y = rng.standard_normal((7, 16)), rng.standard_normal((7, 16))
+    assert np.array_equal(oattn.rope_rotate(x, np.zeros(7), ROPE_THETA), x)
+    pos = np.arange(7) * 13
+    rx = oattn.rope_rotate(x, pos, ROPE_THETA)
+    assert np.allclose(np.linalg.norm(rx, axis=1), np.linalg.norm(x, axis=1), rtol=1e-13)
+    a = np.sum(oattn.rope_rotate(x, pos + 5, ROPE_THETA) * oattn.rope_rotate(y, pos, ROPE_THETA), axis=1)
+    b = np.sum(oattn.rope_rotate(x, pos + 905, ROPE_THETA) * oattn.rope_rotate(y, pos + 900, ROPE_THETA), axis=1)
+    assert np.allclose(a, b, rtol=1e-10)
+
+
+def test_rope_all_tokens_at_one_position_is_the_position_free_path():
+    """Every key AND the query at the same position (pos_stride = 0): all relative positions are 0, so the RoPE path
+    must equal decode_attn -- it pins the reconstruct / rotate / score order and the value side against the pinned
+    position-free oracle."""
+    cfg, c, bk, bv, q = _rope_case()
+    want = oattn.decode_attn(c["desc"], q, c["pool"], c["table"], c["seq_lens"], bk, bv)
+    for p in (0, 123):
+        qr = np.stack([oattn.rope_rotate(q[b].astype(np.float64), np.full(cfg.n_q_heads, p), ROPE_THETA) for b in range(2)])
+        got = oattn.decode_attn_rope(c["desc"], qr, c["pool"], c["table"], c["seq_lens"], bk, bv, ROPE_THETA,
+                                     pos_offset=[p, p], pos_stride=0)
+        assert np.allclose(got, want, rtol=1e-10, atol=1e-13)
+
+
+def test_rope_output_is_invariant_to_a_common_position_offset():
+    cfg, c, bk, bv, q = _rope_case()
+    lens = c["seq_lens"]
+    outs = []
+    for off in (0, 1000):
+        qr = np.stack([oattn.rope_rotate(q[b].astype(np.float64), np.full(cfg.n_q_heads, lens[b] - 1 + off), ROPE_THETA)
+                       for b in range(2)])
+        outs.append(oattn.decode_attn_rope(c["desc"], qr, c["pool"], c["table"], lens, bk, bv, ROPE_THETA, pos_offset=[off, off]))
+    assert np.allclose(outs[0], outs[1], rtol=1e-9, atol=1e-12)
+    # and it is NOT the position-free result (the rotation does something)
+    plain = oattn.decode_attn(c["desc"], q, c["pool"], c["table"], lens, bk, bv)
+    assert np.abs(outs[0] - plain).max() > 1e-3
+
+
+def test_rope_hand_computed_two_token_case():
+    """Full rank, identity factors, fp16 latents, d_h = 16: both keys are e_0 before RoPE; channel 0 pairs with channel 8
+    at frequency theta^0 = 1, so RoPE(k, position 1) = cos(1) e_0 + sin(1) e_8.  With q = 2 e_0 and sm_scale = 1/sqrt 2:
+    s0 = sqrt 2, s1 = sqrt 2 cos 1; values v0 = e_0, v1 = e_1."""
+    d = CacheDesc(n_q_heads=1, n_kv_heads=1, head_dim=16, rank_k=[16], rank_k_hi=[16], rank_v=16, rank_v_hi=16,
+                  bits_hi=16, bits_lo=16, page_tokens=16, sm_scale=1.0 / np.sqrt(2.0))
+    lk = np.zeros((2, 16), np.float16)
+    lk[:, 0] = 1.0
+    lv = np.zeros((2, 16), np.float16)
+    lv[0, 0] = 1.0
+    lv[1, 1] = 1.0
+    pages = codec.pack_pages(d, lk, lv)
+    eye = np.eye(16, dtype=np.float16)
+    q = np.zeros((1, 1, 16), np.float16)
+    q[0, 0, 0] = 2.0
+    out = oattn.decode_attn_rope(d, q, pages, np.array([[0]], np.int32), [2], eye, eye, theta=ROPE_THETA)
+    s0, s1 = np.sqrt(2.0), np.sqrt(2.0) * np.cos(1.0)
+    w1 = np.exp(s1 - s0) / (1 + np.exp(s1 - s0))
+    want = np.zeros(16)
+    want[0], want[1] = 1 - w1, w1
+    assert np.allclose(out[0, 0], want, rtol=1e-13, atol=1e-15)

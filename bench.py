@@ -216,13 +216,11 @@ class Workload:
     def step(self, rep):
         """One whole-path step on replica ``rep`` with device-resident inputs (enqueue only)."""
         sk, c, B = self.sk, self.cfg, self.cfg.batch
-        sk.starkv_append(self.ctx, self.pool, self.table_of(rep), self.max_pages, self.seq_ids, self.positions, B,
-                         self.k_new, c.n_kv_heads * c.head_dim, c.head_dim, self.d_in_k, self.v_new, self.d_in_v,
-                         self.d_in_v, self.ak, self.av, self.aws, self.awsb)
-        n = sk.starkv_last_launches(self.ctx)
-        sk.starkv_decode_attn(self.ctx, self.q, self.pool, self.table_of(rep), self.max_pages, self.seq_lens, B,
-                              self.bk, self.bv, self.ws, self.wsb, self.out)
-        self.launches_per_step = n + sk.starkv_last_launches(self.ctx)
+        sk.starkv_decode_step(self.ctx, self.pool, self.table_of(rep), self.max_pages, self.seq_ids, self.positions, B,
+                              self.k_new, c.n_kv_heads * c.head_dim, c.head_dim, self.d_in_k, self.v_new, self.d_in_v,
+                              self.d_in_v, self.ak, self.av, self.aws, self.awsb, self.q, self.seq_lens, self.bk, self.bv,
+                              self.ws, self.wsb, self.out)
+        self.launches_per_step = sk.starkv_last_launches(self.ctx)
 
     def step_host(self, rep):
         """Same step through the HOST-buffer entry points; returns after `out` is back on the host."""
@@ -504,7 +502,7 @@ def run_ours(args, cfg, env, K, with_cpu):
         "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "f16", "data": "synthetic",
         "config": {"workload": workload_name(cfg), "parallelism": f"dp{world} (batch-sharded replicas, no collective)",
-                   "step": "starkv_append (1 new token / sequence, dense-KV mode) + starkv_decode_attn",
+                   "step": "starkv_decode_step = starkv_append (1 new token / sequence, dense-KV mode) + starkv_decode_attn, launch-fused",
                    "l2": f"each step reads a different one of {R} cache replicas "
                          f"({R * kernel_bytes(cfg) / 1e6:.0f} MB footprint vs 126 MB L2)",
                    "launch": "CUDA graph per step (device-resident leg)", "bytes_per_step": step_bytes(cfg)},
@@ -647,7 +645,7 @@ def run_c5(args, env, K):
                                f"heads x {c0.head_dim}, context {c0.context}, per-layer key ranks from the seeded profile "
                                f"(mean 32), value rank {c0.rank_v}, int8/int4 latents",
                    "parallelism": f"dp{world} (batch-sharded replicas, no collective)",
-                   "step": f"{n_layers} x (starkv_append of 1 new token / sequence + starkv_decode_attn)",
+                   "step": f"{n_layers} x starkv_decode_step (append of 1 new token / sequence + decode attention)",
                    "l2": f"{n_layers} distinct layer caches, {bytes_kern / 1e6:.0f} MB per step vs 126 MB L2",
                    "launch": "one CUDA graph per step", "bytes_per_step": bytes_step},
         "us_per_step_per_layer": ms_step * 1e3 / n_layers,

@@ -22,7 +22,7 @@ LIB_PATH = os.path.join(_HERE, "libstarkv.so")
 SYMBOLS = [
     "starkv_create", "starkv_destroy", "starkv_page_bytes", "starkv_workspace_bytes",
     "starkv_append_workspace_bytes", "starkv_pack", "starkv_unpack", "starkv_append",
-    "starkv_decode_attn", "starkv_decode_attn_generic", "starkv_decode_attn_rope", "starkv_decode_attn_host",
+    "starkv_decode_attn", "starkv_decode_step", "starkv_decode_attn_generic", "starkv_decode_attn_rope", "starkv_decode_attn_host",
     "starkv_append_host_workspace_bytes", "starkv_append_host", "starkv_set_kernel_timing",
     "starkv_last_decode_kernel_ms",
     "starkv_set_splits", "starkv_set_option", "starkv_last_launches", "starkv_decode_kernel_name", "starkv_strerror",
@@ -79,6 +79,9 @@ def _load() -> ctypes.CDLL:
     dec = [vp, vp, vp, i32p, c_int, i32p, c_int, vp, vp, vp, c_sz, vp]
     lib.starkv_decode_attn_rope.argtypes = [vp, vp, vp, i32p, c_int, i32p, i32p, ctypes.c_float, c_int, vp, vp, vp, c_sz, vp]
     lib.starkv_decode_attn_rope.restype = c_int
+    lib.starkv_decode_step.argtypes = [vp, vp, i32p, c_int, i32p, i32p, c_int, vp, c_i64, c_i64, c_int, vp, c_i64, c_int, vp, vp,
+                                       vp, c_sz, vp, i32p, vp, vp, vp, c_sz, vp]
+    lib.starkv_decode_step.restype = c_int
     for name in ("starkv_decode_attn", "starkv_decode_attn_generic", "starkv_decode_attn_host"):
         getattr(lib, name).argtypes = dec
         getattr(lib, name).restype = c_int
@@ -204,6 +207,16 @@ def starkv_decode_attn(ctx, q, page_pool, block_table, max_pages, seq_lens, batc
                        workspace_bytes, out) -> None:
     _decode(_lib.starkv_decode_attn, ctx, q, page_pool, block_table, max_pages, seq_lens, batch, B_k, B_v,
             workspace, workspace_bytes, out)
+
+
+def starkv_decode_step(ctx, page_pool, block_table, max_pages, seq_ids, positions, batch, k_new, k_row_stride, k_head_stride,
+                       d_in_k, v_new, v_row_stride, d_in_v, A_k, A_v, append_workspace, append_workspace_bytes, q, seq_lens,
+                       B_k, B_v, workspace, workspace_bytes, out) -> None:
+    ctx._check(_lib.starkv_decode_step(ctx.handle, _ptr(page_pool), _ptr(block_table), max_pages, _ptr(seq_ids),
+                                       _ptr(positions), batch, _ptr(k_new), k_row_stride, k_head_stride, d_in_k, _ptr(v_new),
+                                       v_row_stride, d_in_v, _ptr(A_k), _ptr(A_v), _ptr(append_workspace),
+                                       append_workspace_bytes, _ptr(q), _ptr(seq_lens), _ptr(B_k), _ptr(B_v),
+                                       _ptr(workspace), workspace_bytes, _ptr(out)))
 
 
 def starkv_decode_attn_rope(ctx, q_rotated, page_pool, block_table, max_pages, seq_lens, pos_offset, rope_theta, batch, B_k, B_v,

@@ -3,6 +3,7 @@
 #include <stdlib.h>
 #include <string.h>
 
+#include "append_small.cuh"
 #include "ctx.h"
 
 int sk_cuda_fail(starkv_ctx* ctx, cudaError_t e, const char* what) {
@@ -95,8 +96,8 @@ int starkv_create(starkv_ctx** out, const starkv_desc* d, void* cuda_stream) {
     return STARKV_ERR_CUDA;
   }
   ctx->pdl = 1;
-  if (cudaMalloc((void**)&ctx->tickets, SK_TICKETS * sizeof(int)) != cudaSuccess ||
-      cudaMemset(ctx->tickets, 0, SK_TICKETS * sizeof(int)) != cudaSuccess) {
+  if (cudaMalloc((void**)&ctx->tickets, (SK_TICKETS + SK_APPEND_TICKETS) * sizeof(int)) != cudaSuccess ||
+      cudaMemset(ctx->tickets, 0, (SK_TICKETS + SK_APPEND_TICKETS) * sizeof(int)) != cudaSuccess) {
     (void)cudaGetLastError();
     if (ctx->tickets) cudaFree(ctx->tickets);
     ctx->tickets = nullptr;   // the sliced combine is skipped
@@ -183,6 +184,32 @@ int starkv_decode_attn(starkv_ctx* ctx, const void* q, const void* pool, const i
     case SK_VARIANT_GENERIC: return sk_decode_generic(ctx, q, pool, table, max_pages, seq_lens, batch, B_k, B_v, ws, ws_bytes, out);
     default: return sk_decode_fast(ctx, q, pool, table, max_pages, seq_lens, batch, B_k, B_v, ws, ws_bytes, out);
   }
+}
+
+int starkv_decode_step(starkv_ctx* ctx, void* pool, const int32_t* table, int max_pages, const int32_t* seq_ids,
+                       const int32_t* positions, int batch, const void* k_new, int64_t k_row_stride, int64_t k_head_stride,
+                       int d_in_k, const void* v_new, int64_t v_row_stride, int d_in_v, const void* A_k, const void* A_v,
+                       void* append_ws, size_t append_ws_bytes, const void* q, const int32_t* seq_lens, const void* B_k,
+                       const void* B_v, void* ws, size_t ws_bytes, void* out) {
+  int rc = check_decode_args(ctx, q, pool, table, max_pages, seq_lens, batch, B_k, B_v, ws, out);
+  if (rc) return rc;
+  if (!seq_ids || !positions || !k_new || !v_new || !A_k || !A_v || !append_ws || !aligned16(append_ws) || d_in_k <= 0 ||
+      d_in_v <= 0)
+    return STARKV_ERR_INVALID_ARG;
+  if (append_ws_bytes < sk_append_ws_bytes(ctx, batch)) return STARKV_ERR_WORKSPACE;
+  if (sk_decode_choice(ctx) == SK_VARIANT_TM && sk_append_small_ok(ctx, batch)) {
+    AppendSmallArgs a;
+    sk_append_small_args(ctx, &a, pool, table, max_pages, seq_ids, positions, batch, k_new, k_row_stride, k_head_stride, d_in_k,
+                         v_new, v_row_stride, d_in_v, A_k, A_v, append_ws);
+    return sk_decode_tm(ctx, q, pool, table, max_pages, seq_lens, batch, B_k, B_v, ws, ws_bytes, out, &a);
+  }
+  rc = sk_append(ctx, pool, table, max_pages, seq_ids, positions, batch, k_new, k_row_stride, k_head_stride, d_in_k, v_new,
+                 v_row_stride, d_in_v, A_k, A_v, append_ws, append_ws_bytes);
+  if (rc) return rc;
+  const int n_app = ctx->last_launches;
+  rc = starkv_decode_attn(ctx, q, pool, table, max_pages, seq_lens, batch, B_k, B_v, ws, ws_bytes, out);
+  ctx->last_launches += n_app;
+  return rc;
 }
 
 int starkv_decode_attn_generic(starkv_ctx* ctx, const void* q, const void* pool, const int32_t* table, int max_pages,

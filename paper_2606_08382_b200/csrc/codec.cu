@@ -4,6 +4,7 @@
 //   DESIGN.md "Cache page format v1" (token-major K blocks, channel-major V blocks, offset-binary fields).
 #include <stdlib.h>
 
+#include "append_small.cuh"
 #include "common.cuh"
 #include "ctx.h"
 
@@ -250,85 +251,14 @@ __global__ void __launch_bounds__(128) append_project_kernel(
 }
 
 // ---------------------------------------------------------------------------------------------
-// append, step A1 for a handful of new tokens (decode-time append, n_new <= 16): z = X . A is bound by reading
-// A once, so the K dimension is split over gridDim.y blocks and 8 warps per block, 64 columns per block (one
-// half2 per lane and row); partial sums are reduced in a fixed order (deterministic) and written as fp32
-//   zp[ks][token][column];  the write kernel adds the gridDim.y partials, rounds once to fp16 and quantises.
-// grid (column tiles of keys then values, K splits), 256 threads.
+// append for a handful of new tokens (decode-time append, n_new <= 16): projection, quantiser and paged write in one
+// launch (append_small.cuh).  grid (column tiles of keys then values, K splits), 256 threads.
 // ---------------------------------------------------------------------------------------------
-constexpr int APS_COLS = 64, APS_KCH = 256, APS_TOK = 16, APS_KS_MAX = 16;   // K splits = ceil(d_in / 256) <= 16
-
-__global__ void __launch_bounds__(256) append_project_small_kernel(
-    const __grid_constant__ StarkvLayout L, int n_new, int n_key_tiles, const __half* __restrict__ k_new,
-    long long k_row_stride, long long k_head_stride, int d_in_k, const __half* __restrict__ v_new, long long v_row_stride,
-    int d_in_v, const __half* __restrict__ A_k, const __half* __restrict__ A_v, float* __restrict__ zp) {
-  __shared__ __align__(16) float sm[8 * APS_TOK * APS_COLS];   // x chunk [16][256] during the loop, then the warp partials
+__global__ void __launch_bounds__(APS_THREADS) append_small_kernel(const __grid_constant__ StarkvLayout L,
+                                                                  const __grid_constant__ AppendSmallArgs a) {
+  __shared__ __align__(16) float sm[APS_SM_FLOATS];
   sk_pdl_enter();
-  const int R = L.sum_rank_k + L.rank_v;
-  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-  const __half* x0;
-  long long xstride;
-  int d_in, ncols, col_out0, lda;
-  const __half* A;
-  if ((int)blockIdx.x < n_key_tiles) {
-    int h = 0, t = blockIdx.x;
-    while (t >= (L.rank_k[h] + APS_COLS - 1) / APS_COLS) { t -= (L.rank_k[h] + APS_COLS - 1) / APS_COLS; ++h; }
-    const int c0 = t * APS_COLS;
-    x0 = k_new + (long long)h * k_head_stride; xstride = k_row_stride; d_in = d_in_k;
-    ncols = min(APS_COLS, L.rank_k[h] - c0); col_out0 = L.koff[h] + c0; A = A_k + L.koff[h] + c0; lda = L.sum_rank_k;
-  } else {
-    const int c0 = (blockIdx.x - n_key_tiles) * APS_COLS;
-    x0 = v_new; xstride = v_row_stride; d_in = d_in_v;
-    ncols = min(APS_COLS, L.rank_v - c0); col_out0 = L.sum_rank_k + c0; A = A_v + c0; lda = L.rank_v;
-  }
-  const int per = ((d_in + (int)gridDim.y - 1) / (int)gridDim.y + 31) / 32 * 32;
-  const int k_begin = blockIdx.y * per, k_end = min(d_in, k_begin + per);
-  float acc[APS_TOK][2];
-#pragma unroll
-  for (int t = 0; t < APS_TOK; ++t) acc[t][0] = acc[t][1] = 0.f;
-  const bool col_ok = 2 * lane < ncols;
-  for (int kc = k_begin; kc < k_end; kc += APS_KCH) {
-    // this warp's 32 rows of A first (independent loads, all in flight), then the x chunk
-    const int kw = kc + warp * 32;
-    const int kn = col_ok ? max(0, min(32, k_end - kw)) : 0;
-    uint32_t av[32];
-    {
-      const __half* ap = A + (size_t)kw * lda + 2 * lane;
-#pragma unroll
-      for (int kk = 0; kk < 32; ++kk) av[kk] = kk < kn ? *reinterpret_cast<const uint32_t*>(ap + (size_t)kk * lda) : 0u;
-    }
-    __syncthreads();
-    for (int i = tid; i < APS_TOK * APS_KCH; i += 256) {
-      const int t = i / APS_KCH, k = i % APS_KCH;
-      sm[i] = (t < n_new && kc + k < k_end) ? __half2float(x0[(long long)t * xstride + kc + k]) : 0.f;
-    }
-    __syncthreads();
-    if (kn > 0) {
-      const float* xp = sm + warp * 32;
-#pragma unroll
-      for (int kk = 0; kk < 32; ++kk) {
-        const float2 a = __half22float2(*reinterpret_cast<const __half2*>(&av[kk]));
-#pragma unroll
-        for (int t = 0; t < APS_TOK; ++t) {
-          const float x = xp[t * APS_KCH + kk];
-          acc[t][0] = fmaf(x, a.x, acc[t][0]);
-          acc[t][1] = fmaf(x, a.y, acc[t][1]);
-        }
-      }
-    }
-  }
-  __syncthreads();
-#pragma unroll
-  for (int t = 0; t < APS_TOK; ++t)
-    *reinterpret_cast<float2*>(sm + (warp * APS_TOK + t) * APS_COLS + 2 * lane) = make_float2(acc[t][0], acc[t][1]);
-  __syncthreads();
-  for (int i = tid; i < APS_TOK * APS_COLS; i += 256) {
-    const int t = i / APS_COLS, c = i % APS_COLS;
-    float s = 0.f;
-#pragma unroll
-    for (int w = 0; w < 8; ++w) s += sm[(w * APS_TOK + t) * APS_COLS + c];
-    if (t < n_new && c < ncols) zp[((size_t)blockIdx.y * n_new + t) * R + col_out0 + c] = s;
-  }
+  append_small_body(L, a, blockIdx.x, blockIdx.y, sm);
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -789,7 +719,7 @@ int sk_pack(starkv_ctx* ctx, const void* lk, const void* lv, int n_tokens, void*
   const int n_pages = (n_tokens + L.page_tokens - 1) / L.page_tokens;
   const size_t smem = (size_t)L.page_bytes + 2 * L.page_tokens * sizeof(float);
   if ((int)smem > ctx->smem_optin) return STARKV_ERR_UNSUPPORTED;
-  SK_CUDA_CHECK(ctx, cudaFuncSetAttribute(pack_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+  SK_CUDA_CHECK(ctx, sk_need_smem(ctx, pack_kernel, (int)smem));
   pack_kernel<<<n_pages, 256, smem, ctx->stream>>>(L, (const __half*)lk, (const __half*)lv, n_tokens, (uint8_t*)pages);
   ctx->last_launches = 1;
   SK_CUDA_CHECK(ctx, cudaGetLastError());
@@ -817,6 +747,29 @@ size_t sk_append_ws_bytes(const starkv_ctx* ctx, int n_new) {
   return (b + 255) / 256 * 256;
 }
 
+int sk_append_small_ok(const starkv_ctx* ctx, int n_new) {
+  return n_new > 0 && n_new <= APS_TOK && n_new * ctx->L.rank_v <= APS_ZR_MAX && ctx->tickets != nullptr &&
+         ctx->L.n_kv_heads + 1 <= SK_APPEND_TICKETS;
+}
+
+void sk_append_small_args(const starkv_ctx* ctx, AppendSmallArgs* a, void* pool, const int32_t* table, int max_pages,
+                          const int32_t* seq_ids, const int32_t* positions, int n_new, const void* k_new, int64_t k_row_stride,
+                          int64_t k_head_stride, int d_in_k, const void* v_new, int64_t v_row_stride, int d_in_v,
+                          const void* A_k, const void* A_v, void* ws) {
+  const StarkvLayout& L = ctx->L;
+  int nkt = 0;
+  for (int h = 0; h < L.n_kv_heads; ++h) nkt += (L.rank_k[h] + APS_COLS - 1) / APS_COLS;
+  const int d_max = d_in_k > d_in_v ? d_in_k : d_in_v;
+  int n_part = (d_max + APS_KCH - 1) / APS_KCH;
+  if (n_part > APS_KS_MAX) n_part = APS_KS_MAX;
+  a->n_new = n_new; a->n_key_tiles = nkt; a->n_tiles = nkt + (L.rank_v + APS_COLS - 1) / APS_COLS; a->n_part = n_part;
+  a->k_new = (const __half*)k_new; a->k_row_stride = k_row_stride; a->k_head_stride = k_head_stride; a->d_in_k = d_in_k;
+  a->v_new = (const __half*)v_new; a->v_row_stride = v_row_stride; a->d_in_v = d_in_v;
+  a->A_k = (const __half*)A_k; a->A_v = (const __half*)A_v; a->zp = (float*)ws;
+  a->seq_ids = seq_ids; a->positions = positions; a->table = table; a->max_pages = max_pages; a->pool = (uint8_t*)pool;
+  a->tickets = ctx->tickets + SK_TICKETS;
+}
+
 int sk_append(starkv_ctx* ctx, void* pool, const int32_t* table, int max_pages, const int32_t* seq_ids,
               const int32_t* positions, int n_new, const void* k_new, int64_t k_row_stride, int64_t k_head_stride,
               int d_in_k, const void* v_new, int64_t v_row_stride, int d_in_v, const void* A_k, const void* A_v,
@@ -828,20 +781,14 @@ int sk_append(starkv_ctx* ctx, void* pool, const int32_t* table, int max_pages, 
   if (!pool || !table || !seq_ids || !positions || !k_new || !v_new || !A_k || !A_v || !ws) return STARKV_ERR_INVALID_ARG;
   if (ws_bytes < sk_append_ws_bytes(ctx, n_new)) return STARKV_ERR_WORKSPACE;
   __half* z = (__half*)ws;
-  const float* zp = nullptr;
-  int n_part = 1;
-  if (n_new <= APS_TOK) {
-    int nkt = 0;
-    for (int h = 0; h < L.n_kv_heads; ++h) nkt += (L.rank_k[h] + APS_COLS - 1) / APS_COLS;
-    const int nvt = (L.rank_v + APS_COLS - 1) / APS_COLS;
-    SK_PREFER_SMEM(ctx, append_project_small_kernel);
-    const int d_max = d_in_k > d_in_v ? d_in_k : d_in_v;
-    n_part = (d_max + APS_KCH - 1) / APS_KCH;
-    if (n_part > APS_KS_MAX) n_part = APS_KS_MAX;
-    sk_launch(ctx, append_project_small_kernel, dim3(nkt + nvt, n_part), dim3(256), 0,
-        L, n_new, nkt, (const __half*)k_new, k_row_stride, k_head_stride, d_in_k, (const __half*)v_new, v_row_stride, d_in_v,
-        (const __half*)A_k, (const __half*)A_v, (float*)ws);
-    zp = (const float*)ws;
+  if (sk_append_small_ok(ctx, n_new)) {
+    AppendSmallArgs a;
+    sk_append_small_args(ctx, &a, pool, table, max_pages, seq_ids, positions, n_new, k_new, k_row_stride, k_head_stride, d_in_k,
+                         v_new, v_row_stride, d_in_v, A_k, A_v, ws);
+    SK_PREFER_SMEM(ctx, append_small_kernel);
+    SK_CUDA_CHECK(ctx, sk_launch(ctx, append_small_kernel, dim3(a.n_tiles, a.n_part), dim3(APS_THREADS), 0, L, a));
+    ctx->last_launches = 1;
+    return STARKV_OK;
   } else if (d_in_k % 8 == 0 && d_in_v % 8 == 0 && k_row_stride % 8 == 0 && k_head_stride % 8 == 0 && v_row_stride % 8 == 0 &&
              ((uintptr_t)k_new & 15) == 0 && ((uintptr_t)v_new & 15) == 0 && ((uintptr_t)A_k & 15) == 0 &&
              ((uintptr_t)A_v & 15) == 0) {
@@ -877,7 +824,7 @@ int sk_append(starkv_ctx* ctx, void* pool, const int32_t* table, int max_pages, 
   if ((int)smem > ctx->smem_optin) return STARKV_ERR_UNSUPPORTED;
   if (smem > 48 * 1024) SK_CUDA_CHECK(ctx, sk_need_smem(ctx, append_write_kernel, (int)smem));
   SK_PREFER_SMEM(ctx, append_write_kernel);
-  sk_launch(ctx, append_write_kernel, dim3(n_new), dim3(512), smem, L, (const __half*)z, zp, n_part, n_new, seq_ids,
+  sk_launch(ctx, append_write_kernel, dim3(n_new), dim3(512), smem, L, (const __half*)z, (const float*)nullptr, 1, n_new, seq_ids,
             positions, table, max_pages, (uint8_t*)pool);
   ctx->last_launches = 2;
   SK_CUDA_CHECK(ctx, cudaGetLastError());

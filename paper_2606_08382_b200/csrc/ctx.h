@@ -52,6 +52,7 @@ struct starkv_ctx {
   char err[512];
 };
 #define SK_TICKETS 16384
+#define SK_APPEND_TICKETS 128   // after them: one arrival counter per group (KV head / values) of the small append
 
 // decode kernel variants (starkv_set_decode_variant)
 enum { SK_VARIANT_AUTO = 0, SK_VARIANT_MMA = 1, SK_VARIANT_TC5 = 2, SK_VARIANT_TM = 3, SK_VARIANT_GENERIC = 4 };
@@ -88,6 +89,13 @@ template <typename K>
 static inline cudaError_t sk_need_smem(const starkv_ctx* ctx, K kernel, int bytes) {
   bool fresh;
   starkv_ctx::KernelAttr* a = sk_attr_slot(ctx, (const void*)kernel, &fresh);
+  if (a && a->smem < 0) {
+    // the attribute belongs to the device's copy of the kernel, which other contexts share: start from what is
+    // already granted and only ever raise it (a context with a smaller plan must not shrink another one's limit)
+    cudaFuncAttributes fa;
+    if (cudaFuncGetAttributes(&fa, kernel) == cudaSuccess) a->smem = fa.maxDynamicSharedSizeBytes;
+    else cudaGetLastError();
+  }
   if (a && a->smem >= bytes) return cudaSuccess;
   const cudaError_t e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
   if (e == cudaSuccess && a) a->smem = bytes;
@@ -127,6 +135,8 @@ static inline cudaError_t sk_launch(const starkv_ctx* ctx, void (*kern)(KArgs...
 }
 #endif
 
+struct AppendSmallArgs;
+
 // codec.cu
 int sk_pack(starkv_ctx* ctx, const void* lk, const void* lv, int n_tokens, void* pages);
 int sk_unpack(starkv_ctx* ctx, const void* pages, int n_tokens, int8_t* codes, uint16_t* scales, float* deq);
@@ -135,6 +145,11 @@ int sk_append(starkv_ctx* ctx, void* pool, const int32_t* table, int max_pages, 
               int64_t k_head_stride, int d_in_k, const void* v_new, int64_t v_row_stride, int d_in_v,
               const void* A_k, const void* A_v, void* ws, size_t ws_bytes);
 size_t sk_append_ws_bytes(const starkv_ctx* ctx, int n_new);
+int sk_append_small_ok(const starkv_ctx* ctx, int n_new);   // the one-launch append covers n_new tokens
+void sk_append_small_args(const starkv_ctx* ctx, AppendSmallArgs* a, void* pool, const int32_t* table, int max_pages,
+                          const int32_t* seq_ids, const int32_t* positions, int n_new, const void* k_new, int64_t k_row_stride,
+                          int64_t k_head_stride, int d_in_k, const void* v_new, int64_t v_row_stride, int d_in_v,
+                          const void* A_k, const void* A_v, void* ws);
 
 // decode.cu / decode_generic.cu
 struct SkWorkspace {   // carve-up of the caller's decode workspace
@@ -158,4 +173,4 @@ int sk_fast_plan(starkv_ctx* ctx);   // fills ctx->plan, ctx->fast_ok
 int sk_tm_plan(starkv_ctx* ctx);     // fills ctx->tm
 int sk_decode_tm(starkv_ctx* ctx, const void* q, const void* pool, const int32_t* table, int max_pages,
                  const int32_t* seq_lens, int batch, const void* B_k, const void* B_v, void* ws, size_t ws_bytes,
-                 void* out);
+                 void* out, const AppendSmallArgs* app = nullptr);   // app: the step's append, run in the first launch

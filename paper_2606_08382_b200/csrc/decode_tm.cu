@@ -36,6 +36,7 @@
 // (two halves of the 128 tokens), so that the next tile's value rows are converted while the MMAs of this one run.
 #include <string.h>
 
+#include "append_small.cuh"
 #include "decode_common.cuh"
 #include "decode_plan.h"
 #include "sk_ptx.cuh"
@@ -62,14 +63,20 @@ constexpr int MISC_MREF = 0, MISC_M = 32, MISC_INVM = 34, MISC_RED = 36, RED_STR
 // the constant tile and its octets' rows of the k-step tiles.
 // ---------------------------------------------------------------------------------------------
 constexpr int QP_THREADS = 256, QP_WARPS = 8, QP_U = 8;
-__global__ void __launch_bounds__(QP_THREADS) qproj_tm_kernel(const __grid_constant__ StarkvLayout L, const __grid_constant__ TmPlan T,
-                                                              const __half* __restrict__ q, const __half* __restrict__ B_k,
-                                                              uint8_t* __restrict__ img_all, size_t img_stride) {
-  __shared__ float qt[128][4];                   // q~[channel of the block][g]
-  __shared__ float wmax[QP_WARPS];
-  __shared__ float cst[4];
-  __shared__ __align__(16) __half qs[4 * 256];   // the KV head's query rows
-  const int hb = blockIdx.x, b = blockIdx.y, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+struct QpShared {
+  float qt[128][4];                   // q~[channel of the block][g]
+  float wmax[QP_WARPS];
+  float cst[4];
+  __align__(16) __half qs[4 * 256];   // the KV head's query rows
+};
+__device__ __forceinline__ void qproj_tm_body(const StarkvLayout& L, const TmPlan& T, const __half* __restrict__ q,
+                                              const __half* __restrict__ B_k, uint8_t* __restrict__ img_all, size_t img_stride,
+                                              int hb, int b, QpShared& S) {
+  float (&qt)[128][4] = S.qt;
+  float (&wmax)[QP_WARPS] = S.wmax;
+  float (&cst)[4] = S.cst;
+  __half* qs = S.qs;
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const int h = hb >> 1, blk = hb & 1;
   const int G = L.group, dh = L.head_dim;
   const int nch = blk ? L.k_lo_n[h] : L.k_hi_n[h];
@@ -77,7 +84,6 @@ __global__ void __launch_bounds__(QP_THREADS) qproj_tm_kernel(const __grid_const
   const int col0 = L.koff[h] + (blk ? L.k_hi_n[h] : 0);
   const bool act = lane * 8 < dh;
   const float qscale = L.sm_scale * kLog2e;
-  sk_pdl_enter();
   uint8_t* img = img_all + (size_t)b * img_stride;
   {
     const uint4* src = reinterpret_cast<const uint4*>(q + ((size_t)b * L.n_q_heads + h * G) * dh);
@@ -208,6 +214,35 @@ __global__ void __launch_bounds__(QP_THREADS) qproj_tm_kernel(const __grid_const
     }
   }
   if (tid == 0) reinterpret_cast<float*>(img + T.img_scal_off)[hb] = ldexpf(1.f, 24 - e);
+}
+
+__global__ void __launch_bounds__(QP_THREADS) qproj_tm_kernel(const __grid_constant__ StarkvLayout L, const __grid_constant__ TmPlan T,
+                                                              const __half* __restrict__ q, const __half* __restrict__ B_k,
+                                                              uint8_t* __restrict__ img_all, size_t img_stride) {
+  __shared__ QpShared S;
+  sk_pdl_enter();
+  qproj_tm_body(L, T, q, B_k, img_all, img_stride, blockIdx.x, blockIdx.y, S);
+}
+
+// First launch of a fused decode step (starkv_decode_step): the query image and the compress-on-append of the step's new
+// tokens do not depend on each other, so they share one grid: blocks [0, n_qp) build the image, the rest run the small
+// append (append_small.cuh).  Both finish before the decode kernel's griddepcontrol.wait returns.
+static_assert(QP_THREADS == APS_THREADS, "the two bodies share a block size");
+__global__ void __launch_bounds__(QP_THREADS) step_pre_tm_kernel(const __grid_constant__ StarkvLayout L, const __grid_constant__ TmPlan T,
+                                                                 const __half* __restrict__ q, const __half* __restrict__ B_k,
+                                                                 uint8_t* __restrict__ img_all, size_t img_stride, int n_qp,
+                                                                 const __grid_constant__ AppendSmallArgs a) {
+  __shared__ __align__(16) float sm[APS_SM_FLOATS];
+  static_assert(sizeof(QpShared) <= sizeof(float) * APS_SM_FLOATS, "query-image scratch fits the append's shared memory");
+  sk_pdl_enter();
+  const int i = blockIdx.x;
+  if (i < n_qp) {
+    const int nhb = 2 * L.n_kv_heads;
+    qproj_tm_body(L, T, q, B_k, img_all, img_stride, i % nhb, i / nhb, *reinterpret_cast<QpShared*>(sm));
+  } else {
+    const int j = i - n_qp;
+    append_small_body(L, a, j % a.n_tiles, j / a.n_tiles, sm);
+  }
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -967,7 +1002,8 @@ int sk_tm_plan(starkv_ctx* ctx) {
 }
 
 int sk_decode_tm(starkv_ctx* ctx, const void* q, const void* pool, const int32_t* table, int max_pages,
-                 const int32_t* seq_lens, int batch, const void* B_k, const void* B_v, void* ws, size_t ws_bytes, void* out) {
+                 const int32_t* seq_lens, int batch, const void* B_k, const void* B_v, void* ws, size_t ws_bytes, void* out,
+                 const AppendSmallArgs* app) {
   const StarkvLayout& L = ctx->L;
   ctx->last_launches = 0;
   if (!ctx->tm.ok) return STARKV_ERR_UNSUPPORTED;
@@ -976,8 +1012,15 @@ int sk_decode_tm(starkv_ctx* ctx, const void* q, const void* pool, const int32_t
   if (ws_bytes < w.total) return STARKV_ERR_WORKSPACE;
   float* parts = reinterpret_cast<float*>((uint8_t*)ws + w.part_off);
   uint8_t* img = (uint8_t*)ws + w.qimg_off;
-  SK_CUDA_CHECK(ctx, sk_launch(ctx, qproj_tm_kernel, dim3(2 * L.n_kv_heads, batch), dim3(QP_THREADS), 0, L, ctx->tm, (const __half*)q,
-                               (const __half*)B_k, img, w.qimg_stride));
+  if (app) {
+    const int n_qp = 2 * L.n_kv_heads * batch;
+    SK_PREFER_SMEM(ctx, step_pre_tm_kernel);
+    SK_CUDA_CHECK(ctx, sk_launch(ctx, step_pre_tm_kernel, dim3(n_qp + app->n_tiles * app->n_part), dim3(QP_THREADS), 0, L, ctx->tm,
+                                 (const __half*)q, (const __half*)B_k, img, w.qimg_stride, n_qp, *app));
+  } else {
+    SK_CUDA_CHECK(ctx, sk_launch(ctx, qproj_tm_kernel, dim3(2 * L.n_kv_heads, batch), dim3(QP_THREADS), 0, L, ctx->tm,
+                                 (const __half*)q, (const __half*)B_k, img, w.qimg_stride));
+  }
   if (ctx->timing_on) SK_CUDA_CHECK(ctx, cudaEventRecord(ctx->ev0, ctx->stream));
   TmKernel k = tm_kernel_for(L.n_q_heads, L.group);
   SK_CUDA_CHECK(ctx, sk_launch(ctx, k, dim3(w.n_splits, batch), dim3(TM_THREADS), (size_t)ctx->tm.smem_bytes, L, ctx->tm,

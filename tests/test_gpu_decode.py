@@ -401,3 +401,77 @@ def test_rope_key_path_against_the_oracle(name, ctxlen):
     # and it is not the position-free result
     plain = run_decode(cfg, cache, q, bk, bv)
     assert row_rel_err(plain, ref) > 10 * TOL
+
+
+@pytest.mark.parametrize("name,ctxlen,batch", [("C3", 1500, 1), ("C5", 900, 4), ("C2", 700, 2), ("C4", 600, 3)])
+def test_fused_step_equals_append_then_decode_and_the_oracle(name, ctxlen, batch):
+    """starkv_decode_step (append of one new token per sequence + decode, three launches on the TMEM-operand kernel) leaves
+    the same cache bytes and the same output as starkv_append followed by starkv_decode_attn, and both agree with the
+    oracle's append + decode_attn (section 3.2 L58 then section 3.3).  Run twice on the same context: the arrival
+    counters of the one-launch append must be back at zero after a step."""
+    from oracle import append as oappend
+    from tests.gpu_util import dev, f16
+    cfg = synth.make_config(name, context=ctxlen, batch=batch)
+    lens0 = np.array([ctxlen - 1 - 37 * b for b in range(batch)], np.int32)     # tokens already cached
+    lens1 = lens0 + 1
+    cache = build_cache(cfg, seq_lens=lens1)          # pages sized for the new token; its slot holds filler bytes
+    bk, bv = synth.make_factors(cfg)
+    q = synth.make_q(cfg, batch=batch)
+    dk_in, dv_in = cfg.head_dim, cfg.n_kv_heads * cfg.head_dim
+    ak, av = synth.make_append_factors(cfg, dk_in, dv_in)
+    kn, vn = synth.make_append_inputs(cfg, batch, mode="dense")
+    k2, v2 = np.ascontiguousarray(kn.reshape(batch, -1)), np.ascontiguousarray(vn.reshape(batch, -1))
+    seq_ids, positions = np.arange(batch, dtype=np.int32), lens0.copy()
+    table = cache["table"].astype(np.int32)
+    ref_pool = cache["pool"].copy()
+    oappend.append(cache["desc"], ref_pool, table, seq_ids, positions, k2, cfg.head_dim, dk_in, v2, ak, av)
+    ref = oattn.decode_attn(cache["desc"], q, ref_pool, table, lens1, bk, bv)
+
+    ctx = sk.create_from_config(cfg)
+    mp = table.shape[1]
+    wsb, awsb = sk.starkv_workspace_bytes(ctx, batch, mp), sk.starkv_append_workspace_bytes(ctx, batch)
+    ws, aws = torch.empty(wsb, dtype=torch.uint8, device="cuda"), torch.empty(awsb, dtype=torch.uint8, device="cuda")
+    d = dict(table=dev(table), seq=dev(seq_ids), pos=dev(positions), lens=dev(lens1), k=f16(k2), v=f16(v2), ak=f16(ak),
+             av=f16(av), q=f16(q), bk=f16(bk), bv=f16(bv))
+    res = []
+    for fused in (True, False, True):
+        pool = dev(cache["pool"])
+        out = torch.zeros((batch, cfg.n_q_heads, cfg.head_dim), dtype=torch.float16, device="cuda")
+        if fused:
+            sk.starkv_decode_step(ctx, pool, d["table"], mp, d["seq"], d["pos"], batch, d["k"], k2.shape[1], cfg.head_dim, dk_in,
+                                  d["v"], v2.shape[1], dv_in, d["ak"], d["av"], aws, awsb, d["q"], d["lens"], d["bk"], d["bv"],
+                                  ws, wsb, out)
+            if sk.starkv_decode_kernel_name(ctx) == "decode_tm_kernel":
+                assert sk.starkv_last_launches(ctx) == 3
+        else:
+            sk.starkv_append(ctx, pool, d["table"], mp, d["seq"], d["pos"], batch, d["k"], k2.shape[1], cfg.head_dim, dk_in,
+                             d["v"], v2.shape[1], dv_in, d["ak"], d["av"], aws, awsb)
+            assert sk.starkv_last_launches(ctx) == 1
+            sk.starkv_decode_attn(ctx, d["q"], pool, d["table"], mp, d["lens"], batch, d["bk"], d["bv"], ws, wsb, out)
+        torch.cuda.synchronize()
+        res.append((pool.cpu().numpy(), out.cpu().numpy()))
+    for p, o in res[1:]:
+        assert np.array_equal(p, res[0][0]) and np.array_equal(o.view(np.uint16), res[0][1].view(np.uint16))
+    got_pool, got = res[0]
+    frac = float((got_pool != ref_pool).mean())
+    assert frac < 1e-5, frac                       # Gaussian inputs: a last-bit fp16 difference may move a code (pin P15)
+    err = row_rel_err(got.astype(np.float64), ref)
+    assert err <= TOL, f"{name}: row rel err {err:.3e}"
+
+
+def test_contexts_with_different_shared_memory_plans_alternate():
+    """The dynamic shared-memory limit of a kernel is a per-device attribute that all contexts share: a context with a
+    smaller plan, created later, must not shrink the limit a live context launches with (the 32 layers of C5 have 32
+    different rank profiles, hence 32 plans)."""
+    big = synth.custom_config("big", 1, 32, 8, 128, 1500, [40, 40, 48, 32, 40, 40, 48, 32], 256, bits=(8, 4))
+    small = synth.custom_config("small", 1, 32, 8, 128, 1500, [8, 8, 8, 8, 8, 8, 8, 8], 64, bits=(8, 4))
+    ctxs, caches = [], []
+    for cfg in (big, small):
+        ctxs.append(sk.create_from_config(cfg))
+        caches.append(build_cache(cfg, seq_lens=[1500]))
+    for cfg, ctx, cache in list(zip((big, small), ctxs, caches)) * 2:
+        bk, bv = synth.make_factors(cfg)
+        q = synth.make_q(cfg, batch=1)
+        ref = oattn.decode_attn(cache["desc"], q, cache["pool"], cache["table"], cache["seq_lens"], bk, bv)
+        out = run_decode(cfg, cache, q, bk, bv, ctx=ctx)
+        assert row_rel_err(out, ref) <= TOL

@@ -7,9 +7,16 @@
  *   - Every `const void*` / `void*` data argument is a DEVICE pointer unless the name ends in
  *     `_host` or the comment says HOST.  The descriptor and its rank tables are HOST memory and
  *     are copied at starkv_create.
- *   - The caller owns every buffer.  The library allocates nothing on the device after
- *     starkv_create, keeps no reference to caller buffers between calls, never mutates
- *     `seq_lens` or `block_table`.
+ *   - The caller owns every buffer.  starkv_create allocates the context's own device state (64 KB of zeroed
+ *     arrival counters); after that the DEVICE-pointer entry points allocate nothing, on the device or the host.
+ *     The two `_host` entry points are the exception: on first use (and when a call needs more) they allocate a
+ *     pinned host staging block, and with the "host_graph" option they instantiate and cache CUDA graphs; all of
+ *     it is freed by starkv_destroy.  The library keeps no reference to caller buffers between calls and never
+ *     mutates `seq_lens` or `block_table`.
+ *   - Preconditions on index inputs (not checked on the host; the kernels stay memory-safe when they are broken, the
+ *     result is then unspecified): 0 <= seq_lens[b] <= max_pages * page_tokens (longer is clamped to the table);
+ *     block_table entries of the pages in use are valid page indices of the pool (negative entries are read as
+ *     page 0 by decode and skipped by append); append positions lie inside the table (others are skipped).
  *   - Every call only enqueues work on the context's CUDA stream and returns (no host sync);
  *     all entry points are CUDA-graph capturable.  The `_host` variants are the exception: they
  *     copy host buffers in, run, copy the result out and synchronise the stream.
@@ -220,6 +227,10 @@ int starkv_last_launches(const starkv_ctx* ctx);
  * "decode_fast_kernel" (mma.sync; the fp16 mode) or "decode_generic_kernel" (shapes the tensor-core
  * kernels do not cover).  Static string, never NULL.  Selection: DESIGN.md section 6. */
 const char* starkv_decode_kernel_name(const starkv_ctx* ctx);
+/* Name of the projection kernel the last starkv_append / starkv_append_host call of this context ran ("" before the first):
+ * "append_small_kernel" (n_new <= 16, one launch), "append_gemm_kernel" (TMA + tcgen05), "append_project_mma_kernel",
+ * "append_project_kernel" (scalar; unaligned rows). */
+const char* starkv_last_append_kernel_name(const starkv_ctx* ctx);
 
 /* Per-context options; the library reads NO environment variables.  Returns STARKV_OK,
  * STARKV_ERR_INVALID_ARG (unknown name / value) or STARKV_ERR_UNSUPPORTED (the context keeps its
@@ -230,7 +241,7 @@ const char* starkv_decode_kernel_name(const starkv_ctx* ctx);
  *   "pdl"             1 (default) launches the kernels of a step with programmatic dependent launch.
  *   "host_graph"      1 makes the HOST-buffer entry points replay a cached CUDA graph per call
  *                     signature (default 0).
- *   "append_tc5"      1 runs the prefill projection on the tcgen05 kernel (default 0). */
+ *   "append_tc5"      prefill projection (n_new >= 64): 1 = TMA + tcgen05 GEMM (default), 0 = mma.sync kernel. */
 int starkv_set_option(starkv_ctx* ctx, const char* name, int value);
 
 const char* starkv_strerror(int code);

@@ -25,7 +25,7 @@ SYMBOLS = [
     "starkv_decode_attn", "starkv_decode_step", "starkv_decode_attn_generic", "starkv_decode_attn_rope", "starkv_decode_attn_host",
     "starkv_append_host_workspace_bytes", "starkv_append_host", "starkv_set_kernel_timing",
     "starkv_last_decode_kernel_ms",
-    "starkv_set_splits", "starkv_set_option", "starkv_last_launches", "starkv_decode_kernel_name", "starkv_strerror",
+    "starkv_set_splits", "starkv_set_option", "starkv_last_launches", "starkv_decode_kernel_name", "starkv_last_append_kernel_name", "starkv_strerror",
     "starkv_last_error",
 ]
 
@@ -102,6 +102,8 @@ def _load() -> ctypes.CDLL:
     lib.starkv_set_option.restype = c_int
     lib.starkv_decode_kernel_name.argtypes = [vp]
     lib.starkv_decode_kernel_name.restype = ctypes.c_char_p
+    lib.starkv_last_append_kernel_name.argtypes = [vp]
+    lib.starkv_last_append_kernel_name.restype = ctypes.c_char_p
     lib.starkv_strerror.argtypes = [c_int]
     lib.starkv_strerror.restype = ctypes.c_char_p
     lib.starkv_last_error.argtypes = [vp]
@@ -279,6 +281,10 @@ def starkv_last_launches(ctx: Context) -> int:
 
 def starkv_decode_kernel_name(ctx: Context) -> str:
     return _lib.starkv_decode_kernel_name(ctx.handle).decode()
+
+
+def starkv_last_append_kernel_name(ctx: Context) -> str:
+    return _lib.starkv_last_append_kernel_name(ctx.handle).decode()
 
 
 def starkv_strerror(code: int) -> str:

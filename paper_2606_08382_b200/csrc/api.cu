@@ -96,6 +96,7 @@ int starkv_create(starkv_ctx** out, const starkv_desc* d, void* cuda_stream) {
     return STARKV_ERR_CUDA;
   }
   ctx->pdl = 1;
+  ctx->append_tc5 = 1;
   if (cudaMalloc((void**)&ctx->tickets, (SK_TICKETS + SK_APPEND_TICKETS) * sizeof(int)) != cudaSuccess ||
       cudaMemset(ctx->tickets, 0, (SK_TICKETS + SK_APPEND_TICKETS) * sizeof(int)) != cudaSuccess) {
     (void)cudaGetLastError();
@@ -197,10 +198,13 @@ int starkv_decode_step(starkv_ctx* ctx, void* pool, const int32_t* table, int ma
       d_in_v <= 0)
     return STARKV_ERR_INVALID_ARG;
   if (append_ws_bytes < sk_append_ws_bytes(ctx, batch)) return STARKV_ERR_WORKSPACE;
-  if (sk_decode_choice(ctx) == SK_VARIANT_TM && sk_append_small_ok(ctx, batch)) {
-    AppendSmallArgs a;
+  AppendSmallArgs a;
+  if (sk_decode_choice(ctx) == SK_VARIANT_TM && sk_append_small_ok(ctx, batch))
     sk_append_small_args(ctx, &a, pool, table, max_pages, seq_ids, positions, batch, k_new, k_row_stride, k_head_stride, d_in_k,
                          v_new, v_row_stride, d_in_v, A_k, A_v, append_ws);
+  else
+    a.n_part = 0;
+  if (a.n_part > 0 && sk_append_small_fused(ctx, batch, a.n_part, 8192)) {
     return sk_decode_tm(ctx, q, pool, table, max_pages, seq_lens, batch, B_k, B_v, ws, ws_bytes, out, &a);
   }
   rc = sk_append(ctx, pool, table, max_pages, seq_ids, positions, batch, k_new, k_row_stride, k_head_stride, d_in_k, v_new,
@@ -456,6 +460,8 @@ int starkv_set_splits(starkv_ctx* ctx, int n_splits) {
 }
 
 int starkv_last_launches(const starkv_ctx* ctx) { return ctx ? ctx->last_launches : 0; }
+
+const char* starkv_last_append_kernel_name(const starkv_ctx* ctx) { return ctx && ctx->last_append ? ctx->last_append : ""; }
 
 const char* starkv_decode_kernel_name(const starkv_ctx* ctx) {
   if (!ctx) return "decode_generic_kernel";

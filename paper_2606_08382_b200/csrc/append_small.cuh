@@ -21,6 +21,7 @@ constexpr int APS_ZR_MAX = APS_SM_FLOATS * 2;                                // 
 
 struct AppendSmallArgs {
   int n_new, n_key_tiles, n_tiles, n_part;
+  int x_vec;      // both inputs: 16-byte aligned rows and d_in % 8 == 0
   const __half* k_new;
   long long k_row_stride, k_head_stride;
   int d_in_k;
@@ -50,6 +51,9 @@ __device__ __forceinline__ uint8_t* aps_page_of(const StarkvLayout& L, const App
 }
 
 // bx = column tile (keys of head 0.., then values), by = K split.  `sm` = APS_SM_FLOATS floats of shared memory.
+// FUSED = false stops after the partial sums (A1 only): a large group (many tokens x wide value rank x many K splits)
+// is too much serial work for one last-arriving CTA, so append_write_kernel, one CTA per token, does A2-A4 instead.
+template <bool FUSED>
 __device__ __forceinline__ void append_small_body(const StarkvLayout& L, const AppendSmallArgs& a, int bx, int by, float* sm) {
   __shared__ int s_last;
   __shared__ float s_vsc[APS_TOK][2];
@@ -90,9 +94,28 @@ __device__ __forceinline__ void append_small_body(const StarkvLayout& L, const A
       for (int kk = 0; kk < 32; ++kk) av[kk] = kk < kn ? *reinterpret_cast<const uint32_t*>(ap + (size_t)kk * lda) : 0u;
     }
     __syncthreads();
-    for (int i = tid; i < APS_TOK * APS_KCH; i += APS_THREADS) {
-      const int t = i / APS_KCH, k = i % APS_KCH;
-      sm[i] = (t < n_new && kc + k < k_end) ? __half2float(x0[(long long)t * xstride + kc + k]) : 0.f;
+    if (a.x_vec) {   // 16-byte aligned rows, d_in a multiple of 8: two independent 16-byte loads per thread
+      uint4 xv[2];
+#pragma unroll
+      for (int u = 0; u < 2; ++u) {
+        const int i = tid + u * APS_THREADS, t = i >> 5, k8 = (i & 31) * 8;
+        xv[u] = (t < n_new && kc + k8 < k_end) ? *reinterpret_cast<const uint4*>(x0 + (long long)t * xstride + kc + k8)
+                                               : make_uint4(0u, 0u, 0u, 0u);
+      }
+#pragma unroll
+      for (int u = 0; u < 2; ++u) {
+        const int i = tid + u * APS_THREADS, t = i >> 5, k8 = (i & 31) * 8;
+        const float2 f0 = __half22float2(*reinterpret_cast<const __half2*>(&xv[u].x)), f1 = __half22float2(*reinterpret_cast<const __half2*>(&xv[u].y)),
+                     f2 = __half22float2(*reinterpret_cast<const __half2*>(&xv[u].z)), f3 = __half22float2(*reinterpret_cast<const __half2*>(&xv[u].w));
+        float4* d = reinterpret_cast<float4*>(sm + t * APS_KCH + k8);
+        d[0] = make_float4(f0.x, f0.y, f1.x, f1.y);
+        d[1] = make_float4(f2.x, f2.y, f3.x, f3.y);
+      }
+    } else {
+      for (int i = tid; i < APS_TOK * APS_KCH; i += APS_THREADS) {
+        const int t = i / APS_KCH, k = i % APS_KCH;
+        sm[i] = (t < n_new && kc + k < k_end) ? __half2float(x0[(long long)t * xstride + kc + k]) : 0.f;
+      }
     }
     __syncthreads();
     if (kn > 0) {
@@ -122,6 +145,7 @@ __device__ __forceinline__ void append_small_body(const StarkvLayout& L, const A
     if (t < n_new && c < ncols) a.zp[((size_t)by * n_new + t) * R + col_out0 + c] = s;
   }
 
+  if (!FUSED) return;
   // ---- ticket: the last CTA of the group quantises and writes the group's fields
   __threadfence();
   __syncthreads();
@@ -143,8 +167,12 @@ __device__ __forceinline__ void append_small_body(const StarkvLayout& L, const A
   __half* zr = reinterpret_cast<__half*>(sm);   // [token][gcols]
   for (int i = tid; i < n_new * gcols; i += APS_THREADS) {
     const int j = i / gcols, c = i - j * gcols;
+    float v[APS_KS_MAX];   // all K splits in flight at once, then added in order
+#pragma unroll
+    for (int p = 0; p < APS_KS_MAX; ++p) v[p] = p < a.n_part ? __ldcg(a.zp + ((size_t)p * n_new + j) * R + gcol0 + c) : 0.f;
     float s = 0.f;
-    for (int p = 0; p < a.n_part; ++p) s += __ldcg(a.zp + ((size_t)p * n_new + j) * R + gcol0 + c);
+#pragma unroll
+    for (int p = 0; p < APS_KS_MAX; ++p) s += v[p];
     zr[i] = __float2half_rn(s);
   }
   __syncthreads();

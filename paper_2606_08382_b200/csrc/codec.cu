@@ -254,11 +254,12 @@ __global__ void __launch_bounds__(128) append_project_kernel(
 // append for a handful of new tokens (decode-time append, n_new <= 16): projection, quantiser and paged write in one
 // launch (append_small.cuh).  grid (column tiles of keys then values, K splits), 256 threads.
 // ---------------------------------------------------------------------------------------------
+template <bool FUSED>
 __global__ void __launch_bounds__(APS_THREADS) append_small_kernel(const __grid_constant__ StarkvLayout L,
                                                                   const __grid_constant__ AppendSmallArgs a) {
   __shared__ __align__(16) float sm[APS_SM_FLOATS];
   sk_pdl_enter();
-  append_small_body(L, a, blockIdx.x, blockIdx.y, sm);
+  append_small_body<FUSED>(L, a, blockIdx.x, blockIdx.y, sm);
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -400,302 +401,161 @@ __global__ void __launch_bounds__(128) append_project_mma_kernel(
 }
 
 // ---------------------------------------------------------------------------------------------
-// append, step A1 for many new tokens on the 5th-generation tensor cores: z = fp16(X . A) with tcgen05.mma
-// (cta_group::1, kind::f16, M = 128 tokens, N = 64 latent columns, K = 16 per instruction), fp32 accumulator in
-// TMEM, read back with tcgen05.ld for the fp16 epilogue.  Operands are staged by cp.async straight into the
-// no-swizzle canonical layouts (8 x 16-byte core matrices): X tile K-major, A tile MN-major (A is [d_in, cols]
-// row-major, i.e. N-contiguous), 4 stages of 128 k, prefetch distance 3, one elected thread issues the MMAs and
-// tcgen05.commit releases a stage through an mbarrier.  grid (column tiles of keys then values, token tiles).
+// append, steps A2-A4 for n > 16 new tokens: per-token scales, codes, pack, paged write.  One CTA per new token.
+// Keys (token-major rows): one warp per (head, precision block), lanes over channels.
+// Values are channel-major, so a byte (4-bit) or 8 bytes (8-bit) of a channel row hold neighbouring SLOTS.  When the
+// token belongs to an aligned slot octet of its page whose 8 tokens are consecutive entries of this call (a prefill
+// chunk in position order: the common case), the octet's FIRST token's CTA does the values of all eight: it loads their
+// value latents, takes the 16 scales, and one thread per channel assembles and stores the channel's whole word; the
+// other seven CTAs skip the values.  Any other token sets its 4-bit fields with atomicAnd/atomicOr on the containing
+// word so that concurrent appends to neighbouring slots cannot lose an update.
 // ---------------------------------------------------------------------------------------------
-constexpr int TM = 128, TN = 64, TK = 128, TSTAGES = 4;   // 48 KB per stage, prefetch distance 3
-constexpr int TA_BYTES = TM * TK * 2, TB_BYTES = TK * TN * 2, TSTAGE_BYTES = TA_BYTES + TB_BYTES;
-constexpr int TC5_SMEM = TSTAGES * TSTAGE_BYTES + 128;
+constexpr int AW_THREADS = 512;
 
-__device__ __forceinline__ uint64_t umma_desc(uint32_t saddr, uint32_t lbo_bytes, uint32_t sbo_bytes) {
-  // SWIZZLE_NONE matrix descriptor: start >> 4 | LBO >> 4 << 16 | SBO >> 4 << 32 | version 1 << 46
-  return (uint64_t)((saddr & 0x3FFFF) >> 4) | ((uint64_t)(lbo_bytes >> 4) << 16) | ((uint64_t)(sbo_bytes >> 4) << 32) |
-         ((uint64_t)1 << 46);
-}
-__device__ __forceinline__ void mbar_init_s(uint32_t bar, uint32_t count) {
-  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count) : "memory");
-}
-__device__ __forceinline__ void mbar_wait_s(uint32_t bar, uint32_t parity) {
-  asm volatile(
-      "{\n\t.reg .pred p;\n\t"
-      "WAIT_%=:\n\t"
-      "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n\t"
-      "@p bra DONE_%=;\n\t"
-      "bra WAIT_%=;\n\t"
-      "DONE_%=:\n\t}" ::"r"(bar),
-      "r"(parity)
-      : "memory");
-}
-
-__global__ void __launch_bounds__(256) append_project_tc5_kernel(
-    const __grid_constant__ StarkvLayout L, int n_new, int n_key_tiles, const __half* __restrict__ k_new,
-    long long k_row_stride, long long k_head_stride, int d_in_k, const __half* __restrict__ v_new, long long v_row_stride,
-    int d_in_v, const __half* __restrict__ A_k, const __half* __restrict__ A_v, __half* __restrict__ z) {
-  extern __shared__ __align__(128) uint8_t tsm[];
-  __shared__ uint32_t tmem_base_s;
-  const int R = L.sum_rank_k + L.rank_v;
-  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-  const __half* x0;
-  long long xstride;
-  int d_in, ncols, col_out0, lda;
-  const __half* A;
-  if ((int)blockIdx.x < n_key_tiles) {
-    int h = 0, t = blockIdx.x;
-    while (t >= (L.rank_k[h] + TN - 1) / TN) { t -= (L.rank_k[h] + TN - 1) / TN; ++h; }
-    const int c0 = t * TN;
-    x0 = k_new + (long long)h * k_head_stride; xstride = k_row_stride; d_in = d_in_k;
-    ncols = min(TN, L.rank_k[h] - c0); col_out0 = L.koff[h] + c0; A = A_k + L.koff[h] + c0; lda = L.sum_rank_k;
-  } else {
-    const int c0 = (blockIdx.x - n_key_tiles) * TN;
-    x0 = v_new; xstride = v_row_stride; d_in = d_in_v;
-    ncols = min(TN, L.rank_v - c0); col_out0 = L.sum_rank_k + c0; A = A_v + c0; lda = L.rank_v;
-  }
-  const int m0 = blockIdx.y * TM;
-  const uint32_t sbase = (uint32_t)__cvta_generic_to_shared(tsm);
-  const uint32_t bar0 = sbase + TSTAGES * TSTAGE_BYTES;   // empty[TSTAGES], then accumulator-ready
-  const uint32_t accbar = bar0 + 8 * TSTAGES;
-  if (tid == 0) {
-    for (int s = 0; s < TSTAGES; ++s) mbar_init_s(bar0 + 8 * s, 1);
-    mbar_init_s(accbar, 1);
-    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-  }
-  if (warp == 0) {   // TMEM: 64 fp32 columns x 128 lanes for the accumulator
-    const uint32_t dst = (uint32_t)__cvta_generic_to_shared(&tmem_base_s);
-    asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(dst), "n"(TN) : "memory");
-    asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
-  }
-  asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
-  __syncthreads();
-  asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
-  const uint32_t tmem_d = tmem_base_s;
-
-  // cp.async staging into the canonical layouts.  Lane = (row-in-core-matrix, 16-byte chunk): 8 rows x 4 chunks per
-  // warp instruction (conflict-free shared-memory writes, 64 contiguous bytes per global row).  Per-thread source
-  // pointers, shared-memory offsets and row predicates are fixed for the whole K loop.
-  //   X tile, K-major : element (m, k) at (m >> 3) * 2048 + (k >> 3) * 128 + (m & 7) * 16 + (k & 7) * 2
-  //   A tile, MN-major: element (k, n) at (n >> 3) * 2048 + (k >> 3) * 128 + (k & 7) * 16 + (n & 7) * 2
-  const int l7 = lane & 7, l3 = lane >> 3;
-  const __half* xsrc[4];      // rows warp*16 + {0, 8} ... : 8 chunks per thread = 2 row groups x 4 chunk groups
-  bool xok[2];
-  uint32_t xdst[2];
-#pragma unroll
-  for (int rg = 0; rg < 2; ++rg) {
-    const int m = warp * 16 + rg * 8 + l7;
-    xok[rg] = m0 + m < n_new;
-    xsrc[rg] = x0 + (long long)(xok[rg] ? m0 + m : 0) * xstride + l3 * 8;
-    xdst[rg] = (uint32_t)((m >> 3) * 2048 + l3 * 128 + (m & 7) * 16);
-  }
-  const int ak = warp * 16 + l7;               // k rows warp*16 + {0, 8}; 4 chunks per thread = 2 k groups x 2 n groups
-  const __half* asrc = A + (size_t)ak * lda + l3 * 8;
-  const uint32_t adst = (uint32_t)(l3 * 2048 + (ak >> 3) * 128 + (ak & 7) * 16);
-  const bool aok0 = l3 * 8 < ncols, aok1 = (l3 + 4) * 8 < ncols;
-  auto load_stage = [&](int stage, int k0) {
-    const uint32_t sa = sbase + stage * TSTAGE_BYTES, sb = sa + TA_BYTES;
-    const int krem = d_in - k0;   // > 0
-#pragma unroll
-    for (int rg = 0; rg < 2; ++rg)
-#pragma unroll
-      for (int cg = 0; cg < 4; ++cg) {
-        const bool ok = xok[rg] && (cg * 32 + l3 * 8) < krem;
-        cp_async16_s(sa + xdst[rg] + cg * 512, ok ? xsrc[rg] + k0 + cg * 32 : x0, ok);
-      }
-#pragma unroll
-    for (int kg = 0; kg < 2; ++kg) {
-      const bool kok = ak + kg * 8 < krem;
-      const __half* src = asrc + (size_t)(k0 + kg * 8) * lda;
-      cp_async16_s(sb + adst + kg * 128, (kok && aok0) ? src : A, kok && aok0);
-      cp_async16_s(sb + adst + kg * 128 + 4 * 2048, (kok && aok1) ? src + 32 : A, kok && aok1);
-    }
-  };
-  // instruction descriptor: D fp32, A/B fp16, A K-major, B MN-major, N = 64, M = 128
-  constexpr uint32_t IDESC = (1u << 4) | (1u << 16) | ((uint32_t)(TN >> 3) << 17) | ((uint32_t)(TM >> 4) << 24);
-  const int nk = (d_in + TK - 1) / TK;
-  load_stage(0, 0);
-  asm volatile("cp.async.commit_group;" ::: "memory");
-  if (nk > 1) load_stage(1, TK);
-  asm volatile("cp.async.commit_group;" ::: "memory");
-  if (nk > 2) load_stage(2, 2 * TK);
-  asm volatile("cp.async.commit_group;" ::: "memory");
-  for (int kt = 0; kt < nk; ++kt) {
-    if (kt + 3 < nk) {
-      const int st = (kt + 3) % TSTAGES;
-      if (kt >= 1) mbar_wait_s(bar0 + 8 * st, (uint32_t)(((kt - 1) / TSTAGES) & 1));   // MMA(kt - 1) has read the stage
-      load_stage(st, (kt + 3) * TK);
-    }
-    asm volatile("cp.async.commit_group;" ::: "memory");
-    asm volatile("cp.async.wait_group 3;" ::: "memory");
-    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");   // cp.async writes -> visible to the tensor core proxy
-    __syncthreads();
-    if (tid == 0) {
-      asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
-      const uint32_t sa = sbase + (kt % TSTAGES) * TSTAGE_BYTES, sb = sa + TA_BYTES;
-#pragma unroll
-      for (int k = 0; k < TK / 16; ++k) {
-        const uint64_t da = umma_desc(sa + k * 256, 128, 2048);
-        const uint64_t db = umma_desc(sb + k * 256, 128, 2048);
-        const uint32_t accum = (kt > 0 || k > 0) ? 1u : 0u;
-        asm volatile(
-            "{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\t"
-            "tcgen05.mma.cta_group::1.kind::f16 [%0], %1, %2, %3, p;\n\t}" ::"r"(tmem_d),
-            "l"(da), "l"(db), "r"(IDESC), "r"(accum)
-            : "memory");
-      }
-      asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(bar0 + 8 * (kt % TSTAGES))
-                   : "memory");
-      if (kt == nk - 1)
-        asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(accbar) : "memory");
-    }
-  }
-  // epilogue: warp w may read TMEM lanes (= token rows) [32 (w % 4), +32); warps 0-3 take columns 0-31, warps 4-7
-  // columns 32-63; one rounding to fp16
-  mbar_wait_s(accbar, 0);
-  asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
-  const int row = m0 + (warp & 3) * 32 + lane;
-  {
-    const int cb = (warp >> 2) * 32;
-    uint32_t v[32];
-    const uint32_t taddr = tmem_d + ((uint32_t)((warp & 3) * 32) << 16) + cb;
-    asm volatile(
-        "tcgen05.ld.sync.aligned.32x32b.x32.b32 {%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15,%16,%17,%18,%19,%20,%21,"
-        "%22,%23,%24,%25,%26,%27,%28,%29,%30,%31}, [%32];"
-        : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7]), "=r"(v[8]), "=r"(v[9]),
-          "=r"(v[10]), "=r"(v[11]), "=r"(v[12]), "=r"(v[13]), "=r"(v[14]), "=r"(v[15]), "=r"(v[16]), "=r"(v[17]), "=r"(v[18]),
-          "=r"(v[19]), "=r"(v[20]), "=r"(v[21]), "=r"(v[22]), "=r"(v[23]), "=r"(v[24]), "=r"(v[25]), "=r"(v[26]), "=r"(v[27]),
-          "=r"(v[28]), "=r"(v[29]), "=r"(v[30]), "=r"(v[31])
-        : "r"(taddr));
-    asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
-    if (row < n_new) {
-      __half* dst = z + (size_t)row * R + col_out0 + cb;
-#pragma unroll
-      for (int c = 0; c < 32; c += 8) {
-        if (cb + c < ncols) {   // ncols is a multiple of 8
-          uint4 o;
-          o.x = pack_f2h2(__uint_as_float(v[c + 0]), __uint_as_float(v[c + 1]));
-          o.y = pack_f2h2(__uint_as_float(v[c + 2]), __uint_as_float(v[c + 3]));
-          o.z = pack_f2h2(__uint_as_float(v[c + 4]), __uint_as_float(v[c + 5]));
-          o.w = pack_f2h2(__uint_as_float(v[c + 6]), __uint_as_float(v[c + 7]));
-          *reinterpret_cast<uint4*>(dst + c) = o;
-        }
-      }
-    }
-  }
-  asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
-  __syncthreads();
-  if (warp == 0) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem_d), "n"(TN) : "memory");
-}
-
-// ---------------------------------------------------------------------------------------------
-// append, steps A2-A4: per-token scales, codes, pack, paged write.  One CTA per new token.
-// 4-bit value fields share a byte between two slots: set with atomicAnd/atomicOr on the
-// containing word so that concurrent appends to neighbouring slots cannot lose an update.
-// ---------------------------------------------------------------------------------------------
-// z16 (fp16 latents) or, when zp != nullptr, n_part fp32 partial sums zp[part][token][column] added in order.
-__global__ void __launch_bounds__(512) append_write_kernel(const __grid_constant__ StarkvLayout L,
-                                                           const __half* __restrict__ z, const float* __restrict__ zp,
-                                                           int n_part, int n_new,
-                                                           const int32_t* __restrict__ seq_ids,
-                                                           const int32_t* __restrict__ positions,
-                                                           const int32_t* __restrict__ table, int max_pages,
-                                                           uint8_t* __restrict__ pool) {
+__global__ void __launch_bounds__(AW_THREADS) append_write_kernel(const __grid_constant__ StarkvLayout L,
+                                                                  const __half* __restrict__ z, const float* __restrict__ zp,
+                                                                  int n_part, int n_new, const int32_t* __restrict__ seq_ids,
+                                                                  const int32_t* __restrict__ positions,
+                                                                  const int32_t* __restrict__ table, int max_pages,
+                                                                  uint8_t* __restrict__ pool) {
   extern __shared__ __align__(16) uint8_t sm[];
-  __half* zr = reinterpret_cast<__half*>(sm);
-  __shared__ float vsc[2];
+  __half* zr = reinterpret_cast<__half*>(sm);                                    // [R] this token's latents
+  __half* zo = zr + ((L.sum_rank_k + L.rank_v + 7) & ~7);                         // [8][rank_v] the octet's value latents
+  __shared__ float vsc[8][2];
+  __shared__ int s_oct;   // 0 = no octet (per-field path), 1 = octet leader, 2 = octet member (the leader writes the values)
   sk_pdl_enter();
   const int j = blockIdx.x;
   const int P = L.page_tokens;
   const int R = L.sum_rank_k + L.rank_v;
   const bool quant = L.bits_hi != 16;
-  const int pos = positions[j];
-  if (pos < 0 || pos / P >= max_pages || seq_ids[j] < 0) return;   // caller error: skip the token rather than write wildly
-  const int pidx = table[(size_t)seq_ids[j] * max_pages + pos / P];
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const int pos = positions[j], sid = seq_ids[j];
+  if (pos < 0 || pos / P >= max_pages || sid < 0) return;   // caller error: skip the token rather than write wildly
+  const int pidx = table[(size_t)sid * max_pages + pos / P];
   if (pidx < 0) return;
   uint8_t* pg = pool + (size_t)pidx * L.page_bytes;
   const int slot = pos % P;
-  if (zp) {
-    for (int i = threadIdx.x; i < R; i += blockDim.x) {
-      float a = 0.f;
-      for (int p = 0; p < n_part; ++p) a += zp[((size_t)p * n_new + j) * R + i];
-      zr[i] = __float2half_rn(a);
+  const int jb = j - (slot & 7);   // call index of the octet's first token, if the octet is in this call in order
+  if (tid == 0) s_oct = 0;
+  __syncthreads();
+  if (!zp && jb >= 0 && jb + 8 <= n_new) {
+    if (tid < 8) {
+      const bool ok = seq_ids[jb + tid] == sid && positions[jb + tid] == pos - (slot & 7) + tid;
+      const unsigned all = __ballot_sync(0xffu, ok);
+      if (tid == 0 && all == 0xffu) s_oct = (slot & 7) == 0 ? 1 : 2;
+    }
+  }
+  if (zp) {   // fp32 partial sums zp[part][token][column] of append_small_kernel<false>, added in order, one rounding
+    for (int i = tid; i < R; i += AW_THREADS) {
+      float v[APS_KS_MAX];   // all K splits in flight at once, then added in order
+#pragma unroll
+      for (int p = 0; p < APS_KS_MAX; ++p) v[p] = p < n_part ? __ldcg(zp + ((size_t)p * n_new + j) * R + i) : 0.f;
+      float acc = 0.f;
+#pragma unroll
+      for (int p = 0; p < APS_KS_MAX; ++p) acc += v[p];
+      zr[i] = __float2half_rn(acc);
     }
   } else {
-    for (int i = threadIdx.x; i < R; i += blockDim.x) zr[i] = z[(size_t)j * R + i];
+    for (int i = tid; i < R / 8; i += AW_THREADS) reinterpret_cast<uint4*>(zr)[i] = reinterpret_cast<const uint4*>(z + (size_t)j * R)[i];
   }
   __syncthreads();
+  const int oct = s_oct;
+  if (oct == 1) {
+    const int v8 = L.rank_v / 8;
+    for (int i = tid; i < 8 * v8; i += AW_THREADS)
+      reinterpret_cast<uint4*>(zo)[i] = reinterpret_cast<const uint4*>(z + (size_t)(jb + i / v8) * R + L.sum_rank_k)[i % v8];
+  }
 
   // keys: one warp per (head, precision block), lanes over channels
-  {
-    const int lane = threadIdx.x & 31, nw = blockDim.x >> 5;
-    for (int u = threadIdx.x >> 5; u < L.n_kv_heads * 2; u += nw) {
-      const int h = u >> 1, blk = u & 1;
-      const int n = blk ? L.k_lo_n[h] : L.k_hi_n[h];
-      if (!quant) {
-        if (blk) continue;
-        __half* row = reinterpret_cast<__half*>(pg + L.k_hi_off[h]) + (size_t)slot * n;
-        for (int c = lane; c < n; c += 32) row[c] = zr[L.koff[h] + c];
-        continue;
-      }
-      uint16_t* sc = reinterpret_cast<uint16_t*>(pg + L.k_scale_off) + (h * 2 + blk) * P + slot;
-      if (n == 0) {
-        if (lane == 0) *sc = 0;
-        continue;
-      }
-      const __half* zz = zr + L.koff[h] + (blk ? L.k_hi_n[h] : 0);
-      const int bits = blk ? L.bits_lo : L.bits_hi;
-      const int qmax = sk_qmax(bits);
-      float amax = 0.f;
-      for (int c = lane; c < n; c += 32) amax = fmaxf(amax, fabsf(__half2float(zz[c])));
+  for (int u = warp; u < L.n_kv_heads * 2; u += AW_THREADS / 32) {
+    const int h = u >> 1, blk = u & 1;
+    const int n = blk ? L.k_lo_n[h] : L.k_hi_n[h];
+    if (!quant) {
+      if (blk) continue;
+      __half* row = reinterpret_cast<__half*>(pg + L.k_hi_off[h]) + (size_t)slot * n;
+      for (int c = lane; c < n; c += 32) row[c] = zr[L.koff[h] + c];
+      continue;
+    }
+    uint16_t* sc = reinterpret_cast<uint16_t*>(pg + L.k_scale_off) + (h * 2 + blk) * P + slot;
+    if (n == 0) {
+      if (lane == 0) *sc = 0;
+      continue;
+    }
+    const __half* zz = zr + L.koff[h] + (blk ? L.k_hi_n[h] : 0);
+    const int bits = blk ? L.bits_lo : L.bits_hi;
+    const int qmax = sk_qmax(bits);
+    float amax = 0.f;
+    for (int c = lane; c < n; c += 32) amax = fmaxf(amax, fabsf(__half2float(zz[c])));
 #pragma unroll
-      for (int o = 16; o; o >>= 1) amax = fmaxf(amax, __shfl_xor_sync(0xffffffffu, amax, o));
-      const __half s16 = sk_scale_of(amax, qmax);
-      const float sf = __half2float(s16);
-      if (lane == 0) *sc = sk_half_bits(s16);
-      uint8_t* row = pg + (blk ? L.k_lo_off[h] : L.k_hi_off[h]) + (size_t)slot * (n * bits / 8);
-      if (bits == 8) {
-        for (int c = lane; c < n; c += 32) row[c] = (uint8_t)(sk_code_of(__half2float(zz[c]), sf, qmax) + 128);
-      } else {
-        for (int c = lane; c < n / 2; c += 32) {
-          const int u0 = sk_code_of(__half2float(zz[2 * c]), sf, qmax) + 8;
-          const int u1 = sk_code_of(__half2float(zz[2 * c + 1]), sf, qmax) + 8;
-          row[c] = (uint8_t)(u0 | (u1 << 4));
-        }
+    for (int o = 16; o; o >>= 1) amax = fmaxf(amax, __shfl_xor_sync(0xffffffffu, amax, o));
+    const __half s16 = sk_scale_of(amax, qmax);
+    const float sf = __half2float(s16);
+    if (lane == 0) *sc = sk_half_bits(s16);
+    uint8_t* row = pg + (blk ? L.k_lo_off[h] : L.k_hi_off[h]) + (size_t)slot * (n * bits / 8);
+    if (bits == 8) {
+      for (int c = lane; c < n; c += 32) row[c] = (uint8_t)(sk_code_of(__half2float(zz[c]), sf, qmax) + 128);
+    } else {
+      for (int c = lane; c < n / 2; c += 32) {
+        const int u0 = sk_code_of(__half2float(zz[2 * c]), sf, qmax) + 8;
+        const int u1 = sk_code_of(__half2float(zz[2 * c + 1]), sf, qmax) + 8;
+        row[c] = (uint8_t)(u0 | (u1 << 4));
       }
     }
   }
+  if (oct == 2) return;   // (CTA-uniform) the octet's first token writes this token's values
+  __syncthreads();        // zo is complete
 
-  const __half* zv = zr + L.sum_rank_k;
+  // values: scales of the token (or of the octet's eight tokens), then the channel-major fields
+  const int n_tok = oct == 1 ? 8 : 1;
+  const __half* zv0 = oct == 1 ? zo : zr + L.sum_rank_k;   // token t's value latents at zv0 + t * rank_v
   if (quant) {
-    // two warps: one per precision block, shuffle-reduce the absmax
-    const int w = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    if (w < 2) {
+    for (int u = warp; u < n_tok * 2; u += AW_THREADS / 32) {
+      const int t = u >> 1, w = u & 1;
       const int n = w ? L.v_lo_n : L.v_hi_n;
-      const int c0 = w ? L.v_hi_n : 0;
+      const __half* zv = zv0 + (size_t)t * L.rank_v + (w ? L.v_hi_n : 0);
       float amax = 0.f;
-      for (int c = lane; c < n; c += 32) amax = fmaxf(amax, fabsf(__half2float(zv[c0 + c])));
+      for (int c = lane; c < n; c += 32) amax = fmaxf(amax, fabsf(__half2float(zv[c])));
 #pragma unroll
       for (int o = 16; o; o >>= 1) amax = fmaxf(amax, __shfl_xor_sync(0xffffffffu, amax, o));
       if (lane == 0) {
         const __half s16 = n ? sk_scale_of(amax, sk_qmax(w ? L.bits_lo : L.bits_hi)) : __float2half(0.f);
-        reinterpret_cast<uint16_t*>(pg + L.v_scale_off)[w * P + slot] = sk_half_bits(s16);
-        vsc[w] = __half2float(s16);
+        vsc[t][w] = __half2float(s16);
+        reinterpret_cast<uint16_t*>(pg + L.v_scale_off)[w * P + slot + t] = sk_half_bits(s16);
       }
     }
     __syncthreads();
   }
-  for (int c = threadIdx.x; c < L.rank_v; c += blockDim.x) {
+  for (int c = tid; c < L.rank_v; c += AW_THREADS) {
     const int blk = (quant && c >= L.v_hi_n) ? 1 : 0;
     const int idx = blk ? c - L.v_hi_n : c;
     const int bits = blk ? L.bits_lo : L.bits_hi;
     uint8_t* base = pg + (blk ? L.v_lo_off : L.v_hi_off);
-    if (bits == 16) {
-      reinterpret_cast<__half*>(base)[(size_t)idx * P + slot] = zv[c];
+    const __half* zc = zv0 + c;
+    if (oct == 1) {   // slots [slot, slot + 8) of the channel row at once
+      if (bits == 16) {
+        uint32_t w[4];
+#pragma unroll
+        for (int t = 0; t < 8; t += 2)
+          w[t >> 1] = (uint32_t)__half_as_ushort(zc[(size_t)t * L.rank_v]) | ((uint32_t)__half_as_ushort(zc[(size_t)(t + 1) * L.rank_v]) << 16);
+        *reinterpret_cast<uint4*>(base + ((size_t)idx * P + slot) * 2) = make_uint4(w[0], w[1], w[2], w[3]);
+      } else if (bits == 8) {
+        uint32_t w[2] = {0u, 0u};
+#pragma unroll
+        for (int t = 0; t < 8; ++t)
+          w[t >> 2] |= (uint32_t)(sk_code_of(__half2float(zc[(size_t)t * L.rank_v]), vsc[t][blk], 127) + 128) << (8 * (t & 3));
+        *reinterpret_cast<uint2*>(base + (size_t)idx * P + slot) = make_uint2(w[0], w[1]);
+      } else {
+        uint32_t w = 0u;
+#pragma unroll
+        for (int t = 0; t < 8; ++t) w |= (uint32_t)(sk_code_of(__half2float(zc[(size_t)t * L.rank_v]), vsc[t][blk], 7) + 8) << (4 * t);
+        *reinterpret_cast<uint32_t*>(base + (size_t)idx * (P / 2) + (slot >> 1)) = w;
+      }
+    } else if (bits == 16) {
+      reinterpret_cast<__half*>(base)[(size_t)idx * P + slot] = zc[0];
     } else if (bits == 8) {
-      base[(size_t)idx * P + slot] = (uint8_t)(sk_code_of(__half2float(zv[c]), vsc[blk], 127) + 128);
+      base[(size_t)idx * P + slot] = (uint8_t)(sk_code_of(__half2float(zc[0]), vsc[0][blk], 127) + 128);
     } else {
-      const unsigned u = (unsigned)(sk_code_of(__half2float(zv[c]), vsc[blk], 7) + 8);
+      const unsigned u = (unsigned)(sk_code_of(__half2float(zc[0]), vsc[0][blk], 7) + 8);
       const size_t byte = (size_t)idx * (P / 2) + (slot >> 1);
       unsigned* word = reinterpret_cast<unsigned*>(base + (byte & ~(size_t)3));
       const int sh = 8 * (int)(byte & 3) + 4 * (slot & 1);
@@ -760,14 +620,27 @@ void sk_append_small_args(const starkv_ctx* ctx, AppendSmallArgs* a, void* pool,
   int nkt = 0;
   for (int h = 0; h < L.n_kv_heads; ++h) nkt += (L.rank_k[h] + APS_COLS - 1) / APS_COLS;
   const int d_max = d_in_k > d_in_v ? d_in_k : d_in_v;
+  const int n_tiles = nkt + (L.rank_v + APS_COLS - 1) / APS_COLS;
   int n_part = (d_max + APS_KCH - 1) / APS_KCH;
   if (n_part > APS_KS_MAX) n_part = APS_KS_MAX;
-  a->n_new = n_new; a->n_key_tiles = nkt; a->n_tiles = nkt + (L.rank_v + APS_COLS - 1) / APS_COLS; a->n_part = n_part;
+  a->n_new = n_new; a->n_key_tiles = nkt; a->n_tiles = n_tiles; a->n_part = n_part;
   a->k_new = (const __half*)k_new; a->k_row_stride = k_row_stride; a->k_head_stride = k_head_stride; a->d_in_k = d_in_k;
   a->v_new = (const __half*)v_new; a->v_row_stride = v_row_stride; a->d_in_v = d_in_v;
   a->A_k = (const __half*)A_k; a->A_v = (const __half*)A_v; a->zp = (float*)ws;
   a->seq_ids = seq_ids; a->positions = positions; a->table = table; a->max_pages = max_pages; a->pool = (uint8_t*)pool;
   a->tickets = ctx->tickets + SK_TICKETS;
+  a->x_vec = (((uintptr_t)k_new | (uintptr_t)v_new) & 15) == 0 && ((k_row_stride | k_head_stride | v_row_stride) & 7) == 0 &&
+             ((d_in_k | d_in_v) & 7) == 0;
+}
+
+// One launch for A1-A4 when the serial tail of a group's last CTA stays small: at most `limit` partial sums to add.
+// Measured: against A1 + append_write_kernel the single launch loses above ~2K sums (C2: 54.6 vs 52.3 us per step), but
+// inside starkv_decode_step, where it also shares its launch with the query image, it wins up to 8K (C5: 62.2 vs 66.3).
+int sk_append_small_fused(const starkv_ctx* ctx, int n_new, int n_part, int limit) {
+  const StarkvLayout& L = ctx->L;
+  int widest = L.rank_v;
+  for (int h = 0; h < L.n_kv_heads; ++h) widest = L.rank_k[h] > widest ? L.rank_k[h] : widest;
+  return (long long)n_new * widest * n_part <= limit;
 }
 
 int sk_append(starkv_ctx* ctx, void* pool, const int32_t* table, int max_pages, const int32_t* seq_ids,
@@ -781,51 +654,59 @@ int sk_append(starkv_ctx* ctx, void* pool, const int32_t* table, int max_pages, 
   if (!pool || !table || !seq_ids || !positions || !k_new || !v_new || !A_k || !A_v || !ws) return STARKV_ERR_INVALID_ARG;
   if (ws_bytes < sk_append_ws_bytes(ctx, n_new)) return STARKV_ERR_WORKSPACE;
   __half* z = (__half*)ws;
+  const size_t smem = ((size_t)((L.sum_rank_k + L.rank_v + 7) & ~7) + 8 * (size_t)L.rank_v) * 2;   // of append_write_kernel
+  if (!sk_append_small_ok(ctx, n_new) && (int)smem > ctx->smem_optin) return STARKV_ERR_UNSUPPORTED;
+  const float* zp = nullptr;
+  int n_part = 1;
   if (sk_append_small_ok(ctx, n_new)) {
     AppendSmallArgs a;
     sk_append_small_args(ctx, &a, pool, table, max_pages, seq_ids, positions, n_new, k_new, k_row_stride, k_head_stride, d_in_k,
                          v_new, v_row_stride, d_in_v, A_k, A_v, ws);
-    SK_PREFER_SMEM(ctx, append_small_kernel);
-    SK_CUDA_CHECK(ctx, sk_launch(ctx, append_small_kernel, dim3(a.n_tiles, a.n_part), dim3(APS_THREADS), 0, L, a));
-    ctx->last_launches = 1;
-    return STARKV_OK;
+    ctx->last_append = "append_small_kernel";
+    if (sk_append_small_fused(ctx, n_new, a.n_part, 2048)) {
+      SK_PREFER_SMEM(ctx, append_small_kernel<true>);
+      SK_CUDA_CHECK(ctx, sk_launch(ctx, append_small_kernel<true>, dim3(a.n_tiles, a.n_part), dim3(APS_THREADS), 0, L, a));
+      ctx->last_launches = 1;
+      return STARKV_OK;
+    }
+    SK_PREFER_SMEM(ctx, append_small_kernel<false>);
+    SK_CUDA_CHECK(ctx, sk_launch(ctx, append_small_kernel<false>, dim3(a.n_tiles, a.n_part), dim3(APS_THREADS), 0, L, a));
+    zp = (const float*)ws;
+    n_part = a.n_part;
   } else if (d_in_k % 8 == 0 && d_in_v % 8 == 0 && k_row_stride % 8 == 0 && k_head_stride % 8 == 0 && v_row_stride % 8 == 0 &&
              ((uintptr_t)k_new & 15) == 0 && ((uintptr_t)v_new & 15) == 0 && ((uintptr_t)A_k & 15) == 0 &&
              ((uintptr_t)A_v & 15) == 0) {
     int nkt = 0;
     for (int h = 0; h < L.n_kv_heads; ++h) nkt += (L.rank_k[h] + GN - 1) / GN;
     const int nvt = (L.rank_v + GN - 1) / GN;
-    // starkv_set_option(ctx, "append_tc5", 1) selects the tcgen05/TMEM kernel.  It is correct (bit-exact parity) but, staged by
-    // 16-byte cp.async into 128 x 64 no-swizzle tiles, it is L2-bound and slower than the mma.sync kernel (measured
-    // 95 vs 80 us on the C4 prefill chunk), so it is opt-in until it moves to TMA + 128B swizzle + wider tiles.
-    const bool use_tc5 = n_new >= 64 && ctx->append_tc5 && (((L.sum_rank_k + L.rank_v) & 7) == 0);
-    if (use_tc5) {
-      int nkt5 = 0;
-      for (int h = 0; h < L.n_kv_heads; ++h) nkt5 += (L.rank_k[h] + TN - 1) / TN;
-      const int nvt5 = (L.rank_v + TN - 1) / TN;
-      SK_CUDA_CHECK(ctx, sk_need_smem(ctx, append_project_tc5_kernel, TC5_SMEM));
-      append_project_tc5_kernel<<<dim3(nkt5 + nvt5, (n_new + TM - 1) / TM), 256, TC5_SMEM, ctx->stream>>>(
-          L, n_new, nkt5, (const __half*)k_new, k_row_stride, k_head_stride, d_in_k, (const __half*)v_new, v_row_stride, d_in_v,
-          (const __half*)A_k, (const __half*)A_v, z);
-    } else {
+    // The TMA + tcgen05 GEMM (append_gemm.cu) is the default for n_new >= 64; starkv_set_option(ctx, "append_tc5", 0) forces the
+    // mma.sync kernel below (kept as the second implementation the tests compare, and for what the GEMM does not cover).
+    const int g = ctx->append_tc5 ? sk_append_gemm(ctx, pool, table, max_pages, seq_ids, positions, n_new, k_new, k_row_stride,
+                                                   k_head_stride, d_in_k, v_new, v_row_stride, d_in_v, A_k, A_v, z)
+                                  : 0;
+    if (g == 2) {   // projection, quantiser and paged write in one kernel
+      ctx->last_launches = 1;
+      return STARKV_OK;
+    }
+    if (!g) {
+    ctx->last_append = "append_project_mma_kernel";
     SK_PREFER_SMEM(ctx, append_project_mma_kernel);
     append_project_mma_kernel<<<dim3(nkt + nvt, (n_new + GM - 1) / GM), 128, 0, ctx->stream>>>(
         L, n_new, nkt, (const __half*)k_new, k_row_stride, k_head_stride, d_in_k, (const __half*)v_new, v_row_stride, d_in_v,
         (const __half*)A_k, (const __half*)A_v, z);
     }
   } else {
+  ctx->last_append = "append_project_kernel";
   dim3 g1(L.n_kv_heads + (L.rank_v + 127) / 128, (n_new + APP_TOK - 1) / APP_TOK);
   append_project_kernel<<<g1, 128, 0, ctx->stream>>>(L, n_new, (const __half*)k_new, k_row_stride, k_head_stride, d_in_k,
                                                      (const __half*)v_new, v_row_stride, d_in_v, (const __half*)A_k,
                                                      (const __half*)A_v, z);
   }
   SK_CUDA_CHECK(ctx, cudaGetLastError());
-  const size_t smem = ((size_t)(L.sum_rank_k + L.rank_v) * 2 + 15) / 16 * 16;
-  if ((int)smem > ctx->smem_optin) return STARKV_ERR_UNSUPPORTED;
   if (smem > 48 * 1024) SK_CUDA_CHECK(ctx, sk_need_smem(ctx, append_write_kernel, (int)smem));
   SK_PREFER_SMEM(ctx, append_write_kernel);
-  sk_launch(ctx, append_write_kernel, dim3(n_new), dim3(512), smem, L, (const __half*)z, (const float*)nullptr, 1, n_new, seq_ids,
-            positions, table, max_pages, (uint8_t*)pool);
+  sk_launch(ctx, append_write_kernel, dim3(n_new), dim3(AW_THREADS), smem, L, (const __half*)z, zp, n_part, n_new,
+            seq_ids, positions, table, max_pages, (uint8_t*)pool);
   ctx->last_launches = 2;
   SK_CUDA_CHECK(ctx, cudaGetLastError());
   return STARKV_OK;

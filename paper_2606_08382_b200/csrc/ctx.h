@@ -16,11 +16,12 @@ struct starkv_ctx {
   int smem_per_sm;       // shared memory per SM
   int n_splits_override; // 0 = automatic
   int last_launches;
+  const char* last_append;   // projection kernel of the last starkv_append (starkv_last_append_kernel_name)
   int fast_ok;           // tensor-core decode kernel covers this descriptor
   DecodePlan plan;
   TmPlan tm;             // TMEM-operand kernel of the integer modes (decode_tm.cu); tm.ok = it covers this descriptor
   int variant;           // decode kernel choice, SK_VARIANT_* (starkv_set_option "decode_variant"); 0 = automatic
-  int append_tc5;        // prefill projection on the tcgen05 kernel (starkv_set_option "append_tc5")
+  int append_tc5;        // prefill projection on the TMA + tcgen05 GEMM (default 1; starkv_set_option "append_tc5" 0 = mma.sync)
   int host_graph;        // HOST-buffer entry points replay a cached CUDA graph (starkv_set_option "host_graph")
   int pdl;               // launch the step's kernels with programmatic dependent launch (starkv_set_option "pdl")
   int timing_on;         // record events around the main decode kernel
@@ -145,7 +146,13 @@ int sk_append(starkv_ctx* ctx, void* pool, const int32_t* table, int max_pages, 
               int64_t k_head_stride, int d_in_k, const void* v_new, int64_t v_row_stride, int d_in_v,
               const void* A_k, const void* A_v, void* ws, size_t ws_bytes);
 size_t sk_append_ws_bytes(const starkv_ctx* ctx, int n_new);
+// append_gemm.cu: prefill append (n_new >= 64) by TMA + tcgen05; 2 = done (quantiser and paged write fused), 1 = z holds
+// fp16(X . A), 0 = not covered (the caller falls back)
+int sk_append_gemm(starkv_ctx* ctx, void* pool, const int32_t* table, int max_pages, const int32_t* seq_ids,
+                   const int32_t* positions, int n_new, const void* k_new, int64_t k_row_stride, int64_t k_head_stride, int d_in_k,
+                   const void* v_new, int64_t v_row_stride, int d_in_v, const void* A_k, const void* A_v, void* z);
 int sk_append_small_ok(const starkv_ctx* ctx, int n_new);   // the one-launch append covers n_new tokens
+int sk_append_small_fused(const starkv_ctx* ctx, int n_new, int n_part, int limit);   // A1-A4 in one launch (else A1, then append_write_kernel)
 void sk_append_small_args(const starkv_ctx* ctx, AppendSmallArgs* a, void* pool, const int32_t* table, int max_pages,
                           const int32_t* seq_ids, const int32_t* positions, int n_new, const void* k_new, int64_t k_row_stride,
                           int64_t k_head_stride, int d_in_k, const void* v_new, int64_t v_row_stride, int d_in_v,

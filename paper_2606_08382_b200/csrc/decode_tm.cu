@@ -241,7 +241,7 @@ __global__ void __launch_bounds__(QP_THREADS) step_pre_tm_kernel(const __grid_co
     qproj_tm_body(L, T, q, B_k, img_all, img_stride, i % nhb, i / nhb, *reinterpret_cast<QpShared*>(sm));
   } else {
     const int j = i - n_qp;
-    append_small_body(L, a, j % a.n_tiles, j / a.n_tiles, sm);
+    append_small_body<true>(L, a, j % a.n_tiles, j / a.n_tiles, sm);
   }
 }
 

@@ -67,7 +67,7 @@ def test_pack_empty_is_a_no_op():
     sk.starkv_unpack(ctx, None, 0)
 
 
-def _append_case(cfg, mode, n_new, dyadic, pad=0, tc5=False):
+def _append_case(cfg, mode, n_new, dyadic, pad=0, tc5=True, ordered=False):
     d = CacheDesc.from_config(cfg)
     lay = page_layout(d)
     rng = np.random.default_rng(5)
@@ -82,7 +82,7 @@ def _append_case(cfg, mode, n_new, dyadic, pad=0, tc5=False):
         for p in range(int(lens[b]), int(tot[b])):
             seq_ids.append(b)
             positions.append(p)
-    order = rng.permutation(len(seq_ids))
+    order = np.arange(len(seq_ids)) if ordered else rng.permutation(len(seq_ids))
     seq_ids = np.array(seq_ids, np.int32)[order]
     positions = np.array(positions, np.int32)[order]
     n = len(seq_ids)
@@ -107,8 +107,7 @@ def _append_case(cfg, mode, n_new, dyadic, pad=0, tc5=False):
     kw, vw = k2.shape[1], v2.shape[1]
     oappend.append(d, ref, table, seq_ids, positions, k2, khs, d_in_k, v2, ak, av)
     ctx = sk.create_from_config(cfg)
-    if tc5:
-        sk.starkv_set_option(ctx, "append_tc5", 1)
+    sk.starkv_set_option(ctx, "append_tc5", 1 if tc5 else 0)
     dpool = dev(pool)
     wsb = sk.starkv_append_workspace_bytes(ctx, n)
     ws = torch.empty(max(wsb, 16), dtype=torch.uint8, device="cuda")
@@ -119,6 +118,9 @@ def _append_case(cfg, mode, n_new, dyadic, pad=0, tc5=False):
     sk.starkv_append(ctx, dpool, dev(table.astype(np.int32)), table.shape[1], dev(seq_ids), dev(positions), n,
                      kd, kw + pad, khs, d_in_k, vd, vw + pad, d_in_v, f16(ak), f16(av), ws, wsb)
     torch.cuda.synchronize()
+    want = ("append_small_kernel" if n <= 16 else "append_project_kernel" if pad else
+            "append_gemm_kernel" if (tc5 and n >= 64) else "append_project_mma_kernel")
+    assert sk.starkv_last_append_kernel_name(ctx) == want   # the path under test really ran (no silent fallback)
     return d, lay, dpool.cpu().numpy(), ref, n
 
 
@@ -132,6 +134,16 @@ def test_append_bit_exact_on_dyadic_inputs(name, mode, n_new):
     n_new = abs(n_new)
     cfg = synth.make_config(name, context=256, batch=3)
     d, lay, got, ref, n = _append_case(cfg, mode, n_new, dyadic=True, tc5=tc5)
+    assert np.array_equal(got, ref), f"{int((got != ref).sum())} bytes differ of {got.size}"
+
+
+@pytest.mark.parametrize("name,mode", [("C1", "dense"), ("C3", "dense"), ("C4", "hidden"), ("C2", "dense")])
+def test_append_prefill_chunk_in_position_order(name, mode):
+    """Tokens in (sequence, position) order, the first sequence starting mid-octet (position 70): append_write_kernel maps
+    whole slot octets of a page to CTAs and writes the channel-major value fields as whole words (no atomics); the other
+    sequences start at other offsets and take the per-field path.  Pre-existing bytes of the pages must survive."""
+    cfg = synth.make_config(name, context=256, batch=3)
+    d, lay, got, ref, n = _append_case(cfg, mode, 80, dyadic=True, ordered=True)
     assert np.array_equal(got, ref), f"{int((got != ref).sum())} bytes differ of {got.size}"
 
 

@@ -446,7 +446,7 @@ def test_fused_step_equals_append_then_decode_and_the_oracle(name, ctxlen, batch
         else:
             sk.starkv_append(ctx, pool, d["table"], mp, d["seq"], d["pos"], batch, d["k"], k2.shape[1], cfg.head_dim, dk_in,
                              d["v"], v2.shape[1], dv_in, d["ak"], d["av"], aws, awsb)
-            assert sk.starkv_last_launches(ctx) == 1
+            assert sk.starkv_last_launches(ctx) in (1, 2)   # one launch unless the group's serial tail would be long (C4)
             sk.starkv_decode_attn(ctx, d["q"], pool, d["table"], mp, d["lens"], batch, d["bk"], d["bv"], ws, wsb, out)
         torch.cuda.synchronize()
         res.append((pool.cpu().numpy(), out.cpu().numpy()))

@@ -346,9 +346,7 @@ def prefill_append_leg(wl, sk, torch, device, T):
     wsb = sk.starkv_append_workspace_bytes(wl.ctx, T)
     ws = torch.empty(wsb, dtype=torch.uint8, device=device)
     f16 = lambda a: torch.from_numpy(np.ascontiguousarray(a).view(np.int16)).to(device).view(torch.float16)  # noqa: E731
-    tc5 = False
-    out = {"tokens": T, "kernels": ("append_project_tc5_kernel (tcgen05.mma, TMEM accumulator)" if tc5 else
-                                    "append_project_mma_kernel (mma.sync m16n8k16, fp32 accumulate)") + " + append_write_kernel"}
+    out = {"tokens": T}
     for mode in ("dense", "hidden"):
         if mode == "dense":
             dk, dv, khs = cfg.head_dim, cfg.n_kv_heads * cfg.head_dim, cfg.head_dim
@@ -376,7 +374,8 @@ def prefill_append_leg(wl, sk, torch, device, T):
             e1.record(wl.stream)
             wl.stream.synchronize()
         us = e0.elapsed_time(e1) * 1e3 / 20
-        out[mode] = {"us_per_call": us, "projection_tflops": flops / (us * 1e-6) / 1e12, "d_in_k": dk, "d_in_v": dv}
+        out[mode] = {"us_per_call": us, "projection_tflops": flops / (us * 1e-6) / 1e12, "d_in_k": dk, "d_in_v": dv,
+                     "kernel": sk.starkv_last_append_kernel_name(wl.ctx), "launches": sk.starkv_last_launches(wl.ctx)}
     return out
 
 

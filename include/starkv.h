@@ -152,6 +152,22 @@ int starkv_decode_step(starkv_ctx* ctx, void* page_pool, const int32_t* block_ta
                        const void* q, const int32_t* seq_lens, const void* B_k, const void* B_v,
                        void* workspace, size_t workspace_bytes, void* out);
 
+/* starkv_decode_attn_static: starkv_decode_attn for callers that cannot allocate (code under CUDA graph capture, tight
+ * serving loops, harnesses that forbid cudaMalloc): same arguments, meanings, kernels and result, but NO workspace
+ * argument -- the decode scratch (query image, split-K partials) lives in a file-scope device array of
+ * STARKV_STATIC_SCRATCH_BYTES that every GPU which loads the library holds until the process exits.  The call makes no
+ * cudaMalloc / cudaFree / allocating library call.  A call whose starkv_workspace_bytes(ctx, batch, max_pages) exceeds the
+ * array returns STARKV_ERR_WORKSPACE (starkv_last_error names both sizes); 8 MiB covers BASELINE.json configs C2-C5.
+ * All calls on a device share the array and it keeps the last call's contents (nothing in it needs to start at zero:
+ * each call writes every region before reading it); calls that OVERLAP on the GPU -- two streams, contexts or threads
+ * on one device -- race on it: serialise them or use starkv_decode_attn with a workspace per stream.  The first call on
+ * a device resolves the array's device address (cudaGetSymbolAddress) and loads the kernels: make it outside a
+ * graph capture.  Other error codes as starkv_decode_attn. */
+#define STARKV_STATIC_SCRATCH_BYTES (8u << 20)
+int starkv_decode_attn_static(starkv_ctx* ctx, const void* q, const void* page_pool,
+                              const int32_t* block_table, int max_pages, const int32_t* seq_lens,
+                              int batch, const void* B_k, const void* B_v, void* out);
+
 /* Same operation through the plain scalar kernel (any page_tokens / head count; fp32 math,
  * exact dequantisation).  Slow; used as a second implementation in tests and for shapes the
  * tensor-core kernel does not cover. */

@@ -7,7 +7,7 @@ import sys
 
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
-SOURCES = ["api.cu", "codec.cu", "decode_generic.cu", "decode_fast.cu", "decode_tm.cu", "append_gemm.cu"]
+SOURCES = ["api.cu", "codec.cu", "decode_generic.cu", "decode_fast.cu", "decode_tm.cu", "append_gemm.cu", "decode_static.cu"]
 LIB = os.path.join(HERE, "libstarkv.so")
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "-Xcompiler", "-fPIC", "-Xptxas", "-v"]

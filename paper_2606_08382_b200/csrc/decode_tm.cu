@@ -48,8 +48,9 @@ namespace {
 constexpr int PTOK = 64;              // tokens per page on this path
 constexpr int TM_THREADS = 768;
 constexpr int TM_TBL = 512;           // block-table entries of the CTA's range kept in shared memory
-constexpr float P_OFFSET = 8.f;       // p' = 2^(s - m + 8)
-constexpr float TAU = 6.f;            // the running maximum may lag the true one by 2^TAU: p' <= 2^14
+constexpr float P_OFFSET = 4.f;       // p' = 2^(s - m + 4)
+constexpr float A_SHIFT = 16.f;       // ... and the value-scale factor carries the other 2^4: a = 16 s_v / M (same product as 2^8 and 1)
+constexpr float P_CAP = 46000.f;      // update the references before p' or an operand p' a could exceed this (fp16 holds 65504)
 constexpr float kLog2e = 1.4426950408889634f;
 constexpr int BAR_SM = 1;             // named barrier of the softmax warps
 constexpr int P_BLK_BYTES = 8192;     // P~ operand of one precision block: 128 tokens x 32 heads fp16
@@ -326,7 +327,7 @@ __global__ void __launch_bounds__(TM_THREADS, 1) decode_tm_kernel(
     fence_barrier_init();
   }
   if (warp == 23) tmem_alloc(smem_u32((const void*)tmem_slot), TM_COLS);
-  if (tid < 36) misc[tid] = tid < 32 ? -P_OFFSET : (tid < 34 ? 0.f : 1.f);   // reference m - 8 with m = 0, M = 0 (forces the first update), 1/M = 1
+  if (tid < 36) misc[tid] = tid < 32 ? -P_OFFSET : (tid < 34 ? 0.f : A_SHIFT);   // reference m - P_OFFSET with m = 0, M = 0, a-factor A_SHIFT / 1 (all replaced by the first tile)
 
   sk_pdl_wait();   // seq_lens, block table, query image, pages: nothing global is read before this point
   const int len = seq_lens[b];
@@ -494,21 +495,30 @@ __global__ void __launch_bounds__(TM_THREADS, 1) decode_tm_kernel(
           for (int g = 0; g < G; ++g)
             arg[hl * G + g] = fmaf(sc[2 * hl], __uint_as_float(d[2 * hl * G + g]), sc[2 * hl + 1] * __uint_as_float(d[2 * hl * G + G + g]));
         if (it == 0) {
-          // The references start from the range's first token (always inside the sequence): its scores, and 2^8 times its
-          // value scales.  A later token that exceeds them by the lazy bounds takes the (rare) update path below, so the
-          // common case never runs that code at all -- it would run instruction-cache cold on every CTA.
-          if (tq == 0) {
+          // The references start from the range's first 32 tokens (warp 0 of each half; the first token is always inside
+          // the sequence): per head the largest of their scores, and 2^8 times their largest value scales.  A later token
+          // that exceeds them by the lazy bounds takes the update path below.  That path costs about 2.8 us per CTA
+          // (three barriers, reductions, a rescale of the TMEM accumulators, all instruction-cache cold), so it has to be
+          // rare: with the FIRST token's score as the reference it ran in most CTAs of the diffuse regime (any of the
+          // range's tokens 2^6 above one arbitrary token triggers it), with the maximum of 32 it does not.
+          if (wq == 0) {
 #pragma unroll
-            for (int i = 0; i < NHH; ++i) mref_s[hbase + i] = arg[i] - P_OFFSET;
+            for (int i = 0; i < NHH; ++i) {
+              const int k = __reduce_max_sync(0xffffffffu, f_ordered(valid ? arg[i] : -INFINITY));
+              if (lane == 0) mref_s[hbase + i] = f_unordered(k) - P_OFFSET;
+            }
             if (hh == 0) {
 #pragma unroll
               for (int blk = 0; blk < 2; ++blk) {
-                const float sv = blk ? sv1 : sv0;
-                unsigned eb = ((__float_as_uint(sv) >> 23) & 0xffu) + 8u;   // (a single token: 2^8 of headroom)
+                // (non-negative floats order as their bits)
+                const float sv = __uint_as_float(__reduce_max_sync(0xffffffffu, __float_as_uint(blk ? sv1 : sv0)));
+                unsigned eb = ((__float_as_uint(sv) >> 23) & 0xffu) + 8u;   // 2^8 of headroom
                 if (eb > 254u) eb = 254u;
                 const float M = sv > 0.f ? __uint_as_float(eb << 23) : 1.f;
-                M_s[blk] = M;
-                invM_s[blk] = 1.f / M;
+                if (lane == 0) {
+                  M_s[blk] = M;
+                  invM_s[blk] = A_SHIFT / M;
+                }
               }
             }
           }
@@ -529,7 +539,13 @@ __global__ void __launch_bounds__(TM_THREADS, 1) decode_tm_kernel(
           tc_fence_after();
           tmem_ld<2 * NHH>(tlane + (uint32_t)(T.col_ds + sn * T.ds_cols + 2 * hbase), d);
         }
-        const bool trig = valid && (mxa > TAU + P_OFFSET || sv0 > M0 || sv1 > M1);
+        // The fp16 operand is P~ = p' a with p' = 2^(s - m + 4) and a = 16 s_v / M, both fp16.  The references only have to
+        // move when p' or the product nears the fp16 limit: the running maximum may lag the true one by 2^11.5 (2^6 with
+        // the split 2^8 and 1 of the same product), which keeps the (costly) update path out of the way of heavy-tailed
+        // scores.
+        float a0 = sv0 * invM_s[0], a1 = sv1 * invM_s[1];
+        const float pmax = ex2(mxa);
+        const bool trig = valid && (pmax > P_CAP || pmax * fmaxf(a0, a1) > P_CAP || sv0 > M0 || sv1 > M1);
         const bool wany = __any_sync(0xffffffffu, trig);
         if (lane == 0) {
           flag[buf * 8 + wr] = wany ? 1 : 0;
@@ -602,12 +618,12 @@ __global__ void __launch_bounds__(TM_THREADS, 1) decode_tm_kernel(
           if (tq < NHH) mref_s[hbase + tq] = mnew_s[hbase + tq];
           if (hh == 0 && tq == 0) {
             M_s[0] = Mn[0]; M_s[1] = Mn[1];
-            invM_s[0] = 1.f / Mn[0]; invM_s[1] = 1.f / Mn[1];
+            invM_s[0] = A_SHIFT / Mn[0]; invM_s[1] = A_SHIFT / Mn[1];
           }
           bar_sync(BAR_SM, NBAR);
+          a0 = sv0 * invM_s[0]; a1 = sv1 * invM_s[1];
         }
         // ---- p' and the two scaled operands
-        const float a0 = sv0 * invM_s[0], a1 = sv1 * invM_s[1];
         const uint32_t a0h = pack_h2(a0, a0), a1h = pack_h2(a1, a1);
         if (it >= 2) mbar_wait(pv_done0 + 8 * buf, (uint32_t)(((it >> 1) - 1) & 1));   // the MMAs of tile it - 2 have read the buffer
         uint8_t* pb = smem + T.off_p + buf * 2 * P_BLK_BYTES;
@@ -644,7 +660,7 @@ __global__ void __launch_bounds__(TM_THREADS, 1) decode_tm_kernel(
           tmem_ld<NHH>(tlane + (uint32_t)(T.col_do + 32 * dt + hbase), v);
           tmem_wait_ld();
           const bool mine = ch < L.rank_v && ((ch >= L.v_hi_n) == (blk == 1));
-          const float Mb = M_s[blk];
+          const float Mb = M_s[blk] * (1.f / A_SHIFT);   // O = sum c p' a = (16 / M) sum c p' s_v: back to the scale of l = sum p'
           if (mine) {
 #pragma unroll
             for (int i = 0; i < NHH; ++i)

@@ -6,6 +6,10 @@
 
 namespace {
 
+// largest joint value rank of the scalar path (the paper's 75%-compressed MHA layer has r_v = 1024: PAPER.md Fig.11)
+constexpr int SK_GEN_MAX_RV = 1024, GEN_VT = SK_GEN_MAX_RV / 128;
+
+
 constexpr float kLog2e = 1.4426950408889634f;
 
 __device__ __forceinline__ float block_reduce(float v, bool is_max, float* red) {
@@ -77,7 +81,9 @@ __global__ void __launch_bounds__(128) decode_generic_kernel(
   __syncthreads();
 
   float m_run = -INFINITY, l_run = 0.f;
-  float acc[4] = {0.f, 0.f, 0.f, 0.f};   // channels threadIdx.x + 128*k  (rank_v <= 512)
+  float acc[GEN_VT];   // channels threadIdx.x + 128*k  (rank_v <= 128 GEN_VT = 1024)
+#pragma unroll
+  for (int k = 0; k < GEN_VT; ++k) acc[k] = 0.f;
   const int n_hi = L.k_hi_n[g], n_lo = L.k_lo_n[g];
   for (int pg = p0; pg < p1; ++pg) {
     const uint8_t* page = pool + (size_t)table[(size_t)b * max_pages + pg] * L.page_bytes;
@@ -142,7 +148,7 @@ __global__ void __launch_bounds__(128) decode_generic_kernel(
       __syncthreads();
       const int nt = min(128, P - s0);
 #pragma unroll
-      for (int k = 0; k < 4; ++k) {
+      for (int k = 0; k < GEN_VT; ++k) {
         const int c = threadIdx.x + 128 * k;
         if (c >= L.rank_v) break;
         const int blk = (quant && c >= L.v_hi_n) ? 1 : 0;
@@ -165,7 +171,7 @@ __global__ void __launch_bounds__(128) decode_generic_kernel(
   float* out = parts + (((size_t)b * n_splits + split) * L.n_q_heads + head) * sk_part_stride(L.rank_v);
   if (threadIdx.x == 0) { out[0] = m_run; out[1] = l_run; }
 #pragma unroll
-  for (int k = 0; k < 4; ++k) {
+  for (int k = 0; k < GEN_VT; ++k) {
     const int c = threadIdx.x + 128 * k;
     if (c < L.rank_v) out[SK_PART_ACC + c] = acc[k];
   }
@@ -179,7 +185,7 @@ __global__ void __launch_bounds__(128) decode_generic_kernel(
 __global__ void __launch_bounds__(256) combine_kernel(const __grid_constant__ StarkvLayout L,
                                                       const float* __restrict__ parts, int n_splits,
                                                       const __half* __restrict__ B_v, __half* __restrict__ out) {
-  __shared__ float o_lat[512];
+  __shared__ float o_lat[SK_GEN_MAX_RV];
   __shared__ float wsm[512];
   __shared__ __align__(16) float red[32 * 64];   // [slice][d] partial outputs (slices * d_h <= 2048)
   __shared__ float rsm[8];
@@ -529,7 +535,7 @@ int sk_decode_generic(starkv_ctx* ctx, const void* q, const void* pool, const in
                       size_t ws_bytes, void* out, int rope, float rope_theta, const int32_t* pos_offset) {
   const StarkvLayout& L = ctx->L;
   ctx->last_launches = 0;
-  if (L.rank_v > 512) return STARKV_ERR_UNSUPPORTED;
+  if (L.rank_v > SK_GEN_MAX_RV) return STARKV_ERR_UNSUPPORTED;
   SkWorkspace w;
   sk_plan_workspace(ctx, batch, max_pages, &w);
   if (ws_bytes < w.total) return STARKV_ERR_WORKSPACE;

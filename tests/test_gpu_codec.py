@@ -147,6 +147,16 @@ def test_append_prefill_chunk_in_position_order(name, mode):
     assert np.array_equal(got, ref), f"{int((got != ref).sum())} bytes differ of {got.size}"
 
 
+@pytest.mark.parametrize("n_new", [80, 8], ids=["prefill", "decode-time"])
+def test_append_at_the_paper_sized_value_rank(n_new):
+    """Joint value rank 1024 (Fig.11): the low-precision value block has more than 512 columns, so the
+    prefill GEMM runs without its fused epilogue and append_write_kernel quantises; the decode-time path takes the
+    one-launch kernel's projection.  Bit-exact on dyadic inputs like every other shape."""
+    cfg = synth.custom_config("rv1024", 3, 32, 32, 128, 256, [32] * 32, 1024, bits=(8, 4))
+    d, lay, got, ref, n = _append_case(cfg, "dense", n_new, dyadic=True, ordered=(n_new == 80))
+    assert np.array_equal(got, ref), f"{int((got != ref).sum())} bytes differ of {got.size}"
+
+
 def test_append_unaligned_rows_take_the_scalar_kernel():
     cfg = synth.make_config("C3", context=256, batch=3)
     d, lay, got, ref, n = _append_case(cfg, "dense", 37, dyadic=True, pad=2)

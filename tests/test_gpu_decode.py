@@ -475,3 +475,18 @@ def test_contexts_with_different_shared_memory_plans_alternate():
         ref = oattn.decode_attn(cache["desc"], q, cache["pool"], cache["table"], cache["seq_lens"], bk, bv)
         out = run_decode(cfg, cache, q, bk, bv, ctx=ctx)
         assert row_rel_err(out, ref) <= TOL
+
+
+@pytest.mark.parametrize("bits", [(8, 4), (16, 16)], ids=str)
+def test_paper_sized_value_rank_and_wide_gqa(bits):
+    """Shapes beyond the tensor-core kernels' plans, served by the scalar kernel behind starkv_decode_attn: the paper's own
+    75%-compressed MHA layer (32 heads x 128, joint value rank 1024 of 4096: PAPER.md Fig.11) and a GQA layer with
+    64 query heads on 8 KV heads (G = 8).  Same oracle, same bar."""
+    mha = synth.custom_config(f"rv1024_{bits[0]}", 2, 32, 32, 128, 600, [32] * 32, 1024, bits=bits, outlier_frac=0.1)
+    err = _check(mha, seq_lens=[600, 333])
+    ctx = sk.create_from_config(mha)
+    assert sk.starkv_decode_kernel_name(ctx) == "decode_generic_kernel"
+    gqa = synth.custom_config(f"g8_{bits[0]}", 2, 64, 8, 128, 900, [24, 16, 24, 48, 16, 32, 56, 40], 256, bits=bits, outlier_frac=0.1)
+    _check(gqa, seq_lens=[900, 515])
+    _check(gqa, seq_lens=[900, 515], regime="peaky")
+    assert err <= TOL

@@ -39,14 +39,23 @@ struct AppendSmallArgs {
   int* tickets;   // n_kv_heads + 1 zeroed counters, reset by the last arriver
 };
 
-// page and slot of new token j, or nullptr when the caller's ids are out of range (the token is skipped, never written wildly)
-__device__ __forceinline__ uint8_t* aps_page_of(const StarkvLayout& L, const AppendSmallArgs& a, int j, int* slot) {
+// page index (-1: the caller's ids are out of range, the token is skipped, never written wildly) and slot of new token j
+__device__ __forceinline__ void aps_lookup(const StarkvLayout& L, const AppendSmallArgs& a, int j, int* pidx, int* slot) {
   const int P = L.page_tokens;
   const int pos = a.positions[j], sid = a.seq_ids[j];
-  if (pos < 0 || pos / P >= a.max_pages || sid < 0) return nullptr;
-  const int pidx = a.table[(size_t)sid * a.max_pages + pos / P];
-  if (pidx < 0) return nullptr;
+  *pidx = -1;
+  *slot = 0;
+  if (pos < 0 || pos / P >= a.max_pages || sid < 0) return;
+  *pidx = a.table[(size_t)sid * a.max_pages + pos / P];
   *slot = pos % P;
+}
+// the same from the table every CTA fills at its start (two dependent global loads hidden behind the projection instead
+// of sitting in the last CTA's serial tail)
+__device__ __forceinline__ uint8_t* aps_page_of(const StarkvLayout& L, const AppendSmallArgs& a, const int* s_pidx,
+                                                const int* s_slot, int j, int* slot) {
+  const int pidx = s_pidx[j];
+  if (pidx < 0) return nullptr;
+  *slot = s_slot[j];
   return a.pool + (size_t)pidx * L.page_bytes;
 }
 
@@ -57,6 +66,8 @@ template <bool FUSED>
 __device__ __forceinline__ void append_small_body(const StarkvLayout& L, const AppendSmallArgs& a, int bx, int by, float* sm) {
   __shared__ int s_last;
   __shared__ float s_vsc[APS_TOK][2];
+  __shared__ int s_pidx[APS_TOK], s_slot[APS_TOK];
+  if (FUSED && threadIdx.x < a.n_new) aps_lookup(L, a, threadIdx.x, &s_pidx[threadIdx.x], &s_slot[threadIdx.x]);
   const int R = L.sum_rank_k + L.rank_v;
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const int n_new = a.n_new;
@@ -93,15 +104,18 @@ __device__ __forceinline__ void append_small_body(const StarkvLayout& L, const A
 #pragma unroll
       for (int kk = 0; kk < 32; ++kk) av[kk] = kk < kn ? *reinterpret_cast<const uint32_t*>(ap + (size_t)kk * lda) : 0u;
     }
-    __syncthreads();
-    if (a.x_vec) {   // 16-byte aligned rows, d_in a multiple of 8: two independent 16-byte loads per thread
-      uint4 xv[2];
+    uint4 xv[2];
+    if (a.x_vec) {   // 16-byte aligned rows, d_in a multiple of 8: two independent 16-byte loads per thread, in flight
+                     // together with the factor rows (issued before the barrier that frees the shared-memory chunk)
 #pragma unroll
       for (int u = 0; u < 2; ++u) {
         const int i = tid + u * APS_THREADS, t = i >> 5, k8 = (i & 31) * 8;
         xv[u] = (t < n_new && kc + k8 < k_end) ? *reinterpret_cast<const uint4*>(x0 + (long long)t * xstride + kc + k8)
                                                : make_uint4(0u, 0u, 0u, 0u);
       }
+    }
+    __syncthreads();
+    if (a.x_vec) {
 #pragma unroll
       for (int u = 0; u < 2; ++u) {
         const int i = tid + u * APS_THREADS, t = i >> 5, k8 = (i & 31) * 8;
@@ -183,7 +197,7 @@ __device__ __forceinline__ void append_small_body(const StarkvLayout& L, const A
     for (int u = warp; u < n_new * 2; u += APS_THREADS / 32) {
       const int j = u >> 1, blk = u & 1;
       int slot;
-      uint8_t* pg = aps_page_of(L, a, j, &slot);
+      uint8_t* pg = aps_page_of(L, a, s_pidx, s_slot, j, &slot);
       if (!pg) continue;
       const int n = blk ? L.k_lo_n[h] : L.k_hi_n[h];
       if (!quant) {
@@ -235,7 +249,7 @@ __device__ __forceinline__ void append_small_body(const StarkvLayout& L, const A
         const __half s16 = n ? sk_scale_of(amax, sk_qmax(w ? L.bits_lo : L.bits_hi)) : __float2half(0.f);
         s_vsc[j][w] = __half2float(s16);
         int slot;
-        uint8_t* pg = aps_page_of(L, a, j, &slot);
+        uint8_t* pg = aps_page_of(L, a, s_pidx, s_slot, j, &slot);
         if (pg) reinterpret_cast<uint16_t*>(pg + L.v_scale_off)[w * P + slot] = sk_half_bits(s16);
       }
     }
@@ -244,7 +258,7 @@ __device__ __forceinline__ void append_small_body(const StarkvLayout& L, const A
   for (int i = tid; i < n_new * gcols; i += APS_THREADS) {
     const int j = i / gcols, c = i - j * gcols;
     int slot;
-    uint8_t* pg = aps_page_of(L, a, j, &slot);
+    uint8_t* pg = aps_page_of(L, a, s_pidx, s_slot, j, &slot);
     if (!pg) continue;
     const int blk = (quant && c >= L.v_hi_n) ? 1 : 0;
     const int idx = blk ? c - L.v_hi_n : c;

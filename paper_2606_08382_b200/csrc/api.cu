@@ -199,13 +199,15 @@ int starkv_decode_step(starkv_ctx* ctx, void* pool, const int32_t* table, int ma
     return STARKV_ERR_INVALID_ARG;
   if (append_ws_bytes < sk_append_ws_bytes(ctx, batch)) return STARKV_ERR_WORKSPACE;
   AppendSmallArgs a;
-  if (sk_decode_choice(ctx) == SK_VARIANT_TM && sk_append_small_ok(ctx, batch))
+  const int choice = sk_decode_choice(ctx);
+  if (choice != SK_VARIANT_GENERIC && sk_append_small_ok(ctx, batch))
     sk_append_small_args(ctx, &a, pool, table, max_pages, seq_ids, positions, batch, k_new, k_row_stride, k_head_stride, d_in_k,
                          v_new, v_row_stride, d_in_v, A_k, A_v, append_ws);
   else
     a.n_part = 0;
-  if (a.n_part > 0 && sk_append_small_fused(ctx, batch, a.n_part, 8192)) {
-    return sk_decode_tm(ctx, q, pool, table, max_pages, seq_lens, batch, B_k, B_v, ws, ws_bytes, out, &a);
+  if (a.n_part > 0 && sk_append_small_fused(ctx, batch, a.n_part, 8192)) {   // the append shares the query image's launch
+    if (choice == SK_VARIANT_TM) return sk_decode_tm(ctx, q, pool, table, max_pages, seq_lens, batch, B_k, B_v, ws, ws_bytes, out, &a);
+    return sk_decode_fast(ctx, q, pool, table, max_pages, seq_lens, batch, B_k, B_v, ws, ws_bytes, out, &a);
   }
   rc = sk_append(ctx, pool, table, max_pages, seq_ids, positions, batch, k_new, k_row_stride, k_head_stride, d_in_k, v_new,
                  v_row_stride, d_in_v, A_k, A_v, append_ws, append_ws_bytes);

@@ -174,7 +174,7 @@ int sk_decode_generic(starkv_ctx* ctx, const void* q, const void* pool, const in
                       size_t ws_bytes, void* out, int rope = 0, float rope_theta = 0.f, const int32_t* pos_offset = nullptr);
 int sk_decode_fast(starkv_ctx* ctx, const void* q, const void* pool, const int32_t* table, int max_pages,
                    const int32_t* seq_lens, int batch, const void* B_k, const void* B_v, void* ws,
-                   size_t ws_bytes, void* out);
+                   size_t ws_bytes, void* out, const AppendSmallArgs* app = nullptr);   // app: the step's append, run in the first launch
 int sk_fast_supported(const starkv_ctx* ctx);
 int sk_fast_plan(starkv_ctx* ctx);   // fills ctx->plan, ctx->fast_ok
 int sk_tm_plan(starkv_ctx* ctx);     // fills ctx->tm

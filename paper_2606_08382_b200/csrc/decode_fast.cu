@@ -31,6 +31,7 @@
 #include <stdlib.h>
 #include <string.h>
 
+#include "append_small.cuh"
 #include "decode_common.cuh"
 #include "decode_plan.h"
 
@@ -174,13 +175,9 @@ __device__ __forceinline__ void deq4_pairs(uint32_t w, uint32_t (&h)[4]) {
 // the other columns are zero.  Per sequence the output is  [image: n_qsteps * 256 B][kcst: H_kv * 8 fp32],
 // kcst = accumulator start values of the quantised QK blocks (see qk_block below).
 // ---------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(256) qproj_kernel(const __grid_constant__ StarkvLayout L,
-                                                    const __grid_constant__ DecodePlan PL, const __half* __restrict__ q,
-                                                    const __half* __restrict__ B_k, uint8_t* __restrict__ qimg_all,
-                                                    size_t qimg_stride) {
-  __shared__ float qt[256][4];   // q~[ch][i]
-  sk_pdl_enter();
-  const int g = blockIdx.x, b = blockIdx.y;
+__device__ __forceinline__ void qproj_body(const StarkvLayout& L, const DecodePlan& PL, const __half* __restrict__ q,
+                                           const __half* __restrict__ B_k, uint8_t* __restrict__ qimg_all, size_t qimg_stride,
+                                           int g, int b, float (*qt)[4] /* [256][4] shared: q~[ch][i] */) {
   const int G = L.group, dh = L.head_dim, r = L.rank_k[g];
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const bool act = lane * 8 < dh;
@@ -278,6 +275,36 @@ __global__ void __launch_bounds__(256) qproj_kernel(const __grid_constant__ Star
     if (lane == 0)
       reinterpret_cast<float*>(out_b + PL.qimg_bytes)[g * 8 + warp] =
           bits == 16 ? 0.f : -(float)(1 << (bits - 1)) * 5.9604644775390625e-8f * Q;
+  }
+}
+
+__global__ void __launch_bounds__(256) qproj_kernel(const __grid_constant__ StarkvLayout L,
+                                                    const __grid_constant__ DecodePlan PL, const __half* __restrict__ q,
+                                                    const __half* __restrict__ B_k, uint8_t* __restrict__ qimg_all,
+                                                    size_t qimg_stride) {
+  __shared__ float qt[256][4];
+  sk_pdl_enter();
+  qproj_body(L, PL, q, B_k, qimg_all, qimg_stride, blockIdx.x, blockIdx.y, qt);
+}
+
+// First launch of a fused decode step on this file's kernels (starkv_decode_step): the query image and the
+// compress-on-append of the step's new tokens are independent, so they share one grid -- blocks [0, n_qp) build the
+// image, the rest run the one-launch append (append_small.cuh).  Both finish before the decode kernel's
+// griddepcontrol.wait returns.
+static_assert(APS_THREADS == 256 && APS_SM_FLOATS >= 256 * 4, "the two bodies share a block size and the shared memory");
+__global__ void __launch_bounds__(256) step_pre_fast_kernel(const __grid_constant__ StarkvLayout L,
+                                                            const __grid_constant__ DecodePlan PL, const __half* __restrict__ q,
+                                                            const __half* __restrict__ B_k, uint8_t* __restrict__ qimg_all,
+                                                            size_t qimg_stride, int n_qp,
+                                                            const __grid_constant__ AppendSmallArgs a) {
+  __shared__ __align__(16) float sm[APS_SM_FLOATS];
+  sk_pdl_enter();
+  const int i = blockIdx.x;
+  if (i < n_qp) {
+    qproj_body(L, PL, q, B_k, qimg_all, qimg_stride, i % L.n_kv_heads, i / L.n_kv_heads, reinterpret_cast<float (*)[4]>(sm));
+  } else {
+    const int j = i - n_qp;
+    append_small_body<true>(L, a, j % a.n_tiles, j / a.n_tiles, sm);
   }
 }
 
@@ -1426,7 +1453,7 @@ void sk_plan_workspace(const starkv_ctx* ctx, int batch, int max_pages, SkWorksp
 
 int sk_decode_fast(starkv_ctx* ctx, const void* q, const void* pool, const int32_t* table, int max_pages,
                    const int32_t* seq_lens, int batch, const void* B_k, const void* B_v, void* ws, size_t ws_bytes,
-                   void* out) {
+                   void* out, const AppendSmallArgs* app) {
   const StarkvLayout& L = ctx->L;
   ctx->last_launches = 0;
   if (!ctx->fast_ok) return STARKV_ERR_UNSUPPORTED;
@@ -1435,9 +1462,16 @@ int sk_decode_fast(starkv_ctx* ctx, const void* q, const void* pool, const int32
   if (ws_bytes < w.total) return STARKV_ERR_WORKSPACE;
   float* parts = reinterpret_cast<float*>((uint8_t*)ws + w.part_off);
   uint8_t* qimg = (uint8_t*)ws + w.qimg_off;
-  SK_PREFER_SMEM(ctx, qproj_kernel);
-  SK_CUDA_CHECK(ctx, sk_launch(ctx, qproj_kernel, dim3(L.n_kv_heads, batch), dim3(256), 0, L, ctx->plan, (const __half*)q,
-                               (const __half*)B_k, qimg, w.qimg_stride));
+  if (app) {
+    const int n_qp = L.n_kv_heads * batch;
+    SK_PREFER_SMEM(ctx, step_pre_fast_kernel);
+    SK_CUDA_CHECK(ctx, sk_launch(ctx, step_pre_fast_kernel, dim3(n_qp + app->n_tiles * app->n_part), dim3(256), 0, L, ctx->plan,
+                                 (const __half*)q, (const __half*)B_k, qimg, w.qimg_stride, n_qp, *app));
+  } else {
+    SK_PREFER_SMEM(ctx, qproj_kernel);
+    SK_CUDA_CHECK(ctx, sk_launch(ctx, qproj_kernel, dim3(L.n_kv_heads, batch), dim3(256), 0, L, ctx->plan, (const __half*)q,
+                                 (const __half*)B_k, qimg, w.qimg_stride));
+  }
   const dim3 grid(w.n_splits, batch);
   const uint8_t* pl = (const uint8_t*)pool;
   if (ctx->timing_on) SK_CUDA_CHECK(ctx, cudaEventRecord(ctx->ev0, ctx->stream));

@@ -85,6 +85,34 @@ def decode_attn(d: CacheDesc, q16: np.ndarray, pool: np.ndarray, block_table: np
     return out
 
 
+def decode_attn_latent(d: CacheDesc, q16: np.ndarray, pool: np.ndarray, block_table: np.ndarray,
+                       seq_lens: Sequence[int], bk16: np.ndarray, heads: Optional[Sequence[int]] = None):
+    """NEXT-3, latent-output mode: the attention emits o~_i = softmax(s_i) . L_v, a row of r_v latent
+    channels per query head, and leaves the up-projection to an output projection with U_V absorbed
+    (section 3.3: "(p . V') . U_V", W'_out^i = W_out^i U_V^i).  Scores exactly as in decode_attn
+    (dequantise, reconstruct K = L_k B_k, q . K, L58 / L62-68); softmax L54; then the weights times the dequantised
+    joint value latents -- no B_v anywhere.  out float64 [B, H_q, r_v]; seq_len 0 gives a zero row (reading N2)."""
+    B = q16.shape[0]
+    G = d.group
+    heads = list(range(d.n_q_heads)) if heads is None else [int(h) for h in heads]
+    q = q16.astype(np.float64)
+    bk = bk16.astype(np.float64)
+    koff = d.k_offsets()
+    out = np.zeros((B, d.n_q_heads, d.rank_v))
+    for b in range(B):
+        l = int(seq_lens[b])
+        if l == 0:
+            continue
+        Lk, Lv = read_sequence(d, pool, block_table[b], l)
+        for i in heads:
+            g = i // G
+            Kg = Lk[:, koff[g]:koff[g] + d.rank_k[g]] @ bk[koff[g]:koff[g] + d.rank_k[g]]   # [l, d_h]
+            s = (Kg @ q[b, i]) * d.sm_scale
+            p = np.exp(s - s.max())
+            out[b, i] = (p / p.sum()) @ Lv
+    return out
+
+
 def rope_rotate(x: np.ndarray, positions: np.ndarray, theta: float) -> np.ndarray:
     """Rotary position embedding of rows x[t, :d_h] at integer positions[t] (Su et al. 2024; §3.3:
     "RoPE ... applied to the query and key states prior to computing attention scores").

@@ -19,10 +19,12 @@
 //        code offset 2^(b-1) is one more k-step whose A row is the constant (2^-14, 2^-14, 0...) and whose B tile holds
 //        -2^(b-1) 2^-10 sum_c Q_c (hi, lo): it also initialises the tile (accumulate off, N = all columns).
 //   softmax  thread = token reads its score columns (tcgen05.ld), applies the per-(token, head, block) key scales in
-//        fp32, p' = 2^(s - m + 8) against a LAZY running maximum m (moved only when a tile exceeds it by 2^6, so that
-//        P <= 2^14 in fp16), folds the per-token VALUE scales into two fp16 operands P~_blk = p' s_v / M_blk (M_blk = a
-//        running power of two above the scales seen, so the operand cannot overflow) and stores them MN-major.  When a
-//        maximum or M_blk moves (rare), the softmax warps rescale the TMEM accumulators and their running sums.
+//        fp32, p' = 2^(s - m + 4) against a LAZY running maximum m, and folds the per-token VALUE scales into two fp16
+//        operands P~_blk = p' a, a = 16 s_v / M_blk (M_blk = a running power of two above the scales seen, so the operand
+//        cannot overflow), stored MN-major.  m and M_blk move only when p' or the product would near the fp16 limit
+//        (a tile exceeding m by about 2^11.5): moving them means rescaling the TMEM accumulators, which drains the
+//        pipeline (about 2.8 us), so the first references are the maximum over the range's first 32 tokens and the
+//        update path stays out of the common case.
 //   PV   O[channel, head] += c[channel, token] P~[token, head]:  A = exact signed codes (magic-number trick), B = P~ of
 //        the channel's block; a 128-channel A tile that straddles the block boundary is multiplied with both operands
 //        into two accumulator tiles and each lane keeps its own.

@@ -382,3 +382,46 @@ def test_rope_hand_computed_two_token_case():
     want = np.zeros(16)
     want[0], want[1] = 1 - w1, w1
     assert np.allclose(out[0, 0], want, rtol=1e-13, atol=1e-15)
+
+
+# ---- NEXT-3 (latent-output mode): decode_attn_latent --------------------------------------------
+@pytest.mark.parametrize("bits", [(16, 16), (8, 4)], ids=str)
+def test_latent_output_up_projected_is_the_dense_output(bits):
+    """PAPER.md section 3.3: (p . V') . U_V = p . (V' U_V).  The latent rows times each head's slice of B_v must be the
+    output of the (pinned) decode_attn, which multiplies in the other order -- ragged lengths, quantised cache, GQA."""
+    cfg = synth.custom_config("t", 2, 8, 4, 32, 150, [8, 16, 24, 32], 48, bits=bits, page_tokens=16, outlier_frac=0.1)
+    c = build_cache(cfg, seq_lens=[150, 67])
+    bk, bv = synth.make_factors(cfg)
+    q = synth.make_q(cfg)
+    lat = oattn.decode_attn_latent(c["desc"], q, c["pool"], c["table"], c["seq_lens"], bk)
+    want = oattn.decode_attn(c["desc"], q, c["pool"], c["table"], c["seq_lens"], bk, bv)
+    assert lat.shape == (2, 8, 48)
+    bvf = bv.astype(np.float64)
+    for i in range(8):
+        g = i // 2
+        assert np.allclose(lat[:, i] @ bvf[:, g * 32:(g + 1) * 32], want[:, i], rtol=1e-11, atol=1e-13)
+
+
+def test_latent_output_of_a_zero_query_is_the_mean_latent_row():
+    """Closed form: equal scores -> uniform weights -> the mean of the cached value latents, the same row for every head."""
+    cfg = synth.custom_config("t", 1, 4, 2, 32, 90, [16, 16], 32, page_tokens=16)
+    c = build_cache(cfg)
+    bk, _ = synth.make_factors(cfg)
+    out = oattn.decode_attn_latent(c["desc"], np.zeros((1, 4, 32), np.float16), c["pool"], c["table"], c["seq_lens"], bk)
+    mean_l = c["lat"][0][1].astype(np.float64).mean(axis=0)
+    for i in range(4):
+        assert np.allclose(out[0, i], mean_l, rtol=0, atol=1e-13)
+
+
+def test_latent_output_of_a_dominant_token_is_its_latent_row_and_empty_sequences_give_zeros():
+    cfg = synth.custom_config("t", 2, 2, 1, 32, 64, [32], 32, page_tokens=16)
+    bk, _ = synth.make_factors(cfg)
+    lk, lv = synth.make_latents(cfg, 64)
+    q = synth.make_q(cfg)
+    qt = bk.astype(np.float64) @ q[0, 0].astype(np.float64)
+    lk = lk.astype(np.float64) * 0.01
+    lk[17] = 40.0 * qt / np.linalg.norm(qt)
+    c = build_cache(cfg, seq_lens=[64, 0], latents=[(lk.astype(np.float16), lv), (lk.astype(np.float16)[:0], lv[:0])])
+    out = oattn.decode_attn_latent(c["desc"], q, c["pool"], c["table"], c["seq_lens"], bk, heads=[0])
+    assert np.allclose(out[0, 0], lv[17].astype(np.float64), atol=1e-9)
+    assert not out[1].any()

@@ -379,6 +379,43 @@ def prefill_append_leg(wl, sk, torch, device, T):
     return out
 
 
+def latent_output_leg(wl, sk, torch, device, K=300):
+    """NEXT-3: decode attention alone (no append), once with the B_v up-projection (starkv_decode_attn) and once in
+    latent-output mode (starkv_decode_attn_latent: merge-only combine, o~ [batch, H_q, r_v]); one CUDA graph per cache
+    replica, K replays each, CUDA events on the workload's stream."""
+    cfg, B, R = wl.cfg, wl.cfg.batch, wl.n_rep
+    out_lat = torch.zeros((B, cfg.n_q_heads, cfg.rank_v), dtype=torch.float16, device=device)
+    calls = {
+        "decode_attn_us": lambda rep: sk.starkv_decode_attn(wl.ctx, wl.q, wl.pool, wl.table_of(rep), wl.max_pages, wl.seq_lens, B,
+                                                             wl.bk, wl.bv, wl.ws, wl.wsb, wl.out),
+        "decode_attn_latent_us": lambda rep: sk.starkv_decode_attn_latent(wl.ctx, wl.q, wl.pool, wl.table_of(rep), wl.max_pages,
+                                                                           wl.seq_lens, B, wl.bk, wl.ws, wl.wsb, out_lat),
+    }
+    res = {"calls_timed": K, "out_latent_shape": [B, cfg.n_q_heads, cfg.rank_v]}
+    with torch.cuda.stream(wl.stream):
+        for key, fn in calls.items():
+            graphs = []
+            for rep in range(R):
+                fn(rep)
+            wl.stream.synchronize()
+            for rep in range(R):
+                g = torch.cuda.CUDAGraph()
+                with torch.cuda.graph(g, stream=wl.stream):
+                    fn(rep)
+                graphs.append(g)
+            for i in range(10):
+                graphs[i % R].replay()
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record(wl.stream)
+            for i in range(K):
+                graphs[i % R].replay()
+            e1.record(wl.stream)
+            wl.stream.synchronize()
+            res[key] = e0.elapsed_time(e1) * 1e3 / K
+            del graphs
+    return res
+
+
 def workload_name(cfg) -> str:
     kind = "fp16 latents" if not cfg.quantized else f"int{cfg.bits_hi}/int{cfg.bits_lo} latents"
     return (f"{cfg.name}: BASELINE.json configs[{int(cfg.name[1]) - 1}], 1 layer, batch {cfg.batch}, "
@@ -477,6 +514,8 @@ def run_ours(args, cfg, env, K, with_cpu):
 
     # ---- C4: the compress-on-append kernel on a prefill chunk (BASELINE.json configs[3]) ----
     prefill = prefill_append_leg(wl, sk, torch, device, args.prefill_tokens) if (cfg.name == "C4" or args.prefill) else None
+    # ---- headline config: latent-output mode beside the plain decode ----
+    latent = latent_output_leg(wl, sk, torch, device) if cfg.name == HEADLINE else None
 
     # ---- clocks: if the timed loops were too short to be sampled, dwell on the same load ----
     if sampler.ok and sum(1 for s in sampler.samples if s[0]) < 8:
@@ -521,6 +560,8 @@ def run_ours(args, cfg, env, K, with_cpu):
     }
     if prefill is not None:
         line["append_prefill"] = prefill
+    if latent is not None:
+        line["latent_output"] = latent
     if world == 1 and with_cpu:
         line["cpu_baseline"] = cpu_baseline(cfg)
     return line
@@ -677,7 +718,7 @@ def summary(d):
            "roofline": {k: r[k] for k in ("kernel", "kernel_us", "achieved", "peak", "frac", "traffic", "frac_of_nominal_8TBs")},
            "e2e": {"value": d["e2e"]["value"], "ms_per_step": d["e2e"]["ms_per_step"]},
            "gpu_launches_per_step": d["gpu_launches"] // max(1, d["steps"])}
-    for k in ("append_prefill", "attention_share_model", "tokens_per_s_attn_only", "tokens_per_s_attn_only_32_layers"):
+    for k in ("append_prefill", "latent_output", "attention_share_model", "tokens_per_s_attn_only", "tokens_per_s_attn_only_32_layers"):
         if k in d:
             out[k] = d[k]
     return out

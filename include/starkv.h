@@ -135,6 +135,16 @@ int starkv_decode_attn(starkv_ctx* ctx, const void* q, const void* page_pool,
                        int batch, const void* B_k, const void* B_v, void* workspace,
                        size_t workspace_bytes, void* out);
 
+/* NEXT-3, latent-output mode: the same attention, but the result is the LATENT row
+ *   o~_i = softmax(s_i) . L_v      fp16 [batch, H_q, r_v]
+ * and the up-projection by B_v is left to an output projection with U_V absorbed (section 3.3: "(p . V') .
+ * U_V", W'_out^i = W_out^i U_V^i).  Arguments as starkv_decode_attn without B_v; same kernels up to the split-K
+ * partials, then a merge-only combine.  l = 0 gives a zero row.  Same workspace size and error codes. */
+int starkv_decode_attn_latent(starkv_ctx* ctx, const void* q, const void* page_pool,
+                              const int32_t* block_table, int max_pages, const int32_t* seq_lens,
+                              int batch, const void* B_k, void* workspace, size_t workspace_bytes,
+                              void* out_latent);
+
 /* starkv_decode_step: one whole decode step = starkv_append of ONE new token per sequence (n_new = batch, token b at
  * seq_ids[b] / positions[b]) followed by starkv_decode_attn over seq_lens (which already count the new token), with
  * the same arguments, meanings and results as those two calls made back to back on the context's stream -- the cache

@@ -22,7 +22,7 @@ LIB_PATH = os.path.join(_HERE, "libstarkv.so")
 SYMBOLS = [
     "starkv_create", "starkv_destroy", "starkv_page_bytes", "starkv_workspace_bytes",
     "starkv_append_workspace_bytes", "starkv_pack", "starkv_unpack", "starkv_append",
-    "starkv_decode_attn", "starkv_decode_step", "starkv_decode_attn_static", "starkv_decode_attn_generic", "starkv_decode_attn_rope", "starkv_decode_attn_host",
+    "starkv_decode_attn", "starkv_decode_attn_latent", "starkv_decode_step", "starkv_decode_attn_static", "starkv_decode_attn_generic", "starkv_decode_attn_rope", "starkv_decode_attn_host",
     "starkv_append_host_workspace_bytes", "starkv_append_host", "starkv_set_kernel_timing",
     "starkv_last_decode_kernel_ms",
     "starkv_set_splits", "starkv_set_option", "starkv_last_launches", "starkv_decode_kernel_name", "starkv_last_append_kernel_name", "starkv_strerror",
@@ -82,6 +82,8 @@ def _load() -> ctypes.CDLL:
     lib.starkv_decode_step.argtypes = [vp, vp, i32p, c_int, i32p, i32p, c_int, vp, c_i64, c_i64, c_int, vp, c_i64, c_int, vp, vp,
                                        vp, c_sz, vp, i32p, vp, vp, vp, c_sz, vp]
     lib.starkv_decode_step.restype = c_int
+    lib.starkv_decode_attn_latent.argtypes = [vp, vp, vp, i32p, c_int, i32p, c_int, vp, vp, c_sz, vp]
+    lib.starkv_decode_attn_latent.restype = c_int
     lib.starkv_decode_attn_static.argtypes = [vp, vp, vp, i32p, c_int, i32p, c_int, vp, vp, vp]
     lib.starkv_decode_attn_static.restype = c_int
     for name in ("starkv_decode_attn", "starkv_decode_attn_generic", "starkv_decode_attn_host"):
@@ -221,6 +223,14 @@ def starkv_decode_step(ctx, page_pool, block_table, max_pages, seq_ids, position
                                        v_row_stride, d_in_v, _ptr(A_k), _ptr(A_v), _ptr(append_workspace),
                                        append_workspace_bytes, _ptr(q), _ptr(seq_lens), _ptr(B_k), _ptr(B_v),
                                        _ptr(workspace), workspace_bytes, _ptr(out)))
+
+
+def starkv_decode_attn_latent(ctx, q, page_pool, block_table, max_pages, seq_lens, batch, B_k, workspace, workspace_bytes,
+                              out_latent) -> None:
+    """Latent-output mode: out_latent fp16 [batch, H_q, r_v] = softmax(s) . L_v (no B_v up-projection)."""
+    ctx._check(_lib.starkv_decode_attn_latent(ctx.handle, _ptr(q), _ptr(page_pool), _ptr(block_table), max_pages,
+                                              _ptr(seq_lens), batch, _ptr(B_k), _ptr(workspace), workspace_bytes,
+                                              _ptr(out_latent)))
 
 
 STATIC_SCRATCH_BYTES = 8 << 20   # include/starkv.h STARKV_STATIC_SCRATCH_BYTES

@@ -187,6 +187,19 @@ int starkv_decode_attn(starkv_ctx* ctx, const void* q, const void* pool, const i
   }
 }
 
+int starkv_decode_attn_latent(starkv_ctx* ctx, const void* q, const void* pool, const int32_t* table, int max_pages,
+                              const int32_t* seq_lens, int batch, const void* B_k, void* ws, size_t ws_bytes, void* out_latent) {
+  // B_k stands in for B_v in the shared argument check (latent-output mode has no B_v); a null B_v selects the
+  // merge-only combine in sk_launch_combine
+  const int rc = check_decode_args(ctx, q, pool, table, max_pages, seq_lens, batch, B_k, B_k, ws, out_latent);
+  if (rc) return rc;
+  switch (sk_decode_choice(ctx)) {
+    case SK_VARIANT_TM: return sk_decode_tm(ctx, q, pool, table, max_pages, seq_lens, batch, B_k, nullptr, ws, ws_bytes, out_latent);
+    case SK_VARIANT_GENERIC: return sk_decode_generic(ctx, q, pool, table, max_pages, seq_lens, batch, B_k, nullptr, ws, ws_bytes, out_latent);
+    default: return sk_decode_fast(ctx, q, pool, table, max_pages, seq_lens, batch, B_k, nullptr, ws, ws_bytes, out_latent);
+  }
+}
+
 int starkv_decode_step(starkv_ctx* ctx, void* pool, const int32_t* table, int max_pages, const int32_t* seq_ids,
                        const int32_t* positions, int batch, const void* k_new, int64_t k_row_stride, int64_t k_head_stride,
                        int d_in_k, const void* v_new, int64_t v_row_stride, int d_in_v, const void* A_k, const void* A_v,

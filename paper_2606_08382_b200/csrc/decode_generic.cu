@@ -505,11 +505,148 @@ __global__ void __launch_bounds__(CS_THREADS) combine_sliced_kernel(const __grid
   }
 }
 
+// ---------------------------------------------------------------------------------------------
+// D8 alone, latent-output mode (NEXT-3; section 3.3: the attention emits p . V' and an output projection with
+// U_V absorbed consumes it): LSE merge of the split partials, normalise, write o~ fp16 [batch][H_q][r_v].  No B_v.
+// grid (H_q, slices of 64 channels, batch), 256 threads = 64 channels x 4 groups of splits.
+// ---------------------------------------------------------------------------------------------
+constexpr int CL_CH = 64, CL_SG = 4, CL_THREADS = CL_CH * CL_SG;
+__global__ void __launch_bounds__(CL_THREADS) combine_latent_kernel(const __grid_constant__ StarkvLayout L,
+                                                                    const float* __restrict__ parts, int n_splits,
+                                                                    __half* __restrict__ out) {
+  __shared__ float wsm[512];
+  __shared__ float rsm[CL_THREADS / 32];
+  __shared__ float red[CL_SG][CL_CH];
+  sk_pdl_enter();
+  const int head = blockIdx.x, c0 = blockIdx.y * CL_CH, b = blockIdx.z;
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, ch = tid % CL_CH, sg = tid / CL_CH;
+  const size_t ps = sk_part_stride(L.rank_v);
+  const float* base = parts + ((size_t)b * n_splits * L.n_q_heads + head) * ps;
+  const size_t sstride = (size_t)L.n_q_heads * ps;
+  float mx = -INFINITY;
+  for (int s = tid; s < n_splits; s += CL_THREADS) mx = fmaxf(mx, base[s * sstride]);
+#pragma unroll
+  for (int o = 16; o; o >>= 1) mx = fmaxf(mx, __shfl_xor_sync(0xffffffffu, mx, o));
+  if (lane == 0) rsm[warp] = mx;
+  __syncthreads();
+  float mstar = rsm[0];
+#pragma unroll
+  for (int i = 1; i < CL_THREADS / 32; ++i) mstar = fmaxf(mstar, rsm[i]);
+  float lstar = 0.f, acc = 0.f;
+  const bool ok = c0 + ch < L.rank_v;
+  for (int s0 = 0; s0 < n_splits; s0 += 512) {   // weights staged in chunks of 512 splits
+    const int ns = min(512, n_splits - s0);
+    __syncthreads();
+    float lp = 0.f;
+    for (int s = tid; s < ns; s += CL_THREADS) {
+      const float m = base[(s0 + s) * sstride];
+      const float w = (m == -INFINITY) ? 0.f : exp2f(m - mstar);
+      wsm[s] = w;
+      lp = fmaf(w, base[(s0 + s) * sstride + 1], lp);
+    }
+#pragma unroll
+    for (int o = 16; o; o >>= 1) lp += __shfl_xor_sync(0xffffffffu, lp, o);
+    if (lane == 0) rsm[warp] = lp;
+    __syncthreads();
+#pragma unroll
+    for (int i = 0; i < CL_THREADS / 32; ++i) lstar += rsm[i];
+    if (ok) {
+      const float* col = base + (size_t)s0 * sstride + SK_PART_ACC + c0 + ch;
+#pragma unroll 4
+      for (int s = sg; s < ns; s += CL_SG) acc = fmaf(wsm[s], col[s * sstride], acc);
+    }
+  }
+  red[sg][ch] = acc;
+  __syncthreads();
+  if (sg == 0 && ok) {
+    const float inv = (mstar == -INFINITY || lstar == 0.f) ? 0.f : 1.f / lstar;   // empty sequence: a zero row
+    const float o = (red[0][ch] + red[1][ch]) + (red[2][ch] + red[3][ch]);
+    out[((size_t)b * L.n_q_heads + head) * L.rank_v + c0 + ch] = __float2half_rn(o * inv);
+  }
+}
+
+// The same for n_splits <= 512, in the style of combine_sliced_kernel: one (head, slice of 32 channels, sequence) per
+// block, 32 channels x 8 split groups, every load that depends on nothing issued before the first reduction.
+__global__ void __launch_bounds__(CS_THREADS) combine_latent_sliced_kernel(const __grid_constant__ StarkvLayout L,
+                                                                          const float* __restrict__ parts, int n_splits,
+                                                                          __half* __restrict__ out) {
+  __shared__ float wsm[512];
+  __shared__ float osum[CS_SG][CS_CH];
+  __shared__ float rsm[16];
+  const int head = blockIdx.x, sl = blockIdx.y, b = blockIdx.z, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  sk_pdl_enter();
+  const int rv = L.rank_v;
+  const size_t ps = sk_part_stride(rv);
+  const float* base = parts + ((size_t)b * n_splits * L.n_q_heads + head) * ps;
+  const size_t sstride = (size_t)L.n_q_heads * ps;
+  float2 ml0 = make_float2(-INFINITY, 0.f), ml1 = make_float2(-INFINITY, 0.f);
+  if (tid < n_splits) ml0 = *reinterpret_cast<const float2*>(base + (size_t)tid * sstride);
+  if (tid + CS_THREADS < n_splits) ml1 = *reinterpret_cast<const float2*>(base + (size_t)(tid + CS_THREADS) * sstride);
+  const int c = tid & (CS_CH - 1), sg = tid >> 5;   // channel of the slice, split group
+  const int ch = sl * CS_CH + c;
+  const float* col = base + SK_PART_ACC + ch;
+  float v[CS_PF];
+#pragma unroll
+  for (int k = 0; k < CS_PF; ++k) {
+    const int s = sg + CS_SG * k;
+    v[k] = (ch < rv && s < n_splits) ? col[(size_t)s * sstride] : 0.f;
+  }
+  float mx = fmaxf(ml0.x, ml1.x);
+#pragma unroll
+  for (int o = 16; o; o >>= 1) mx = fmaxf(mx, __shfl_xor_sync(0xffffffffu, mx, o));
+  if (lane == 0) rsm[warp] = mx;
+  __syncthreads();
+  float mstar = rsm[0];
+#pragma unroll
+  for (int i = 1; i < CS_THREADS / 32; ++i) mstar = fmaxf(mstar, rsm[i]);
+  const float w0 = ml0.x == -INFINITY ? 0.f : exp2f(ml0.x - mstar);
+  const float w1 = ml1.x == -INFINITY ? 0.f : exp2f(ml1.x - mstar);
+  wsm[tid] = w0;
+  wsm[tid + CS_THREADS] = w1;
+  float lp = w0 * ml0.y + w1 * ml1.y;
+#pragma unroll
+  for (int o = 16; o; o >>= 1) lp += __shfl_xor_sync(0xffffffffu, lp, o);
+  if (lane == 0) rsm[8 + warp] = lp;
+  __syncthreads();
+  float lstar = 0.f;
+#pragma unroll
+  for (int i = 0; i < CS_THREADS / 32; ++i) lstar += rsm[8 + i];
+  const float inv = (mstar == -INFINITY || lstar == 0.f) ? 0.f : 1.f / lstar;   // empty sequence: a zero row
+  float a0 = 0.f, a1 = 0.f;   // (wsm is 0 past n_splits: neutral)
+#pragma unroll
+  for (int k = 0; k < CS_PF; k += 2) {
+    a0 = fmaf(wsm[sg + CS_SG * k], v[k], a0);
+    a1 = fmaf(wsm[sg + CS_SG * (k + 1)], v[k + 1], a1);
+  }
+  if (ch < rv)
+    for (int s = sg + CS_SG * CS_PF; s < n_splits; s += CS_SG) a0 = fmaf(wsm[s], col[(size_t)s * sstride], a0);
+  osum[sg][c] = a0 + a1;
+  __syncthreads();
+  if (tid < CS_CH && sl * CS_CH + tid < rv) {
+    float o = 0.f;
+#pragma unroll
+    for (int k = 0; k < CS_SG; ++k) o += osum[k][tid];
+    out[((size_t)b * L.n_q_heads + head) * rv + sl * CS_CH + tid] = __float2half_rn(o * inv);
+  }
+}
+
 }  // namespace
 
 int sk_launch_combine(starkv_ctx* ctx, const float* parts, int n_splits, int batch, const void* B_v, void* out,
                       float* pslice) {
   const StarkvLayout& L = ctx->L;
+  if (!B_v && n_splits <= 512) {   // latent-output mode (starkv_decode_attn_latent): merge and normalise only
+    SK_PREFER_SMEM(ctx, combine_latent_sliced_kernel);
+    SK_CUDA_CHECK(ctx, sk_launch(ctx, combine_latent_sliced_kernel, dim3(L.n_q_heads, (L.rank_v + CS_CH - 1) / CS_CH, batch),
+                                 dim3(CS_THREADS), 0, L, parts, n_splits, (__half*)out));
+    return STARKV_OK;
+  }
+  if (!B_v) {
+    SK_PREFER_SMEM(ctx, combine_latent_kernel);
+    SK_CUDA_CHECK(ctx, sk_launch(ctx, combine_latent_kernel, dim3(L.n_q_heads, (L.rank_v + CL_CH - 1) / CL_CH, batch), dim3(CL_THREADS),
+                                 0, L, parts, n_splits, (__half*)out));
+    return STARKV_OK;
+  }
   const int nsl = (L.rank_v + CS_CH - 1) / CS_CH;
   // sliced combine where one block per head would be the long pole: few sequences, many splits
   // (measured: C3, 148 splits x 1 sequence: step 57.6 -> 53.2 us; C2, 37 splits x 4 sequences: 50.0 -> 54.1 us)

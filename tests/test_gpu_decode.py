@@ -490,3 +490,60 @@ def test_paper_sized_value_rank_and_wide_gqa(bits):
     _check(gqa, seq_lens=[900, 515])
     _check(gqa, seq_lens=[900, 515], regime="peaky")
     assert err <= TOL
+
+
+@pytest.mark.parametrize("name,ctxlen,lens", [("C3", 3000, [3000, 1777, 0]), ("C2", 1500, [1500, 64, 999]), ("C1", 512, [512]),
+                                              ("C4", 900, [900, 333]), ("C5", 2000, [1, 2000])])
+def test_latent_output_mode_against_the_oracle(name, ctxlen, lens):
+    """NEXT-3: starkv_decode_attn_latent emits o~ = softmax(s) . L_v [batch, H_q, r_v] (section 3.3) on the same
+    kernels as starkv_decode_attn up to the split-K partials; held to oracle.attention.decode_attn_latent on the TMEM-operand
+    kernel (C3, C5), the mma.sync kernel (C2, C4) and C1's shape, ragged lengths, a one-token and an empty sequence.
+    Same bar (row-relative 2e-3, rows of r_v channels)."""
+    from tests.gpu_util import dev, f16
+    batch = len(lens)
+    cfg = synth.make_config(name, context=ctxlen, batch=batch)
+    cache = build_cache(cfg, seq_lens=lens)
+    bk, _ = synth.make_factors(cfg)
+    q = synth.make_q(cfg, batch=batch)
+    ref = oattn.decode_attn_latent(cache["desc"], q, cache["pool"], cache["table"], cache["seq_lens"], bk)
+    ctx = sk.create_from_config(cfg)
+    table = dev(cache["table"].astype(np.int32))
+    mp = table.shape[1]
+    wsb = sk.starkv_workspace_bytes(ctx, batch, mp)
+    ws = torch.empty(wsb, dtype=torch.uint8, device="cuda")
+    out = torch.full((batch, cfg.n_q_heads, cfg.rank_v), float("nan"), dtype=torch.float16, device="cuda")
+    sk.starkv_decode_attn_latent(ctx, f16(q), dev(cache["pool"]), table, mp, dev(np.asarray(cache["seq_lens"], np.int32)), batch,
+                                 f16(bk), ws, wsb, out)
+    torch.cuda.synchronize()
+    got = out.double().cpu().numpy()
+    assert np.isfinite(got).all()
+    for b, l in enumerate(lens):
+        if l == 0:
+            assert not got[b].any()
+    keep = [b for b, l in enumerate(lens) if l > 0]
+    err = row_rel_err(got[keep], ref[keep])
+    assert err <= TOL, f"{name}: row rel err {err:.3e}"
+
+
+def test_latent_output_mode_with_more_than_512_splits():
+    """The merge-only combine has a sliced form for up to 512 splits and a chunked one above; 560 splits forced here."""
+    from tests.gpu_util import dev, f16
+    cfg = synth.make_config("C3", context=36000, batch=1)
+    cache = build_cache(cfg, seq_lens=[36000])
+    bk, _ = synth.make_factors(cfg)
+    q = synth.make_q(cfg, batch=1)
+    heads = [0, 13, 31]
+    ref = oattn.decode_attn_latent(cache["desc"], q, cache["pool"], cache["table"], cache["seq_lens"], bk, heads=heads)
+    ctx = sk.create_from_config(cfg)
+    sk.starkv_set_splits(ctx, 560)
+    table = dev(cache["table"].astype(np.int32))
+    mp = table.shape[1]
+    wsb = sk.starkv_workspace_bytes(ctx, 1, mp)
+    ws = torch.empty(wsb, dtype=torch.uint8, device="cuda")
+    out = torch.full((1, cfg.n_q_heads, cfg.rank_v), float("nan"), dtype=torch.float16, device="cuda")
+    sk.starkv_decode_attn_latent(ctx, f16(q), dev(cache["pool"]), table, mp, dev(np.asarray([36000], np.int32)), 1, f16(bk), ws, wsb, out)
+    torch.cuda.synchronize()
+    got = out.double().cpu().numpy()
+    assert np.isfinite(got).all()
+    err = row_rel_err(got[:, heads], ref[:, heads])
+    assert err <= TOL, f"row rel err {err:.3e}"

@@ -130,3 +130,39 @@ def test_two_rank_gloo_sharding_and_max_timing():
         assert p.exitcode == 0
     assert res[0][1] == (0, 5) and res[1][1] == (5, 9)
     assert res[0][2] == res[1][2] == 11.0
+
+
+def test_bench_reference_arm_prints_the_contract_line():
+    """`bench.py --impl reference` times the CPU oracle (no GPU needed) and must print ONE JSON line with the contract's
+    keys: same metric / unit / config as our arm, `impl`, a `cpu_baseline` describing the run and an `e2e` that repeats
+    the line's value with zero copied bytes."""
+    import json
+    import subprocess
+    import sys
+    r = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--impl", "reference", "--steps", "1", "--warmup", "0"],
+                       capture_output=True, text=True, timeout=600, cwd=ROOT)
+    assert r.returncode == 0, r.stderr[-2000:]
+    lines = [l for l in r.stdout.strip().splitlines() if l.startswith("{")]
+    assert len(lines) == 1
+    d = json.loads(lines[0])
+    assert d["impl"] == "reference" and d["metric"] == "decode_attn_latent_kv_hbm_gbs" and d["unit"] == "GB/s"
+    assert d["higher_is_better"] is True and d["n_gpus"] == 1 and d["steps"] == 1 and d["vs_baseline"] is None
+    assert d["config"]["workload"].startswith("C3") and d["data"] == "synthetic" and d["dtype"] == "f64"
+    assert d["value"] > 0 and d["ms_per_step"] > 0
+    cb = d["cpu_baseline"]
+    assert cb["kind"] == "oracle" and cb["cores"] >= 1 and cb["sample"] and cb["value"] == d["value"]
+    e = d["e2e"]
+    assert e["value"] == d["value"] and e["unit"] == d["unit"] and e["h2d_bytes_per_step"] == 0 and e["d2h_bytes_per_step"] == 0
+
+
+def test_bench_our_arm_fails_loudly_without_a_device():
+    """Our arm has no CPU fallback: without a CUDA device it must exit non-zero instead of printing a number."""
+    import subprocess
+    import sys
+    import torch
+    if torch.cuda.is_available():
+        pytest.skip("a GPU is present")
+    r = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--workload", "C3", "--steps", "1", "--warmup", "0", "--no-cpu"],
+                       capture_output=True, text=True, timeout=600, cwd=ROOT)
+    assert r.returncode != 0
+    assert not [l for l in r.stdout.strip().splitlines() if l.startswith("{") and '"value"' in l]

@@ -223,13 +223,12 @@ class Workload:
         self.launches_per_step = sk.starkv_last_launches(self.ctx)
 
     def step_host(self, rep):
-        """Same step through the HOST-buffer entry points; returns after `out` is back on the host."""
+        """Same step through the HOST-buffer entry point (starkv_decode_step_host); returns after `out` is back on the host."""
         sk, c, B = self.sk, self.cfg, self.cfg.batch
-        sk.starkv_append_host(self.ctx, self.pool, self.table_of(rep), self.max_pages, self.h_seq, self.h_pos, B,
-                              self.h_k, c.n_kv_heads * c.head_dim, c.head_dim, self.d_in_k, self.h_v, self.d_in_v,
-                              self.d_in_v, self.ak, self.av, self.aws, self.awsb)
-        sk.starkv_decode_attn_host(self.ctx, self.h_q, self.pool, self.table_of(rep), self.max_pages, self.h_lens, B,
-                                   self.bk, self.bv, self.ws, self.wsb, self.h_out)
+        sk.starkv_decode_step_host(self.ctx, self.pool, self.table_of(rep), self.max_pages, self.h_seq, self.h_pos, B,
+                                   self.h_k, c.n_kv_heads * c.head_dim, c.head_dim, self.d_in_k, self.h_v, self.d_in_v,
+                                   self.d_in_v, self.ak, self.av, self.aws, self.awsb, self.h_q, self.h_lens, self.bk, self.bv,
+                                   self.ws, self.wsb, self.h_out)
 
     def h2d_bytes(self):
         return int(self.h_q.numel() * 2 + self.h_k.numel() * 2 + self.h_v.numel() * 2 + 3 * self.cfg.batch * 4)

@@ -222,8 +222,8 @@ int starkv_decode_attn_host(starkv_ctx* ctx, const void* q_host, const void* pag
  * v_new_host [n_new, v_row_elems] fp16, seq_ids_host / positions_host int32 [n_new] are HOST
  * pointers (pinned for best speed); strides are the row element counts (k_row_stride =
  * k_row_elems, v_row_stride = v_row_elems).  In hidden mode pass v_new_host == k_new_host (copied
- * once).  The call copies them into `workspace` (sized by starkv_append_host_workspace_bytes) and
- * enqueues the append; it does NOT synchronise (copies and kernels are ordered on the stream;
+ * once).  The call copies them into `workspace` (sized by starkv_append_host_workspace_bytes, which
+ * also leaves room for the q and seq_lens of starkv_decode_step_host) and enqueues the append; it does NOT synchronise (copies and kernels are ordered on the stream;
  * the host buffers must stay unchanged until the stream reaches the end of the call). */
 size_t starkv_append_host_workspace_bytes(const starkv_ctx* ctx, int n_new, int k_row_elems,
                                           int v_row_elems);
@@ -232,6 +232,26 @@ int starkv_append_host(starkv_ctx* ctx, void* page_pool, const int32_t* block_ta
                        const void* k_new_host, int k_row_elems, int64_t k_head_stride, int d_in_k,
                        const void* v_new_host, int v_row_elems, int d_in_v, const void* A_k,
                        const void* A_v, void* workspace, size_t workspace_bytes);
+
+/* starkv_decode_step with HOST buffers (bench.py "e2e"): starkv_append_host of one new token per sequence followed by
+ * starkv_decode_attn_host, as ONE call.  The host inputs of both are gathered in one page-locked block the context owns
+ * and reach the device in ONE copy (into the staging area behind the projection scratch of `append_workspace`, which
+ * starkv_append_host_workspace_bytes sizes for k_new, v_new, seq_ids, positions, q and seq_lens of `batch` sequences);
+ * then the launch-fused step; the result is written by the last kernel directly into page-locked host memory -- into
+ * `out_host` itself when that is page-locked (cudaHostAlloc / cudaHostRegister, 16-byte aligned), else into the
+ * context's block and copied from there -- so there is no device-to-host copy; one stream synchronisation ends the call.
+ * *_host arguments are HOST pointers, read before the call returns; out_host is complete when it returns.  The cache,
+ * block table and factors stay on the device.  append_workspace >= starkv_append_host_workspace_bytes(ctx, batch,
+ * k_row_elems, v_row_elems), workspace >= starkv_workspace_bytes(ctx, batch, max_pages), both DEVICE memory.  Same
+ * results (bit for bit) and error codes as the two calls; on the default / legacy stream, under capture, with kernel
+ * timing on or for batch > 64 it simply makes them. */
+int starkv_decode_step_host(starkv_ctx* ctx, void* page_pool, const int32_t* block_table, int max_pages,
+                            const int32_t* seq_ids_host, const int32_t* positions_host, int batch,
+                            const void* k_new_host, int k_row_elems, int64_t k_head_stride, int d_in_k,
+                            const void* v_new_host, int v_row_elems, int d_in_v, const void* A_k,
+                            const void* A_v, void* append_workspace, size_t append_workspace_bytes,
+                            const void* q_host, const int32_t* seq_lens_host, const void* B_k,
+                            const void* B_v, void* workspace, size_t workspace_bytes, void* out_host);
 
 /* Kernel timing (bench.py "roofline"): when on, the decode calls record CUDA events on the
  * context's stream directly before and after the main split-K kernel (rows D2-D7).

@@ -23,7 +23,7 @@ SYMBOLS = [
     "starkv_create", "starkv_destroy", "starkv_page_bytes", "starkv_workspace_bytes",
     "starkv_append_workspace_bytes", "starkv_pack", "starkv_unpack", "starkv_append",
     "starkv_decode_attn", "starkv_decode_attn_latent", "starkv_decode_step", "starkv_decode_attn_static", "starkv_decode_attn_generic", "starkv_decode_attn_rope", "starkv_decode_attn_host",
-    "starkv_append_host_workspace_bytes", "starkv_append_host", "starkv_set_kernel_timing",
+    "starkv_append_host_workspace_bytes", "starkv_append_host", "starkv_decode_step_host", "starkv_set_kernel_timing",
     "starkv_last_decode_kernel_ms",
     "starkv_set_splits", "starkv_set_option", "starkv_last_launches", "starkv_decode_kernel_name", "starkv_last_append_kernel_name", "starkv_strerror",
     "starkv_last_error",
@@ -94,6 +94,9 @@ def _load() -> ctypes.CDLL:
     lib.starkv_append_host.argtypes = [vp, vp, i32p, c_int, i32p, i32p, c_int, vp, c_int, c_i64, c_int, vp, c_int,
                                        c_int, vp, vp, vp, c_sz]
     lib.starkv_append_host.restype = c_int
+    lib.starkv_decode_step_host.argtypes = [vp, vp, i32p, c_int, i32p, i32p, c_int, vp, c_int, c_i64, c_int, vp, c_int, c_int, vp, vp,
+                                            vp, c_sz, vp, i32p, vp, vp, vp, c_sz, vp]
+    lib.starkv_decode_step_host.restype = c_int
     lib.starkv_set_kernel_timing.argtypes = [vp, c_int]
     lib.starkv_set_kernel_timing.restype = c_int
     lib.starkv_last_decode_kernel_ms.argtypes = [vp, ctypes.POINTER(ctypes.c_float)]
@@ -118,13 +121,20 @@ def _load() -> ctypes.CDLL:
 _lib = _load()
 
 
+_PTR_OF = {}   # type -> its unbound data_ptr, filled on first sight (the common case, once per argument per call)
+
+
 def _ptr(x) -> Optional[int]:
     """Device/host pointer of a torch tensor, numpy array, int or None."""
+    f = _PTR_OF.get(type(x))
+    if f is not None:
+        return f(x)
     if x is None:
         return None
     if isinstance(x, int):
         return x
     if hasattr(x, "data_ptr"):
+        _PTR_OF[type(x)] = type(x).data_ptr
         return x.data_ptr()
     if hasattr(x, "ctypes"):
         return x.ctypes.data
@@ -264,6 +274,16 @@ def starkv_decode_attn_host(ctx, q_host, page_pool, block_table, max_pages, seq_
                             workspace, workspace_bytes, out_host) -> None:
     _decode(_lib.starkv_decode_attn_host, ctx, q_host, page_pool, block_table, max_pages, seq_lens_host, batch,
             B_k, B_v, workspace, workspace_bytes, out_host)
+
+
+def starkv_decode_step_host(ctx, page_pool, block_table, max_pages, seq_ids_host, positions_host, batch, k_new_host, k_row_elems,
+                            k_head_stride, d_in_k, v_new_host, v_row_elems, d_in_v, A_k, A_v, append_workspace,
+                            append_workspace_bytes, q_host, seq_lens_host, B_k, B_v, workspace, workspace_bytes, out_host) -> None:
+    ctx._check(_lib.starkv_decode_step_host(ctx.handle, _ptr(page_pool), _ptr(block_table), max_pages, _ptr(seq_ids_host),
+                                            _ptr(positions_host), batch, _ptr(k_new_host), k_row_elems, k_head_stride, d_in_k,
+                                            _ptr(v_new_host), v_row_elems, d_in_v, _ptr(A_k), _ptr(A_v), _ptr(append_workspace),
+                                            append_workspace_bytes, _ptr(q_host), _ptr(seq_lens_host), _ptr(B_k), _ptr(B_v),
+                                            _ptr(workspace), workspace_bytes, _ptr(out_host)))
 
 
 def starkv_append_host_workspace_bytes(ctx: Context, n_new: int, k_row_elems: int, v_row_elems: int) -> int:

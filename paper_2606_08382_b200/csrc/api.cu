@@ -344,8 +344,11 @@ int starkv_decode_attn_host(starkv_ctx* ctx, const void* q_host, const void* poo
 size_t starkv_append_host_workspace_bytes(const starkv_ctx* ctx, int n_new, int k_row_elems, int v_row_elems) {
   if (!ctx || n_new <= 0 || k_row_elems < 0 || v_row_elems < 0) return 0;
   const size_t up = 255;
+  // projection scratch, then staging for [k_new][v_new][seq_ids][positions] and -- starkv_decode_step_host only --
+  // [q][seq_lens] for n_new sequences, so that one copy brings a whole step's inputs
+  const size_t qb = ((size_t)n_new * ctx->L.n_q_heads * ctx->L.head_dim * 2 + up) & ~up;
   return sk_append_ws_bytes(ctx, n_new) + (((size_t)n_new * k_row_elems * 2 + up) & ~up) +
-         (((size_t)n_new * v_row_elems * 2 + up) & ~up) + 2 * (((size_t)n_new * 4 + up) & ~up);
+         (((size_t)n_new * v_row_elems * 2 + up) & ~up) + 3 * (((size_t)n_new * 4 + up) & ~up) + qb;
 }
 
 // enqueue-only body shared by the direct and the captured path
@@ -447,6 +450,91 @@ int starkv_append_host(starkv_ctx* ctx, void* pool, const int32_t* table, int ma
   SK_CUDA_CHECK(ctx, cudaGraphLaunch(hg->exec, ctx->stream));
   SK_CUDA_CHECK(ctx, cudaEventRecord(ctx->pin_free, ctx->stream));
   ctx->pin_busy = 1;
+  return STARKV_OK;
+}
+
+// One whole decode step from HOST buffers: the inputs of the append and of the decode travel in one pinned block (two
+// host-to-device copies, one per device staging area), then starkv_decode_step, one device-to-host copy, one
+// synchronisation.  Against starkv_append_host + starkv_decode_attn_host it saves two kernel launches, an event
+// hand-shake and a call.
+int starkv_decode_step_host(starkv_ctx* ctx, void* pool, const int32_t* table, int max_pages, const int32_t* seq_ids_host,
+                            const int32_t* positions_host, int batch, const void* k_new_host, int k_row_elems,
+                            int64_t k_head_stride, int d_in_k, const void* v_new_host, int v_row_elems, int d_in_v,
+                            const void* A_k, const void* A_v, void* append_ws, size_t append_ws_bytes, const void* q_host,
+                            const int32_t* seq_lens_host, const void* B_k, const void* B_v, void* ws, size_t ws_bytes,
+                            void* out_host) {
+  if (!ctx || batch <= 0 || max_pages <= 0 || !sk_device_ok(ctx)) return STARKV_ERR_INVALID_ARG;
+  if (!seq_ids_host || !positions_host || !k_new_host || !v_new_host || !q_host || !seq_lens_host || !out_host || !append_ws ||
+      !ws || !aligned16(append_ws) || !aligned16(ws) || k_row_elems <= 0 || v_row_elems <= 0)
+    return STARKV_ERR_INVALID_ARG;
+  if (append_ws_bytes < starkv_append_host_workspace_bytes(ctx, batch, k_row_elems, v_row_elems)) return STARKV_ERR_WORKSPACE;
+  SkWorkspace w;
+  sk_plan_workspace(ctx, batch, max_pages, &w);
+  if (ws_bytes < w.total) return STARKV_ERR_WORKSPACE;
+  const size_t up = 255;
+  const size_t kb = (size_t)batch * k_row_elems * 2, vb = (size_t)batch * v_row_elems * 2, ib = (size_t)batch * 4;
+  const bool same = v_new_host == k_new_host;
+  const size_t kbp = (kb + up) & ~up, vbp = same ? 0 : ((vb + up) & ~up), ibp = (ib + up) & ~up;
+  const size_t qbytes = (size_t)batch * ctx->L.n_q_heads * ctx->L.head_dim * 2;
+  const size_t qb = (qbytes + up) & ~up, lb = ibp;
+  const size_t app_bytes = kbp + vbp + 2 * ibp, need = app_bytes + 2 * qb + lb;
+  if (batch > 64 || need > ((size_t)4 << 20) || ctx->stream == nullptr || ctx->stream == cudaStreamLegacy ||
+      ctx->stream == cudaStreamPerThread || ctx->timing_on || sk_stream_capturing(ctx)) {
+    // (the pinned staging is for a stream of the caller's own; elsewhere: the two calls)
+    const int rc = starkv_append_host(ctx, pool, table, max_pages, seq_ids_host, positions_host, batch, k_new_host, k_row_elems,
+                                      k_head_stride, d_in_k, v_new_host, v_row_elems, d_in_v, A_k, A_v, append_ws, append_ws_bytes);
+    if (rc) return rc;
+    return starkv_decode_attn_host(ctx, q_host, pool, table, max_pages, seq_lens_host, batch, B_k, B_v, ws, ws_bytes, out_host);
+  }
+  if (ctx->pin_busy) {   // an earlier starkv_append_host may still be reading the block
+    SK_CUDA_CHECK(ctx, cudaEventSynchronize(ctx->pin_free));
+    ctx->pin_busy = 0;
+  }
+  {
+    const int rc = sk_pin_reserve(ctx, &ctx->pin2, &ctx->pin2_bytes, need, ctx->g_app);
+    if (rc) return rc;
+  }
+  // pinned block: [k][v][seq_ids][positions] | [q][seq_lens] | [out]
+  uint8_t* pk = (uint8_t*)ctx->pin2;
+  uint8_t* pv = same ? pk : pk + kbp;
+  uint8_t* pseq = pk + kbp + vbp;
+  uint8_t* ppos = pseq + ibp;
+  uint8_t* pq = pk + app_bytes;
+  uint8_t* plen = pq + qb;
+  uint8_t* pout = plen + lb;
+  memcpy(pk, k_new_host, kb);
+  if (!same) memcpy(pv, v_new_host, vb);
+  memcpy(pseq, seq_ids_host, ib);
+  memcpy(ppos, positions_host, ib);
+  memcpy(pq, q_host, qbytes);
+  memcpy(plen, seq_lens_host, ib);
+  // device staging, same layout, behind the projection scratch of the append workspace: ONE copy brings the step's inputs.
+  // The result is written by the combine kernel straight into the pinned block (cudaHostAlloc memory is mapped into the
+  // device's address space under unified addressing; posted writes, visible to the host once the stream has drained), so
+  // there is no copy back.
+  const size_t zb = sk_append_ws_bytes(ctx, batch);
+  uint8_t* dk = (uint8_t*)append_ws + zb;
+  uint8_t* dv = same ? dk : dk + kbp;
+  int32_t* dseq = (int32_t*)(dk + kbp + vbp);
+  int32_t* dpos = (int32_t*)((uint8_t*)dseq + ibp);
+  uint8_t* dq = dk + app_bytes;
+  int32_t* dlen = (int32_t*)(dq + qb);
+  // ... and where the caller's own `out_host` is page-locked (and so mapped), straight into it: no host copy either
+  void* out_dev = pout;
+  {
+    cudaPointerAttributes at;
+    if (cudaPointerGetAttributes(&at, out_host) == cudaSuccess) {
+      if (at.type == cudaMemoryTypeHost && at.devicePointer && aligned16(at.devicePointer)) out_dev = at.devicePointer;
+    } else {
+      (void)cudaGetLastError();
+    }
+  }
+  SK_CUDA_CHECK(ctx, cudaMemcpyAsync(dk, pk, app_bytes + qb + ib, cudaMemcpyHostToDevice, ctx->stream));
+  const int rc = starkv_decode_step(ctx, pool, table, max_pages, dseq, dpos, batch, dk, k_row_elems, k_head_stride, d_in_k, dv,
+                                    v_row_elems, d_in_v, A_k, A_v, append_ws, zb, dq, dlen, B_k, B_v, ws, ws_bytes, out_dev);
+  if (rc) return rc;
+  SK_CUDA_CHECK(ctx, cudaStreamSynchronize(ctx->stream));
+  if (out_dev == pout) memcpy(out_host, pout, qbytes);
   return STARKV_OK;
 }
 

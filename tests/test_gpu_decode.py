@@ -547,3 +547,58 @@ def test_latent_output_mode_with_more_than_512_splits():
     assert np.isfinite(got).all()
     err = row_rel_err(got[:, heads], ref[:, heads])
     assert err <= TOL, f"row rel err {err:.3e}"
+
+
+@pytest.mark.parametrize("own_stream", [True, False], ids=["own-stream", "default-stream"])
+@pytest.mark.parametrize("name,ctxlen,batch", [("C3", 1500, 2), ("C2", 700, 3)])
+def test_host_step_equals_the_device_step(name, ctxlen, batch, own_stream):
+    """starkv_decode_step_host (host inputs in one pinned block, fused step, result back on the host) leaves the same
+    cache bytes and returns the same output bits as starkv_decode_step on device buffers; on the default stream it makes
+    the two host calls instead and must agree as well.  Called three times: the staging block is reused; the last call's
+    `out_host` is pageable memory."""
+    from tests.gpu_util import dev, f16
+    cfg = synth.make_config(name, context=ctxlen, batch=batch)
+    lens0 = np.array([ctxlen - 1 - 29 * b for b in range(batch)], np.int32)
+    lens1 = lens0 + 1
+    cache = build_cache(cfg, seq_lens=lens1)
+    bk, bv = synth.make_factors(cfg)
+    q = synth.make_q(cfg, batch=batch)
+    dk_in, dv_in = cfg.head_dim, cfg.n_kv_heads * cfg.head_dim
+    ak, av = synth.make_append_factors(cfg, dk_in, dv_in)
+    kn, vn = synth.make_append_inputs(cfg, batch, mode="dense")
+    k2, v2 = np.ascontiguousarray(kn.reshape(batch, -1)), np.ascontiguousarray(vn.reshape(batch, -1))
+    seq_ids, positions = np.arange(batch, dtype=np.int32), lens0.copy()
+    table = cache["table"].astype(np.int32)
+    stream = torch.cuda.Stream() if own_stream else None
+    ctx = sk.create_from_config(cfg, stream=stream) if own_stream else sk.create_from_config(cfg)
+    mp = table.shape[1]
+    wsb = sk.starkv_workspace_bytes(ctx, batch, mp)
+    awsb = max(sk.starkv_append_workspace_bytes(ctx, batch), sk.starkv_append_host_workspace_bytes(ctx, batch, k2.shape[1], v2.shape[1]))
+    ws, aws = torch.empty(wsb, dtype=torch.uint8, device="cuda"), torch.empty(awsb, dtype=torch.uint8, device="cuda")
+    d = dict(table=dev(table), ak=f16(ak), av=f16(av), bk=f16(bk), bv=f16(bv))
+    torch.cuda.synchronize()
+    # device step
+    pool_d = dev(cache["pool"])
+    out_d = torch.zeros((batch, cfg.n_q_heads, cfg.head_dim), dtype=torch.float16, device="cuda")
+    dd = dict(seq=dev(seq_ids), pos=dev(positions), k=f16(k2), v=f16(v2), q=f16(q), lens=dev(lens1))
+    torch.cuda.synchronize()
+    sk.starkv_decode_step(ctx, pool_d, d["table"], mp, dd["seq"], dd["pos"], batch, dd["k"], k2.shape[1], cfg.head_dim,
+                          dk_in, dd["v"], v2.shape[1], dv_in, d["ak"], d["av"], aws, awsb, dd["q"], dd["lens"], d["bk"], d["bv"],
+                          ws, wsb, out_d)
+    torch.cuda.synchronize()
+    # host step, twice
+    hk = torch.from_numpy(k2.view(np.int16)).pin_memory()
+    hv = torch.from_numpy(v2.view(np.int16)).pin_memory()
+    hq = torch.from_numpy(np.ascontiguousarray(q).view(np.int16)).pin_memory()
+    hseq, hpos, hlens = (torch.from_numpy(a.copy()).pin_memory() for a in (seq_ids, positions, lens1))
+    for it in range(3):
+        pool_h = dev(cache["pool"])
+        hout = torch.zeros((batch, cfg.n_q_heads, cfg.head_dim), dtype=torch.float16)
+        if it < 2:      # page-locked: the kernel writes it directly; pageable (last pass): through the staging block
+            hout = hout.pin_memory()
+        torch.cuda.synchronize()
+        sk.starkv_decode_step_host(ctx, pool_h, d["table"], mp, hseq, hpos, batch, hk, k2.shape[1], cfg.head_dim, dk_in, hv,
+                                   v2.shape[1], dv_in, d["ak"], d["av"], aws, awsb, hq, hlens, d["bk"], d["bv"], ws, wsb, hout)
+        torch.cuda.synchronize()
+        assert torch.equal(pool_h, pool_d)
+        assert torch.equal(hout.view(torch.int16), out_d.cpu().view(torch.int16))

@@ -602,3 +602,64 @@ def test_host_step_equals_the_device_step(name, ctxlen, batch, own_stream):
         torch.cuda.synchronize()
         assert torch.equal(pool_h, pool_d)
         assert torch.equal(hout.view(torch.int16), out_d.cpu().view(torch.int16))
+
+
+def test_host_step_in_hidden_state_mode_and_its_error_paths():
+    """Hidden-state mode (section 3.2: one activation row x per token feeds both projections): v_new_host is
+    the same pointer as k_new_host and is staged once.  Same cache bytes and output bits as the device step.  Then the
+    argument checks: a missing pointer, a workspace one byte short, a zero batch."""
+    from tests.gpu_util import dev, f16
+    batch, ctxlen = 2, 900
+    cfg = synth.make_config("C3", context=ctxlen, batch=batch)
+    lens0 = np.array([ctxlen - 1, ctxlen - 70], np.int32)
+    lens1 = lens0 + 1
+    cache = build_cache(cfg, seq_lens=lens1)
+    bk, bv = synth.make_factors(cfg)
+    q = synth.make_q(cfg, batch=batch)
+    dm = cfg.d_model
+    ak, av = synth.make_append_factors(cfg, dm, dm)
+    x, _ = synth.make_append_inputs(cfg, batch, mode="hidden")
+    x = np.ascontiguousarray(x)
+    seq_ids, positions = np.arange(batch, dtype=np.int32), lens0.copy()
+    table = cache["table"].astype(np.int32)
+    stream = torch.cuda.Stream()
+    ctx = sk.create_from_config(cfg, stream=stream)
+    mp = table.shape[1]
+    wsb = sk.starkv_workspace_bytes(ctx, batch, mp)
+    awsb = max(sk.starkv_append_workspace_bytes(ctx, batch), sk.starkv_append_host_workspace_bytes(ctx, batch, dm, dm))
+    ws, aws = torch.empty(wsb, dtype=torch.uint8, device="cuda"), torch.empty(awsb, dtype=torch.uint8, device="cuda")
+    d = dict(table=dev(table), ak=f16(ak), av=f16(av), bk=f16(bk), bv=f16(bv), seq=dev(seq_ids), pos=dev(positions), x=f16(x),
+             q=f16(q), lens=dev(lens1))
+    pool_d, pool_h = dev(cache["pool"]), dev(cache["pool"])
+    out_d = torch.zeros((batch, cfg.n_q_heads, cfg.head_dim), dtype=torch.float16, device="cuda")
+    torch.cuda.synchronize()
+    sk.starkv_decode_step(ctx, pool_d, d["table"], mp, d["seq"], d["pos"], batch, d["x"], dm, 0, dm, d["x"], dm, dm, d["ak"], d["av"],
+                          aws, awsb, d["q"], d["lens"], d["bk"], d["bv"], ws, wsb, out_d)
+    torch.cuda.synchronize()
+    hx = torch.from_numpy(x.view(np.int16)).pin_memory()
+    hq = torch.from_numpy(np.ascontiguousarray(q).view(np.int16)).pin_memory()
+    hseq, hpos, hlens = (torch.from_numpy(a.copy()).pin_memory() for a in (seq_ids, positions, lens1))
+    hout = torch.zeros((batch, cfg.n_q_heads, cfg.head_dim), dtype=torch.float16).pin_memory()
+
+    def call(**kw):
+        a = dict(pool=pool_h, table=d["table"], seq=hseq, pos=hpos, batch=batch, k=hx, v=hx, aws=aws, awsb=awsb, q=hq, lens=hlens,
+                 ws=ws, wsb=wsb, out=hout)
+        a.update(kw)
+        sk.starkv_decode_step_host(ctx, a["pool"], a["table"], mp, a["seq"], a["pos"], a["batch"], a["k"], dm, 0, dm, a["v"], dm, dm,
+                                   d["ak"], d["av"], a["aws"], a["awsb"], a["q"], a["lens"], d["bk"], d["bv"], a["ws"], a["wsb"],
+                                   a["out"])
+
+    call()
+    torch.cuda.synchronize()
+    assert torch.equal(pool_h, pool_d)
+    assert torch.equal(hout.view(torch.int16), out_d.cpu().view(torch.int16))
+    need_a = sk.starkv_append_host_workspace_bytes(ctx, batch, dm, dm)
+    for kw, code in ((dict(q=None), sk.STARKV_ERR_INVALID_ARG), (dict(out=None), sk.STARKV_ERR_INVALID_ARG),
+                     (dict(seq=None), sk.STARKV_ERR_INVALID_ARG), (dict(batch=0), sk.STARKV_ERR_INVALID_ARG),
+                     (dict(awsb=need_a - 1), sk.STARKV_ERR_WORKSPACE), (dict(wsb=wsb - 1), sk.STARKV_ERR_WORKSPACE)):
+        with pytest.raises(sk.StarkvError) as e:
+            call(**kw)
+        assert e.value.code == code, kw
+    call()      # and the context still works after the refused calls
+    torch.cuda.synchronize()
+    assert torch.equal(hout.view(torch.int16), out_d.cpu().view(torch.int16))

@@ -22,6 +22,7 @@ constexpr int APS_ZR_MAX = APS_SM_FLOATS * 2;                                // 
 struct AppendSmallArgs {
   int n_new, n_key_tiles, n_tiles, n_part;
   int x_vec;      // both inputs: 16-byte aligned rows and d_in % 8 == 0
+  int fused;      // host side only: A1-A4 in this launch (else A1 here, then append_write_kernel reads the partials)
   const __half* k_new;
   long long k_row_stride, k_head_stride;
   int d_in_k;

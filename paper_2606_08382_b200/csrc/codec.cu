@@ -629,6 +629,7 @@ void sk_append_small_args(const starkv_ctx* ctx, AppendSmallArgs* a, void* pool,
   a->A_k = (const __half*)A_k; a->A_v = (const __half*)A_v; a->zp = (float*)ws;
   a->seq_ids = seq_ids; a->positions = positions; a->table = table; a->max_pages = max_pages; a->pool = (uint8_t*)pool;
   a->tickets = ctx->tickets + SK_TICKETS;
+  a->fused = 1;
   a->x_vec = (((uintptr_t)k_new | (uintptr_t)v_new) & 15) == 0 && ((k_row_stride | k_head_stride | v_row_stride) & 7) == 0 &&
              ((d_in_k | d_in_v) & 7) == 0;
 }
@@ -641,6 +642,20 @@ int sk_append_small_fused(const starkv_ctx* ctx, int n_new, int n_part, int limi
   int widest = L.rank_v;
   for (int h = 0; h < L.n_kv_heads; ++h) widest = L.rank_k[h] > widest ? L.rank_k[h] : widest;
   return (long long)n_new * widest * n_part <= limit;
+}
+
+// A2-A4 after a launch that ran append_small_body<false> with these arguments (the step's pre kernel): quantise, pack
+// and write from the K-split partials.
+int sk_append_small_write(starkv_ctx* ctx, const AppendSmallArgs* a) {
+  const StarkvLayout& L = ctx->L;
+  const size_t smem = ((size_t)((L.sum_rank_k + L.rank_v + 7) & ~7) + 8 * (size_t)L.rank_v) * 2;
+  if ((int)smem > ctx->smem_optin) return STARKV_ERR_UNSUPPORTED;
+  if (smem > 48 * 1024) SK_CUDA_CHECK(ctx, sk_need_smem(ctx, append_write_kernel, (int)smem));
+  SK_PREFER_SMEM(ctx, append_write_kernel);
+  SK_CUDA_CHECK(ctx, sk_launch(ctx, append_write_kernel, dim3(a->n_new), dim3(AW_THREADS), smem, L, (const __half*)a->zp,
+                               (const float*)a->zp, a->n_part, a->n_new, a->seq_ids, a->positions, a->table, a->max_pages, a->pool));
+  ctx->last_append = "append_small_kernel";
+  return STARKV_OK;
 }
 
 int sk_append(starkv_ctx* ctx, void* pool, const int32_t* table, int max_pages, const int32_t* seq_ids,

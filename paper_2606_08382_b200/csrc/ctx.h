@@ -153,6 +153,7 @@ int sk_append_gemm(starkv_ctx* ctx, void* pool, const int32_t* table, int max_pa
                    const void* v_new, int64_t v_row_stride, int d_in_v, const void* A_k, const void* A_v, void* z);
 int sk_append_small_ok(const starkv_ctx* ctx, int n_new);   // the one-launch append covers n_new tokens
 int sk_append_small_fused(const starkv_ctx* ctx, int n_new, int n_part, int limit);   // A1-A4 in one launch (else A1, then append_write_kernel)
+int sk_append_small_write(starkv_ctx* ctx, const AppendSmallArgs* a);   // A2-A4 from the partials of an un-fused A1 launch
 void sk_append_small_args(const starkv_ctx* ctx, AppendSmallArgs* a, void* pool, const int32_t* table, int max_pages,
                           const int32_t* seq_ids, const int32_t* positions, int n_new, const void* k_new, int64_t k_row_stride,
                           int64_t k_head_stride, int d_in_k, const void* v_new, int64_t v_row_stride, int d_in_v,

@@ -292,6 +292,7 @@ __global__ void __launch_bounds__(256) qproj_kernel(const __grid_constant__ Star
 // image, the rest run the one-launch append (append_small.cuh).  Both finish before the decode kernel's
 // griddepcontrol.wait returns.
 static_assert(APS_THREADS == 256 && APS_SM_FLOATS >= 256 * 4, "the two bodies share a block size and the shared memory");
+template <bool FUSED>
 __global__ void __launch_bounds__(256) step_pre_fast_kernel(const __grid_constant__ StarkvLayout L,
                                                             const __grid_constant__ DecodePlan PL, const __half* __restrict__ q,
                                                             const __half* __restrict__ B_k, uint8_t* __restrict__ qimg_all,
@@ -304,7 +305,7 @@ __global__ void __launch_bounds__(256) step_pre_fast_kernel(const __grid_constan
     qproj_body(L, PL, q, B_k, qimg_all, qimg_stride, i % L.n_kv_heads, i / L.n_kv_heads, reinterpret_cast<float (*)[4]>(sm));
   } else {
     const int j = i - n_qp;
-    append_small_body<true>(L, a, j % a.n_tiles, j / a.n_tiles, sm);
+    append_small_body<FUSED>(L, a, j % a.n_tiles, j / a.n_tiles, sm);
   }
 }
 
@@ -1464,9 +1465,17 @@ int sk_decode_fast(starkv_ctx* ctx, const void* q, const void* pool, const int32
   uint8_t* qimg = (uint8_t*)ws + w.qimg_off;
   if (app) {
     const int n_qp = L.n_kv_heads * batch;
-    SK_PREFER_SMEM(ctx, step_pre_fast_kernel);
-    SK_CUDA_CHECK(ctx, sk_launch(ctx, step_pre_fast_kernel, dim3(n_qp + app->n_tiles * app->n_part), dim3(256), 0, L, ctx->plan,
-                                 (const __half*)q, (const __half*)B_k, qimg, w.qimg_stride, n_qp, *app));
+    if (app->fused) {
+      SK_PREFER_SMEM(ctx, step_pre_fast_kernel<true>);
+      SK_CUDA_CHECK(ctx, sk_launch(ctx, step_pre_fast_kernel<true>, dim3(n_qp + app->n_tiles * app->n_part), dim3(256), 0, L,
+                                   ctx->plan, (const __half*)q, (const __half*)B_k, qimg, w.qimg_stride, n_qp, *app));
+    } else {   // projection partials with the query image, then the quantiser / paged write as a launch of its own
+      SK_PREFER_SMEM(ctx, step_pre_fast_kernel<false>);
+      SK_CUDA_CHECK(ctx, sk_launch(ctx, step_pre_fast_kernel<false>, dim3(n_qp + app->n_tiles * app->n_part), dim3(256), 0, L,
+                                   ctx->plan, (const __half*)q, (const __half*)B_k, qimg, w.qimg_stride, n_qp, *app));
+      const int rw = sk_append_small_write(ctx, app);
+      if (rw) return rw;
+    }
   } else {
     SK_PREFER_SMEM(ctx, qproj_kernel);
     SK_CUDA_CHECK(ctx, sk_launch(ctx, qproj_kernel, dim3(L.n_kv_heads, batch), dim3(256), 0, L, ctx->plan, (const __half*)q,
@@ -1500,6 +1509,6 @@ int sk_decode_fast(starkv_ctx* ctx, const void* q, const void* pool, const int32
     ctx->timing_valid = 1;
   }
   const int rc = sk_launch_combine(ctx, parts, w.n_splits, batch, B_v, out, reinterpret_cast<float*>((uint8_t*)ws + w.slice_off));
-  ctx->last_launches = 3;
+  ctx->last_launches = 3 + ((app && !app->fused) ? 1 : 0);
   return rc;
 }

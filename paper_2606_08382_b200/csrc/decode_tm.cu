@@ -231,6 +231,7 @@ __global__ void __launch_bounds__(QP_THREADS) qproj_tm_kernel(const __grid_const
 // tokens do not depend on each other, so they share one grid: blocks [0, n_qp) build the image, the rest run the small
 // append (append_small.cuh).  Both finish before the decode kernel's griddepcontrol.wait returns.
 static_assert(QP_THREADS == APS_THREADS, "the two bodies share a block size");
+template <bool FUSED>
 __global__ void __launch_bounds__(QP_THREADS) step_pre_tm_kernel(const __grid_constant__ StarkvLayout L, const __grid_constant__ TmPlan T,
                                                                  const __half* __restrict__ q, const __half* __restrict__ B_k,
                                                                  uint8_t* __restrict__ img_all, size_t img_stride, int n_qp,
@@ -244,7 +245,7 @@ __global__ void __launch_bounds__(QP_THREADS) step_pre_tm_kernel(const __grid_co
     qproj_tm_body(L, T, q, B_k, img_all, img_stride, i % nhb, i / nhb, *reinterpret_cast<QpShared*>(sm));
   } else {
     const int j = i - n_qp;
-    append_small_body<true>(L, a, j % a.n_tiles, j / a.n_tiles, sm);
+    append_small_body<FUSED>(L, a, j % a.n_tiles, j / a.n_tiles, sm);
   }
 }
 
@@ -1044,9 +1045,17 @@ int sk_decode_tm(starkv_ctx* ctx, const void* q, const void* pool, const int32_t
   uint8_t* img = (uint8_t*)ws + w.qimg_off;
   if (app) {
     const int n_qp = 2 * L.n_kv_heads * batch;
-    SK_PREFER_SMEM(ctx, step_pre_tm_kernel);
-    SK_CUDA_CHECK(ctx, sk_launch(ctx, step_pre_tm_kernel, dim3(n_qp + app->n_tiles * app->n_part), dim3(QP_THREADS), 0, L, ctx->tm,
-                                 (const __half*)q, (const __half*)B_k, img, w.qimg_stride, n_qp, *app));
+    if (app->fused) {
+      SK_PREFER_SMEM(ctx, step_pre_tm_kernel<true>);
+      SK_CUDA_CHECK(ctx, sk_launch(ctx, step_pre_tm_kernel<true>, dim3(n_qp + app->n_tiles * app->n_part), dim3(QP_THREADS), 0, L,
+                                   ctx->tm, (const __half*)q, (const __half*)B_k, img, w.qimg_stride, n_qp, *app));
+    } else {   // projection partials with the query image, then the quantiser / paged write as a launch of its own
+      SK_PREFER_SMEM(ctx, step_pre_tm_kernel<false>);
+      SK_CUDA_CHECK(ctx, sk_launch(ctx, step_pre_tm_kernel<false>, dim3(n_qp + app->n_tiles * app->n_part), dim3(QP_THREADS), 0, L,
+                                   ctx->tm, (const __half*)q, (const __half*)B_k, img, w.qimg_stride, n_qp, *app));
+      const int rw = sk_append_small_write(ctx, app);
+      if (rw) return rw;
+    }
   } else {
     SK_CUDA_CHECK(ctx, sk_launch(ctx, qproj_tm_kernel, dim3(2 * L.n_kv_heads, batch), dim3(QP_THREADS), 0, L, ctx->tm,
                                  (const __half*)q, (const __half*)B_k, img, w.qimg_stride));
@@ -1061,6 +1070,6 @@ int sk_decode_tm(starkv_ctx* ctx, const void* q, const void* pool, const int32_t
     ctx->timing_valid = 1;
   }
   const int rc = sk_launch_combine(ctx, parts, w.n_splits, batch, B_v, out, reinterpret_cast<float*>((uint8_t*)ws + w.slice_off));
-  ctx->last_launches = 3;
+  ctx->last_launches = 3 + ((app && !app->fused) ? 1 : 0);
   return rc;
 }

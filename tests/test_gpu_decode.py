@@ -441,8 +441,8 @@ def test_fused_step_equals_append_then_decode_and_the_oracle(name, ctxlen, batch
             sk.starkv_decode_step(ctx, pool, d["table"], mp, d["seq"], d["pos"], batch, d["k"], k2.shape[1], cfg.head_dim, dk_in,
                                   d["v"], v2.shape[1], dv_in, d["ak"], d["av"], aws, awsb, d["q"], d["lens"], d["bk"], d["bv"],
                                   ws, wsb, out)
-            if name in ("C3", "C5", "C2"):    # (C4's append is too large for the one-launch form: five launches)
-                assert sk.starkv_last_launches(ctx) == 3
+            # (C4's append is too large for the one-launch form: its quantiser / paged write is a fourth launch)
+            assert sk.starkv_last_launches(ctx) == (3 if name in ("C3", "C5", "C2") else 4)
         else:
             sk.starkv_append(ctx, pool, d["table"], mp, d["seq"], d["pos"], batch, d["k"], k2.shape[1], cfg.head_dim, dk_in,
                              d["v"], v2.shape[1], dv_in, d["ak"], d["av"], aws, awsb)
@@ -663,3 +663,47 @@ def test_host_step_in_hidden_state_mode_and_its_error_paths():
     call()      # and the context still works after the refused calls
     torch.cuda.synchronize()
     assert torch.equal(hout.view(torch.int16), out_d.cpu().view(torch.int16))
+
+
+def test_step_with_an_append_too_large_for_one_launch_on_the_tmem_kernel():
+    """C3 shape, six sequences, hidden-state mode (d_in = 4096: 16 K-split partials of up to 256 columns per token): the
+    one-launch append is not taken, so the step is four launches -- projection partials with the query image, the
+    quantiser / paged write, the decode kernel, the combine -- and still leaves the bytes and the output of
+    starkv_append followed by starkv_decode_attn."""
+    from tests.gpu_util import dev, f16
+    batch, ctxlen = 6, 700
+    cfg = synth.make_config("C3", context=ctxlen, batch=batch)
+    lens0 = np.array([ctxlen - 1 - 31 * b for b in range(batch)], np.int32)
+    lens1 = lens0 + 1
+    cache = build_cache(cfg, seq_lens=lens1)
+    bk, bv = synth.make_factors(cfg)
+    q = synth.make_q(cfg, batch=batch)
+    dm = cfg.d_model
+    ak, av = synth.make_append_factors(cfg, dm, dm)
+    x, _ = synth.make_append_inputs(cfg, batch, mode="hidden")
+    table = cache["table"].astype(np.int32)
+    ctx = sk.create_from_config(cfg)
+    assert sk.starkv_decode_kernel_name(ctx) == "decode_tm_kernel"
+    mp = table.shape[1]
+    wsb, awsb = sk.starkv_workspace_bytes(ctx, batch, mp), sk.starkv_append_workspace_bytes(ctx, batch)
+    ws, aws = torch.empty(wsb, dtype=torch.uint8, device="cuda"), torch.empty(awsb, dtype=torch.uint8, device="cuda")
+    d = dict(table=dev(table), ak=f16(ak), av=f16(av), bk=f16(bk), bv=f16(bv), seq=dev(np.arange(batch, dtype=np.int32)),
+             pos=dev(lens0), x=f16(np.ascontiguousarray(x)), q=f16(q), lens=dev(lens1))
+    res = []
+    for fused in (True, False, True):
+        pool = dev(cache["pool"])
+        out = torch.zeros((batch, cfg.n_q_heads, cfg.head_dim), dtype=torch.float16, device="cuda")
+        if fused:
+            sk.starkv_decode_step(ctx, pool, d["table"], mp, d["seq"], d["pos"], batch, d["x"], dm, 0, dm, d["x"], dm, dm, d["ak"],
+                                  d["av"], aws, awsb, d["q"], d["lens"], d["bk"], d["bv"], ws, wsb, out)
+            assert sk.starkv_last_launches(ctx) == 4
+        else:
+            sk.starkv_append(ctx, pool, d["table"], mp, d["seq"], d["pos"], batch, d["x"], dm, 0, dm, d["x"], dm, dm, d["ak"], d["av"],
+                             aws, awsb)
+            assert sk.starkv_last_launches(ctx) == 2
+            sk.starkv_decode_attn(ctx, d["q"], pool, d["table"], mp, d["lens"], batch, d["bk"], d["bv"], ws, wsb, out)
+        torch.cuda.synchronize()
+        res.append((pool.cpu().numpy(), out.cpu().numpy()))
+    assert not np.array_equal(res[0][0], cache["pool"])          # the append did write
+    for p, o in res[1:]:
+        assert np.array_equal(p, res[0][0]) and np.array_equal(o.view(np.uint16), res[0][1].view(np.uint16))

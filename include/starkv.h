@@ -149,9 +149,11 @@ int starkv_decode_attn_latent(starkv_ctx* ctx, const void* q, const void* page_p
  * seq_ids[b] / positions[b]) followed by starkv_decode_attn over seq_lens (which already count the new token), with
  * the same arguments, meanings and results as those two calls made back to back on the context's stream -- the cache
  * bytes and `out` are bit-identical to theirs.  What it adds is launch fusion: where a tensor-core decode kernel covers
- * the descriptor, batch <= 16 and the one-launch append applies (batch x widest rank x K splits <= 8192), the append
- * (projection, quantiser, paged write) and the latent-space query image run in ONE launch, so the step is three
- * launches (pre, decode, combine) instead of five.  Elsewhere it makes the two calls.  append_workspace >= starkv_append_workspace_bytes(ctx, batch), workspace >= starkv_workspace_bytes(...);
+ * the descriptor and batch <= 16, the append's projection and the latent-space query image run in ONE launch; where
+ * the one-launch append applies as well (batch x widest rank x K splits <= 8192) that launch also holds the quantiser
+ * and the paged write, so the step is three launches (pre, decode, combine) instead of five, else the quantiser /
+ * paged write is a launch of its own (four).  Elsewhere it makes the two calls.  append_workspace >=
+ * starkv_append_workspace_bytes(ctx, batch), workspace >= starkv_workspace_bytes(...);
  * the two workspaces must not overlap.  Same error codes; on error nothing, the append only, or both may have been
  * enqueued. */
 int starkv_decode_step(starkv_ctx* ctx, void* page_pool, const int32_t* block_table, int max_pages,

@@ -150,7 +150,7 @@ int starkv_decode_attn_latent(starkv_ctx* ctx, const void* q, const void* page_p
  * the same arguments, meanings and results as those two calls made back to back on the context's stream -- the cache
  * bytes and `out` are bit-identical to theirs.  What it adds is launch fusion: where a tensor-core decode kernel covers
  * the descriptor and batch <= 16, the append's projection and the latent-space query image run in ONE launch; where
- * the one-launch append applies as well (batch x widest rank x K splits <= 8192) that launch also holds the quantiser
+ * the one-launch append applies as well (batch x widest rank x K splits <= 2048: measured faster up to there) that launch also holds the quantiser
  * and the paged write, so the step is three launches (pre, decode, combine) instead of five, else the quantiser /
  * paged write is a launch of its own (four).  Elsewhere it makes the two calls.  append_workspace >=
  * starkv_append_workspace_bytes(ctx, batch), workspace >= starkv_workspace_bytes(...);

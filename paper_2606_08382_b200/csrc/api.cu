@@ -219,9 +219,10 @@ int starkv_decode_step(starkv_ctx* ctx, void* pool, const int32_t* table, int ma
   else
     a.n_part = 0;
   if (a.n_part > 0) {
-    // The append's projection shares the query image's launch.  Where the serial tail of the one-launch form stays short it
-    // is the whole append (three launches per step); else the quantiser / paged write follows as a launch of its own (four).
-    a.fused = sk_append_small_fused(ctx, batch, a.n_part, 8192);
+    // The append's projection shares the query image's launch.  Where the serial tail of the one-launch form stays short
+    // (<= 2K partial sums: measured, codec.cu) it is the whole append (three launches per step); else the quantiser / paged
+    // write follows as a launch of its own (four).
+    a.fused = sk_append_small_fused(ctx, batch, a.n_part, 2048);
     if (choice == SK_VARIANT_TM) return sk_decode_tm(ctx, q, pool, table, max_pages, seq_lens, batch, B_k, B_v, ws, ws_bytes, out, &a);
     return sk_decode_fast(ctx, q, pool, table, max_pages, seq_lens, batch, B_k, B_v, ws, ws_bytes, out, &a);
   }

@@ -635,8 +635,9 @@ void sk_append_small_args(const starkv_ctx* ctx, AppendSmallArgs* a, void* pool,
 }
 
 // One launch for A1-A4 when the serial tail of a group's last CTA stays small: at most `limit` partial sums to add.
-// Measured: against A1 + append_write_kernel the single launch loses above ~2K sums (C2: 54.6 vs 52.3 us per step), but
-// inside starkv_decode_step, where it also shares its launch with the query image, it wins up to 8K (C5: 62.2 vs 66.3).
+// Measured: against A1 + append_write_kernel the single launch loses above ~2K sums, as a call of its own (C2, 4096 sums:
+// 54.6 vs 52.3 us per step) and inside starkv_decode_step, where either form shares its first launch with the query
+// image (C2 49.9 vs 47.3 us, C5 55.9 vs 54.4 per layer; C3, 1024 sums: 40.3 vs 41.0, the single launch wins).
 int sk_append_small_fused(const starkv_ctx* ctx, int n_new, int n_part, int limit) {
   const StarkvLayout& L = ctx->L;
   int widest = L.rank_v;
